@@ -1,0 +1,331 @@
+"""Pins of the CPU oracle (oracle/bem_oracle.c) against what the paper and the
+mathematics fix -- never against itself and never against the CUDA path.
+
+Citations: PAPER.md = /root/reference/PAPER.md (arXiv 1905.01341).
+  P1  sphere eigen-relations of the single/double layer (consequence of Eq. 11,
+      PAPER.md:131-134, with the exterior harmonics Y_n / r^(n+1))
+  P2  double layer of the constant 1 = -(interior solid angle)/(4 pi) on the
+      surface, -1 inside, 0 outside (Eq. 11 cases; Eq. 19)
+  P3  geometry: closedness, s_j, n_j (Eq. 17)
+  P4  exact flat-triangle weights against closed forms and brute-force quadrature
+  P5  the paper's diagonal identities (Eqs. 19-21)
+  P6  manufactured exterior field satisfies the BIE (Eq. 11)
+  P7  Dirichlet solve on the sphere returns -(n+1)/R Y_n (Eqs. 15-16)
+  P10 invariances
+"""
+import numpy as np
+import pytest
+
+import bem_inputs as bi
+import oracle
+from helpers import tri_areas_normals, interior_solid_angle, brute_triangle_integrals
+
+ETA = 2.5
+ALL = 1e30  # eta = infinity: every triangle exact
+
+
+def _angles(v):
+    return np.arccos(np.clip(v[:, 2] / np.linalg.norm(v, axis=1), -1, 1)), np.arctan2(v[:, 1], v[:, 0])
+
+
+def _rel(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+# ----------------------------------------------------------------- P3
+def test_p3_geometry_closed_and_lumped_weights():
+    for lvl in (1, 2, 3):
+        V, F = bi.icosphere(lvl)
+        assert V.shape[0] == 10 * 4 ** lvl + 2 and F.shape[0] == 20 * 4 ** lvl
+        A, N = tri_areas_normals(V, F)
+        assert np.abs((A[:, None] * N).sum(0)).max() < 1e-13           # closed surface
+        c = V[F].mean(1)
+        assert (np.einsum("ij,ij->i", N, c) > 0).all()                 # normals out of the bubble
+        s, n = oracle.v1_vertex_weights(V, F)
+        assert abs(s.sum() - A.sum()) < 1e-12 * A.sum()                 # sum s_j = sum A_k
+        assert np.abs(np.linalg.norm(n, axis=1) - 1).max() < 1e-14
+        assert (np.einsum("ij,ij->i", n, V) > 0.99).all()              # vertex normals ~ radial
+    # mesh area converges to 4 pi from below
+    V, F = bi.icosphere(4)
+    A, _ = tri_areas_normals(V, F)
+    assert 0 < 4 * np.pi - A.sum() < 0.02
+
+
+# ----------------------------------------------------------------- P4
+def test_p4_incident_weights_closed_form_square():
+    """int over the square [-a,a]^2 of 1/r seen from its centre = 8 a ln(1+sqrt 2)
+    (textbook); split the square into 4 triangles with apex at the centre."""
+    a = 0.7
+    corners = np.array([[a, a, 0], [-a, a, 0], [-a, -a, 0], [a, -a, 0]], float)
+    ctr = np.zeros(3)
+    tot = 0.0
+    for k in range(4):
+        tri = np.array([ctr, corners[k], corners[(k + 1) % 4]])
+        WS, WD = oracle.exact_weights(tri, ctr, incident_local=0)
+        assert np.all(WD == 0.0)
+        tot += WS.sum()
+    assert abs(tot - 8 * a * np.log(1 + np.sqrt(2)) / (4 * np.pi)) < 1e-14
+
+
+def test_p4_incident_weights_closed_form_general():
+    """Closed form of the Duffy integrals (derived in DESIGN.md): with a, b the
+    edge vectors from x, c = b - a, l = |c|:
+    I0 = ln[(|b| l + b.c)/(|a| l + a.c)]/l,  I1 = (|b|-|a|)/l^2 - (a.c/l^2) I0."""
+    rng = np.random.default_rng(7)
+    for _ in range(20):
+        tri = rng.normal(size=(3, 3))
+        tri[2] = tri[0] + (tri[2] - tri[0]) * rng.uniform(0.2, 3.0)     # skewed triangles too
+        for a0 in range(3):
+            x = tri[a0]
+            a = tri[(a0 + 1) % 3] - x
+            b = tri[(a0 + 2) % 3] - x
+            c = b - a
+            l = np.linalg.norm(c)
+            I0 = np.log((np.linalg.norm(b) * l + b @ c) / (np.linalg.norm(a) * l + a @ c)) / l
+            I1 = (np.linalg.norm(b) - np.linalg.norm(a)) / l ** 2 - (a @ c) / l ** 2 * I0
+            twoA = np.linalg.norm(np.cross(a, b))
+            ref = np.zeros(3)
+            ref[a0] = 0.5 * I0
+            ref[(a0 + 1) % 3] = 0.5 * (I0 - I1)
+            ref[(a0 + 2) % 3] = 0.5 * I1
+            ref *= twoA / (4 * np.pi)
+            WS, _ = oracle.exact_weights(tri, x, incident_local=a0)
+            assert np.abs(WS - ref).max() < 5e-13 * np.abs(ref).max()
+
+
+def test_p4_solid_angle_of_square_on_axis():
+    """Solid angle of the square [-a,a]^2 seen from height h on its axis:
+    4 arcsin(a^2/(a^2+h^2)) (textbook).  sum_a W^D_a = Omega/(4 pi), sign of h."""
+    a = 0.5
+    sq = np.array([[a, a, 0], [-a, a, 0], [-a, -a, 0], [a, -a, 0]], float)   # ccw seen from +z: N = +z
+    for h in (2.0, 0.3, 0.05, -0.4):
+        x = np.array([0, 0, h])
+        tot = 0.0
+        for tri in (sq[[0, 1, 2]], sq[[0, 2, 3]]):
+            _, WD = oracle.exact_weights(tri, x)
+            tot += WD.sum()
+        om = 4 * np.arcsin(a * a / (a * a + h * h)) * np.sign(h)
+        assert abs(tot - om / (4 * np.pi)) < 1e-13
+
+
+def test_p4_regular_weights_vs_brute_force():
+    rng = np.random.default_rng(11)
+    for trial in range(6):
+        tri = rng.normal(size=(3, 3))
+        cen = tri.mean(0)
+        d = np.linalg.norm(tri - cen, axis=1).max()
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        x = cen + u * d * rng.uniform(1.2, 3.0)
+        WS, WD = oracle.exact_weights(tri, x)
+        bS, bD = brute_triangle_integrals(tri, x, depth=4, ngl=10)
+        assert np.abs(WS - bS).max() < 1e-13 * np.abs(bS).max()
+        assert np.abs(WD - bD).max() < 1e-12 * max(np.abs(bD).max(), np.abs(bS).max())
+
+
+def test_p4_gauss3_is_exact_for_quadratics():
+    """The 3-point rule (2/3,1/6,1/6) integrates lambda_a lambda_b exactly:
+    int lambda_a lambda_b = A (1+delta_ab)/12; checked through the far-field limit
+    x -> infinity where G -> 1/(4 pi |x|) is constant over the triangle."""
+    tri = np.array([[0, 0, 0], [1, 0, 0], [0, 2, 0]], float)
+    x = np.array([0, 0, 1e9])
+    cS, _ = oracle.gauss3_coeffs(tri, x)
+    assert np.abs(cS * 4 * np.pi * 1e9 - 1.0 / 3.0).max() < 1e-9     # int lambda_a = A/3, A = 1
+
+
+# ----------------------------------------------------------------- P2
+@pytest.mark.parametrize("deform", [False, True])
+def test_p2_double_layer_of_one_is_solid_angle(deform):
+    V, F = bi.icosphere(2)
+    if deform:
+        V = bi.deform_radial(V, lambda t, p: 1 + 0.3 * bi.real_sph_harm(4, 2, t, p) + 0.15 * bi.real_sph_harm(6, 3, t, p))
+    y = oracle.g3_apply(V, F, None, np.ones(V.shape[0]), eta=ALL)       # = -D.1
+    om = np.array([interior_solid_angle(V, F, i) for i in range(V.shape[0])])
+    assert np.abs(-y + om / (4 * np.pi)).max() < 5e-14
+
+
+def test_p2_double_layer_inside_outside():
+    V, F = bi.icosphere(2)
+    tot = {}
+    for name, x in (("in", np.array([0.2, -0.1, 0.3])), ("out", np.array([1.5, 0.4, -0.9]))):
+        s = 0.0
+        for t in F:
+            _, WD = oracle.exact_weights(V[t], x)
+            s += WD.sum()
+        tot[name] = s
+    assert abs(tot["in"] + 1.0) < 1e-13
+    assert abs(tot["out"]) < 1e-13
+
+
+def test_p2_near_radius_residue_is_gauss_error():
+    V, F = bi.icosphere(2)
+    y = oracle.g3_apply(V, F, None, np.ones(V.shape[0]), eta=ETA)
+    om = np.array([interior_solid_angle(V, F, i) for i in range(V.shape[0])])
+    err = np.abs(-y + om / (4 * np.pi)).max()
+    assert 1e-6 < err < 5e-4        # far-field 3-pt Gauss error: 7.7e-5
+
+
+# ----------------------------------------------------------------- P1
+def test_p1_sphere_eigen_relations_converge():
+    errS, errD = [], []
+    for lvl in (2, 3):
+        V, F = bi.icosphere(lvl)
+        th, ph = _angles(V)
+        Y = bi.real_sph_harm(3, 1, th, ph)
+        yS = oracle.g3_apply(V, F, Y, None, eta=ETA)
+        errS.append(_rel(yS, Y / 7))
+        d1 = -oracle.g3_apply(V, F, None, np.ones(V.shape[0]), eta=ETA)
+        dY = -oracle.g3_apply(V, F, None, Y, eta=ETA)
+        errD.append(_rel(dY - d1 * Y, 3 * Y / 7))
+    assert errS[0] < 0.1 and errS[1] < 0.03 and errS[0] / errS[1] > 2.8     # O(h^2)
+    assert errD[0] < 0.06 and errD[1] < 0.015 and errD[0] / errD[1] > 2.8
+
+
+def test_p1_sphere_radius_scaling_and_config1_shape():
+    """S[Y_n] = R/(2n+1) Y_n: check the R factor, and config 1's expected answer
+    y ~ Y_3^1/7 - D.1 with D.1 ~ -0.458 (not -0.5: vertices are not smooth points)."""
+    c = bi.make_config(1)
+    y = oracle.g3_apply(c["V"], c["F"], c["q"], c["phi"], eta=ETA)
+    th, ph = _angles(c["V"])
+    Y = bi.real_sph_harm(3, 1, th, ph)
+    assert np.abs(y - (Y / 7 + 0.4584)).max() < 1e-2
+    V2 = 2.5 * c["V"]
+    yS1 = oracle.g3_apply(c["V"], c["F"], Y, None, eta=ETA)
+    yS2 = oracle.g3_apply(V2, c["F"], Y, None, eta=ETA)
+    assert _rel(yS2, 2.5 * yS1) < 1e-13
+
+
+# ----------------------------------------------------------------- P5
+def test_p5_v1_diagonal_identities():
+    V, F = bi.icosphere(2)
+    V = V * 1.3 + np.array([5.0, -3.0, 2.0])       # off-origin: exercises the translation-invariant form
+    N = V.shape[0]
+    y0 = oracle.v1_apply(V, F, None, np.ones(N))
+    assert np.abs(y0 - 0.5).max() < 1e-14          # sum_j M_ij = -1/2
+    s, n = oracle.v1_vertex_weights(V, F)
+    acc = np.zeros(N)
+    for a in range(3):
+        ya = oracle.v1_apply(V, F, n[:, a], V[:, a])
+        acc += n[:, a] * (ya - 0.5 * V[:, a])
+    assert np.abs(acc).max() < 1e-13               # Eq. 20 projected on n_i
+    # off-diagonal entries are Eq. 17: rebuild one row by hand
+    i = 17
+    d = V[i] - np.delete(V, i, 0)
+    r = np.linalg.norm(d, axis=1)
+    sj = np.delete(s, i); nj = np.delete(n, i, 0)
+    L = sj / (4 * np.pi * r)
+    M = sj * np.einsum("ij,ij->i", nj, d) / (4 * np.pi * r ** 3)
+    rng = np.random.default_rng(3)
+    q = rng.normal(size=N); ph = rng.normal(size=N)
+    y, Ld, Md = oracle.v1_apply(V, F, q, ph, rows=np.array([i]), return_diag=True)
+    Mii = -0.5 - M.sum()
+    Lii = n[i] @ ((M[:, None] * (np.delete(V, i, 0) - V[i]) - L[:, None] * nj).sum(0))
+    assert abs(Md[0] - Mii) < 1e-14 and abs(Ld[0] - Lii) < 1e-14
+    ref = L @ np.delete(q, i) - M @ np.delete(ph, i) + Lii * q[i] - Mii * ph[i]
+    assert abs(y[0] - ref) < 1e-13
+
+
+def test_p5_v1_sphere_convergence():
+    errs = []
+    for lvl in (2, 3):
+        V, F = bi.icosphere(lvl)
+        th, ph = _angles(V)
+        Y = bi.real_sph_harm(3, 1, th, ph)
+        errs.append(_rel(oracle.v1_apply(V, F, Y, None), Y / 7))
+    assert errs[1] < 6e-3 and errs[0] / errs[1] > 2.5
+
+
+# ----------------------------------------------------------------- P6 / P7
+def _bie_residual(lvl):
+    V, F = bi.icosphere(lvl)
+    V = V * np.array([1.0, 0.8, 1.2])              # an ellipsoid: not a sphere
+    z = np.array([[0.2, 0.1, -0.3], [-0.3, 0.2, 0.25]])
+    a = np.array([1.0, -0.6])
+    phi = np.zeros(V.shape[0]); grad = np.zeros_like(V)
+    for zk, ak in zip(z, a):
+        d = V - zk
+        r = np.linalg.norm(d, axis=1)
+        phi += ak / (4 * np.pi * r)
+        grad += -ak * d / (4 * np.pi * r[:, None] ** 3)
+    # q = dphi/dn with the smooth-surface normal of the ellipsoid (gradient of the level set)
+    g = V / np.array([1.0, 0.8, 1.2]) ** 2
+    nrm = g / np.linalg.norm(g, axis=1, keepdims=True)
+    q = np.einsum("ij,ij->i", grad, nrm)
+    c = 1.0 - oracle.g3_apply(V, F, None, np.ones(V.shape[0]), eta=ETA)      # c = 1 + D.1
+    y = oracle.g3_apply(V, F, q, phi, eta=ETA)                               # S q - D phi
+    return np.linalg.norm(y + c * phi) / np.linalg.norm(phi)
+
+
+def test_p6_manufactured_exterior_field_satisfies_bie():
+    r2, r3 = _bie_residual(2), _bie_residual(3)
+    assert r2 < 4e-2 and r3 < 1e-2 and r2 / r3 > 2.5
+
+
+def test_p7_dirichlet_solve_on_sphere():
+    errs = []
+    for lvl in (2, 3):
+        V, F = bi.icosphere(lvl)
+        th, ph = _angles(V)
+        Y = bi.real_sph_harm(1, 0, th, ph)
+        S, D = oracle.g3_dense(V, F, eta=ETA)
+        c = 1.0 + D.sum(1)
+        b = -c * Y + D @ Y
+        q = np.linalg.solve(S, b)
+        errs.append(_rel(q, -2.0 * Y))
+    assert errs[1] < 1.5e-2 and errs[0] / errs[1] > 2.5
+    # dense rows agree with the matrix-free apply
+    rng = np.random.default_rng(5)
+    qq = rng.normal(size=V.shape[0]); pp = rng.normal(size=V.shape[0])
+    assert _rel(S @ qq - D @ pp, oracle.g3_apply(V, F, qq, pp, eta=ETA)) < 1e-13
+
+
+# ----------------------------------------------------------------- P10 and friends
+def test_p10_invariances():
+    V, F = bi.icosphere(2)
+    rng = np.random.default_rng(9)
+    q = rng.normal(size=V.shape[0]); ph = rng.normal(size=V.shape[0])
+    yS = oracle.g3_apply(V, F, q, None, eta=ETA)
+    yD = oracle.g3_apply(V, F, None, ph, eta=ETA)
+    # linearity
+    assert _rel(oracle.g3_apply(V, F, 2 * q, -3 * ph, eta=ETA), 2 * yS - 3 * yD) < 1e-13
+    # rigid motion
+    Q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    if np.linalg.det(Q) < 0:
+        Q[:, 0] *= -1
+    V2 = V @ Q.T + np.array([3.0, -1.0, 7.0])
+    assert _rel(oracle.g3_apply(V2, F, q, ph, eta=ETA), yS + yD) < 1e-12
+    # scaling: S scales with a, D does not
+    assert _rel(oracle.g3_apply(3 * V, F, q, None, eta=ETA), 3 * yS) < 1e-13
+    assert _rel(oracle.g3_apply(3 * V, F, None, ph, eta=ETA), yD) < 1e-13
+    # permuting the vertex order permutes y
+    perm = rng.permutation(V.shape[0])
+    inv = np.argsort(perm)
+    Vp = V[perm]; Fp = inv[F].astype(np.int32)
+    yp = oracle.g3_apply(Vp, Fp, q[perm], ph[perm], eta=ETA)
+    assert _rel(yp, (yS + yD)[perm]) < 1e-13
+    # flipping the orientation flips the double layer only
+    Ff = F[:, [0, 2, 1]].copy()
+    assert _rel(oracle.g3_apply(V, Ff, None, ph, eta=ETA), -yD) < 1e-13
+    assert _rel(oracle.g3_apply(V, Ff, q, None, eta=ETA), yS) < 1e-13
+
+
+def test_near_set_statistics_and_row_subset():
+    V, F = bi.icosphere(3)
+    rng = np.random.default_rng(1)
+    q = rng.normal(size=V.shape[0]); ph = rng.normal(size=V.shape[0])
+    y, near = oracle.g3_apply(V, F, q, ph, eta=ETA, return_near=True)
+    assert 15.5 < near.mean() < 18.5                   # 16.9
+    rows = np.array([5, 99, 640])
+    assert np.array_equal(oracle.g3_apply(V, F, q, ph, eta=ETA, rows=rows), y[rows])
+    # eta = 2.5 vs all-exact differ by the far-field Gauss error only
+    yall = oracle.g3_apply(V, F, q, ph, eta=ALL, rows=np.arange(0, 642, 40))
+    assert 1e-6 < _rel(y[::40], yall) < 2e-3
+
+
+def test_monopole_sum_matches_definition():
+    pts, m = bi.random_cube_points(300, seed=4)
+    tg = pts[:50]
+    y = oracle.monopole_sum(pts, m, tg)
+    d = np.linalg.norm(tg[:, None, :] - pts[None, :, :], axis=2)
+    with np.errstate(divide="ignore"):
+        k = np.where(d > 0, 1.0 / (4 * np.pi * d), 0.0)
+    assert _rel(y, k @ m) < 1e-14
