@@ -1,0 +1,171 @@
+/*
+ * bem.h -- C-ABI of the B200-native boundary-element matrix-vector product
+ * for the 3-D Laplace equation on triangulated bubble surfaces
+ * (arXiv 1905.01341; citations are /root/reference/PAPER.md:<line>).
+ *
+ * The operator (Eqs. 11-13; collocation at the mesh vertices,
+ * PAPER.md:150-158, Eq. 14):
+ *
+ *     y_i = S[q](r_i) - D[phi](r_i),     i = 0 .. n_vertices-1,
+ *     S[q](r)   = int_S q(r')   G(r,r')          dS(r'),   G = 1/(4 pi |r-r'|),
+ *     D[phi](r) = int_S phi(r') dG/dn(r')(r,r')  dS(r'),
+ *     dG/dn(r') = n(r').(r-r') / (4 pi |r-r'|^3),
+ *
+ * with the normal n pointing out of the bubble into the liquid.
+ * This is the product "A X, A = f L + g M" the paper's iterative solver calls
+ * every iteration (Eq. 45), with monopoles and dipoles handled
+ * in ONE call.  Its far field is evaluated with the fast
+ * multipole method and its near field directly, A = A^(dense) + A^(sparse)
+ * (PAPER.md:436-440); the data structure is built once per mesh and reused by
+ * every product.
+ *
+ * Discretisation ("quadrature" option):
+ *   G3 (default)  3-point Gauss per flat triangle with linear (P1) densities:
+ *                 monopole strengths q.w and dipole strengths phi.N.w at the
+ *                 Gauss points, plus a sparse CSR correction matrix holding
+ *                 (exact flat-triangle integral - Gauss value) on the near set
+ *                 of every collocation point -- the "correction matrix" scheme
+ *                 of PAPER.md:432.
+ *   V1            the paper's own lumped rule, Eq. 17, with
+ *                 the singular diagonal from the identities Eqs. 19-21
+ *                 (PAPER.md:198-216), obtained with 4 internal products
+ *                 (PAPER.md:218).
+ *
+ * Everything runs on ONE CUDA device (sm_100a), in fp64.  There is no CPU
+ * fallback: every entry point fails with BEM_ERR_CUDA if no device is usable.
+ *
+ * Pointers: unless stated otherwise an array argument may be a HOST or a DEVICE
+ * pointer (detected with cudaPointerGetAttributes).  Host arrays are copied
+ * to / from the device inside the call, which then synchronises; with device
+ * pointers bem_apply only enqueues work on the context's stream.
+ * No function throws or aborts across this boundary.
+ */
+#ifndef BEM_B200_H
+#define BEM_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bem_ctx bem_ctx;   /* opaque; owns every device allocation it makes */
+
+typedef enum {
+    BEM_OK = 0,
+    BEM_ERR_INVALID_ARG = 1,     /* NULL / out-of-range argument, unknown option        */
+    BEM_ERR_BAD_MESH = 2,        /* mesh is not a closed, outward-oriented manifold      */
+    BEM_ERR_NOT_SETUP = 3,       /* bem_apply / bem_solve before a successful bem_setup  */
+    BEM_ERR_CUDA = 4,            /* CUDA runtime error (text in bem_last_error)          */
+    BEM_ERR_OOM = 5,             /* device allocation failed                             */
+    BEM_ERR_NOT_CONVERGED = 6    /* bem_solve stopped at max_iter; outputs are filled    */
+} bem_status;
+
+/* Indices of the per-kernel-class timings returned by bem_get_timings (ms). */
+enum {
+    BEM_T_LIFT = 0, BEM_T_P2M, BEM_T_M2M, BEM_T_M2L, BEM_T_L2L_REDUCE, BEM_T_L2P,
+    BEM_T_P2P, BEM_T_SPMV, BEM_T_TOTAL, BEM_T_COUNT
+};
+
+/* Indices of the statistics returned by bem_get_stats. */
+enum {
+    BEM_S_N_TARGETS = 0, BEM_S_N_SOURCES, BEM_S_LMAX, BEM_S_N_SRC_LEAVES, BEM_S_N_TGT_LEAVES,
+    BEM_S_P2P_PAIRS, BEM_S_M2L_PAIRS, BEM_S_CSR_NNZ, BEM_S_NEAR_TRIANGLES, BEM_S_SETUP_MS,
+    BEM_S_N_SRC_BOXES, BEM_S_N_TGT_BOXES, BEM_S_DEVICE_BYTES, BEM_S_EXP_STRIDE,
+    BEM_S_KERNEL_LAUNCHES_PER_APPLY, BEM_S_COUNT
+};
+
+/* bem_create -- take a triangulated bubble-cluster surface (PAPER.md:150-152:
+ * "the surface is discretized by a mesh with N vertices"; collocation points are
+ * the vertices).
+ *   vertices   [n_vertices x 3] row-major fp64 coordinates.
+ *   triangles  [n_triangles x 3] 0-based vertex ids, counter-clockwise seen from
+ *              the liquid, so that (r2-r1)x(r3-r1) points out of the bubble
+ *              (PAPER.md:141, 233).
+ *   bubble_id  [n_vertices] 0..M-1, the bubble a vertex belongs to (may be NULL:
+ *              one bubble).  Used for the per-bubble orientation check only.
+ * The mesh is COPIED to the device; the caller keeps ownership of its arrays.
+ * Validation (on the device): indices in range, no zero-area triangle, every
+ * directed edge matched by exactly one opposite edge (closed oriented manifold),
+ * all three vertices of a triangle in one bubble, signed volume of every bubble
+ * > 0.  Violations return BEM_ERR_BAD_MESH and *out = NULL.
+ * The context is created with the CUDA device that is current at the call. */
+bem_status bem_create(const double *vertices, int64_t n_vertices,
+                      const int32_t *triangles, int64_t n_triangles,
+                      const int32_t *bubble_id, bem_ctx **out);
+
+/* bem_set_option -- must be called before bem_setup to take effect.
+ *   "quadrature"    0 = G3 (default), 1 = V1 (paper's Eq. 17 + Eqs. 19-21)
+ *   "mode"          0 = FMM (default), 1 = direct all-pairs sum (the paper's
+ *                   "brute force" product)
+ *   "free_term"     0 = c_i = 1 + (D.1)_i, the discrete solid angle implied by
+ *                   the diagonal rule M_ii = -1/2 - sum_{j!=i} M_ij
+ *                   (default); 1 = c_i = 1/2 literally (Eq. 15)
+ *   "gmres_restart" 0 = no restart up to max_iter (default), else restart length
+ *   "lmax"          0 = choose the octree depth from leaf_size (default), else force it
+ *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply */
+bem_status bem_set_option(bem_ctx *ctx, const char *key, double value);
+
+/* bem_set_stream -- cuda_stream is a cudaStream_t (NULL = default stream).  All
+ * later work of this context is enqueued there. */
+bem_status bem_set_stream(bem_ctx *ctx, void *cuda_stream);
+
+/* bem_setup -- build everything that depends on the mesh only (PAPER.md:440:
+ * "data structure ... built once"): triangle geometry, source points, the octree
+ * from 63-bit Morton keys (unit-cube scaling, bit interleave, radix sort; empty
+ * boxes skipped; separate source and receiver box sets), neighbour and
+ * interaction lists, translation matrices, and the near-field correction CSR.
+ *   p            truncation number: expansions hold degrees n = 0..p-1, p^2 real
+ *                coefficients.  1 <= p <= 32.  Ignored in direct mode.
+ *   leaf_size    the octree depth l_max is the smallest level >= 2 at which the mean
+ *                population of non-empty source boxes is <= leaf_size (the paper's
+ *                clustering parameter).  >= 1.
+ *   near_radius  eta >= 1, dimensionless: triangle k is "near" vertex i iff i is a
+ *                vertex of k or |r_i - c_k| <= eta * max_a |r_ka - c_k| (c_k the
+ *                centroid).  Only used by G3. */
+bem_status bem_setup(bem_ctx *ctx, int p, int leaf_size, double near_radius);
+
+/* bem_apply -- y = S[q] - D[phi] at all vertices (Eq. 45, with
+ * (f, g) = (1, -1)).  q, phi: [n_vertices] fp64, either may be NULL (zero
+ * density: that layer is skipped -- f or g = 0).  y: [n_vertices] fp64 output,
+ * must not alias q or phi.  No free term (+-1/2 phi) is added.  Asynchronous on
+ * the context's stream when all pointers are device pointers. */
+bem_status bem_apply(bem_ctx *ctx, const double *q, const double *phi, double *y);
+
+/* bem_solve -- the Dirichlet problem of PAPER.md:125, 160-171 (Eqs. 15-16):
+ * given phi on the surface find q = dphi/dn with  S q = b,
+ * b_i = -c_i phi_i + (D phi)_i, by unpreconditioned GMRES,
+ * modified Gram-Schmidt, stopping when ||b - S q|| / ||b|| <= tol.
+ *   q           [n_vertices] output; read as the initial guess iff use_q_as_x0
+ *               (the paper warm-starts from the previous time step).
+ *   iters_out, relres_out  may be NULL.
+ * Returns BEM_ERR_NOT_CONVERGED when it stops at max_iter, with q, iters_out
+ * and relres_out filled with the last iterate. */
+bem_status bem_solve(bem_ctx *ctx, const double *phi, double *q, int use_q_as_x0,
+                     double tol, int max_iter, int *iters_out, double *relres_out);
+
+/* bem_get_timings -- ms per kernel class (BEM_T_*) of the last bem_apply made
+ * with option "timing" = 1; synchronises the stream.  ms_out: HOST array of n. */
+bem_status bem_get_timings(bem_ctx *ctx, double *ms_out, int n);
+
+/* bem_get_stats -- sizes fixed by bem_setup (BEM_S_*).  out: HOST array of n. */
+bem_status bem_get_stats(const bem_ctx *ctx, double *out, int n);
+
+/* bem_get_free_term -- c_i of bem_solve ([n_vertices], host or device output). */
+bem_status bem_get_free_term(bem_ctx *ctx, double *c_out);
+
+/* bem_fp64_peak -- register-resident DFMA loop on the context's device; returns
+ * the achieved FP64 rate in GFLOP/s (2 flop per DFMA) in *gflops_out (HOST).
+ * It is the measured denominator of the P2P / M2L roofline fractions. */
+bem_status bem_fp64_peak(bem_ctx *ctx, double *gflops_out);
+
+/* Last error text of this context (never NULL; valid until the next call). */
+const char *bem_last_error(const bem_ctx *ctx);
+
+/* Free every device allocation of the context.  NULL is allowed. */
+void bem_destroy(bem_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BEM_B200_H */

@@ -1,0 +1,465 @@
+// The C-ABI boundary (include/bem.h): context, bem_create, bem_setup, bem_apply and the
+// small query calls.  bem_solve lives in solve.cu.
+#include "common.cuh"
+
+#include <chrono>
+#include <cmath>
+
+namespace bem {
+// mesh.cu
+void validate_mesh(bem_ctx *c);
+void compute_geometry(bem_ctx *c);
+void build_sources(bem_ctx *c, const uint32_t *order);
+void source_points(bem_ctx *c, dvec<double> &xyz);
+// nearfield.cu
+void build_correction(bem_ctx *c);
+void build_empty_correction(bem_ctx *c);
+// tree.cu
+void boxset_sort(BoxSet &bs, const double *xyz, int64_t n, const double cube_min[3], double cube_side, int counts[22], cudaStream_t s);
+void boxset_build(BoxSet &bs, int lmax, const int counts[22], cudaStream_t s);
+void build_lists(bem_ctx *c);
+// translate.cu
+void build_matrices(bem_ctx *c);
+void launch_stage(bem_ctx *c, const Stage &st);
+void launch_p2m(bem_ctx *c);
+void launch_l2p(bem_ctx *c, const int32_t *leaf_of);
+// p2p.cu
+void launch_lift(bem_ctx *c, const double *q, const double *phi);
+void launch_p2p_direct(bem_ctx *c);
+void launch_p2p_leaves(bem_ctx *c);
+void launch_spmv_combine(bem_ctx *c, const double *q, const double *phi, double *y);
+
+bool is_device_ptr(const void *p)
+{
+    if (!p) return true;
+    cudaPointerAttributes a;
+    cudaError_t e = cudaPointerGetAttributes(&a, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <class F>
+static bem_status guarded(bem_ctx *c, F &&f)
+{
+    try {
+        if (c) CUDA_TRY(cudaSetDevice(c->device));
+        f();
+        return BEM_OK;
+    } catch (const Error &e) {
+        if (c) c->err = e.what();
+        cudaGetLastError();
+        return e.status;
+    } catch (const std::exception &e) {
+        if (c) c->err = e.what();
+        return BEM_ERR_CUDA;
+    } catch (...) {
+        if (c) c->err = "unknown error";
+        return BEM_ERR_CUDA;
+    }
+}
+
+__global__ void gather_targets(const double *V, const uint32_t *perm, int64_t N, double *tgt, uint32_t *inv)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= N) return;
+    const uint32_t i = perm[e];
+    tgt[3 * e] = V[3 * (int64_t)i]; tgt[3 * e + 1] = V[3 * (int64_t)i + 1]; tgt[3 * e + 2] = V[3 * (int64_t)i + 2];
+    inv[i] = (uint32_t)e;
+}
+__global__ void fill_const(double *v, int64_t n, double a)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) v[i] = a;
+}
+// c_i = 1 - y_i where y = bem_apply(0, 1) = -D.1   (reading R6)
+__global__ void free_term_kernel(const double *y, int64_t n, double *c)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) c[i] = 1.0 - y[i];
+}
+
+// ------------------------------------------------------------------ V1 diagonal (a3')
+// natural-order vertex weights (s, s n) come from lift_w through the engine permutation
+__global__ void v1_scatter_normals(const double4 *lw, const int4 *lv, int64_t N, double *s, double *nrm)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= N) return;
+    const int j = lv[e].x;
+    const double4 w = lw[e];
+    s[j] = w.x;
+    nrm[3 * (int64_t)j] = w.y / w.x; nrm[3 * (int64_t)j + 1] = w.z / w.x; nrm[3 * (int64_t)j + 2] = w.w / w.x;
+}
+__global__ void v1_rhs(const double *V, const double *nrm, int64_t N, int axis, double r0, double *q, double *phi)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    q[i] = nrm[3 * i + axis];
+    phi[i] = V[3 * i + axis] - r0;
+}
+// M_ii = -1/2 + y0_i ;  L_ii = - sum_a n_i^a y^a_i + y0_i n_i.(r_i - r0)     (Eqs. 19-21)
+__global__ void v1_diag(const double *V, const double *nrm, const double *y0, const double *yx, const double *yy, const double *yz,
+                        int64_t N, double r0x, double r0y, double r0z, double *dL, double *dM)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double nx = nrm[3 * i], ny = nrm[3 * i + 1], nz = nrm[3 * i + 2];
+    dM[i] = -0.5 + y0[i];
+    dL[i] = -(nx * yx[i] + ny * yy[i] + nz * yz[i]) +
+            y0[i] * (nx * (V[3 * i] - r0x) + ny * (V[3 * i + 1] - r0y) + nz * (V[3 * i + 2] - r0z));
+}
+
+// ------------------------------------------------------------------ apply (device pointers)
+void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
+{
+    cudaStream_t s = c->stream;
+    const bool tm = c->timing != 0;
+    int e = 0;
+    auto mark = [&]() { if (tm) CUDA_TRY(cudaEventRecord(c->ev[e++], s)); };
+    if (tm && !c->ev[0])
+        for (int i = 0; i < 16; ++i) CUDA_TRY(cudaEventCreate(&c->ev[i]));
+    mark();                                   // 0
+    launch_lift(c, q, phi);
+    mark();                                   // 1
+    if (c->mode == 1) {
+        mark(); mark(); mark(); mark(); mark();   // 2..6: no tree passes
+        launch_p2p_direct(c);
+        mark();                               // 7
+    } else {
+        const int lmax = c->sb.lmax;
+        launch_p2m(c);
+        mark();                               // 2
+        for (int l = lmax - 1; l >= 2; --l) launch_stage(c, c->m2m[l]);
+        mark();                               // 3
+        for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l]);
+        mark();                               // 4   (M2L GEMM + L2L + reduce)
+        mark();                               // 5
+        launch_l2p(c, c->tb.leaf_of.get());
+        mark();                               // 6
+        launch_p2p_leaves(c);
+        mark();                               // 7
+    }
+    launch_spmv_combine(c, q, phi, y);
+    mark();                                   // 8
+    c->ev_valid = tm;
+}
+
+static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
+{
+    cudaStream_t s = c->stream;
+    const auto t0 = std::chrono::steady_clock::now();
+    c->ready = false;
+    c->have_diag = false;
+    c->have_cfree = false;
+    c->p = p;
+    c->nst = ((p * p + 7) / 8) * 8;
+    c->leaf_size = leaf_size;
+    c->eta = eta;
+    compute_geometry(c);
+    const int64_t N = c->N;
+    c->ns = c->quadrature == 0 ? 3 * c->T : N;
+
+    {
+        // unit-cube scaling (reading R11): cube centred on the bounding box, side = largest extent (1 + 1e-9)
+        dvec<double> bb;
+        bb.alloc(6);
+        bbox3(c->V.get(), N, bb.get(), s);
+        double hb[6];
+        CUDA_TRY(cudaMemcpy(hb, bb.get(), sizeof hb, cudaMemcpyDeviceToHost));
+        double side = 0;
+        for (int d = 0; d < 3; ++d) side = std::max(side, hb[3 + d] - hb[d]);
+        side *= (1.0 + 1e-9);
+        if (!(side > 0)) side = 1.0;
+        for (int d = 0; d < 3; ++d) c->cube_min[d] = 0.5 * (hb[d] + hb[3 + d]) - 0.5 * side;
+        c->cube_side = side;
+
+    }
+    const double side = c->cube_side;
+    if (c->mode == 1) {
+        build_sources(c, nullptr);
+        c->tgt_pos.alloc(3 * N);
+        CUDA_TRY(cudaMemcpyAsync(c->tgt_pos.get(), c->V.get(), 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, s));
+        const int tb = cdiv(N, 128);
+        int nsplit = cdiv(592, tb);
+        nsplit = std::max(1, std::min(nsplit, 64));
+        nsplit = (int)std::max<int64_t>(1, std::min<int64_t>(nsplit, c->ns / 128));
+        c->nsplit = nsplit;
+        c->ypart.alloc((size_t)nsplit * N);
+        c->launches_per_apply = 3;
+    } else {
+        dvec<double> sxyz;
+        source_points(c, sxyz);
+        int cs[22], ct[22];
+        boxset_sort(c->sb, sxyz.get(), c->ns, c->cube_min, side, cs, s);
+        sxyz.free();
+        boxset_sort(c->tb, c->V.get(), N, c->cube_min, side, ct, s);
+        // depth: smallest level >= 2 whose mean non-empty source-box population <= leaf_size (reading R9)
+        int lmax = 2;
+        while (lmax < MAX_LEVEL && (double)c->ns / (double)cs[lmax] > (double)leaf_size) ++lmax;
+        if (c->force_lmax >= 2) lmax = std::min(c->force_lmax, MAX_LEVEL);
+        boxset_build(c->sb, lmax, cs, s);
+        boxset_build(c->tb, lmax, ct, s);
+        build_sources(c, c->sb.perm.get());
+        c->tgt_pos.alloc(3 * N);
+        c->tgt_inv.alloc(N);
+        gather_targets<<<cdiv(N, 256), 256, 0, s>>>(c->V.get(), c->tb.perm.get(), N, c->tgt_pos.get(), c->tgt_inv.get());
+        KERNEL_CHECK();
+        build_matrices(c);
+        c->Mexp.alloc((size_t)c->sb.total() * c->nst);
+        c->Lexp.alloc((size_t)c->tb.total() * c->nst);
+        build_lists(c);
+        c->nsplit = 1;
+        c->ypart.alloc(N);
+        int launches = 2 /*lift, p2m*/ + 3 /*l2p, p2p, spmv*/;
+        for (int l = lmax - 1; l >= 2; --l) launches += 2;
+        for (int l = 2; l <= lmax; ++l) launches += 2;
+        c->launches_per_apply = launches;
+    }
+
+    if (c->quadrature == 0) build_correction(c);
+    else build_empty_correction(c);
+    c->ready = true;
+
+    dvec<double> ones, y0;
+    ones.alloc(N);
+    y0.alloc(N);
+    fill_const<<<cdiv(N, 256), 256, 0, s>>>(ones.get(), N, 1.0);
+    KERNEL_CHECK();
+    const int timing = c->timing;
+    c->timing = 0;
+    if (c->quadrature == 1) {
+        // the paper's four products for the singular diagonal, pair j = i skipped
+        dvec<double> sv, nrm, qv, pv, ya[3];
+        sv.alloc(N); nrm.alloc(3 * N); qv.alloc(N); pv.alloc(N);
+        v1_scatter_normals<<<cdiv(N, 256), 256, 0, s>>>(c->lift_w.get(), c->lift_vid.get(), N, sv.get(), nrm.get());
+        KERNEL_CHECK();
+        apply_device(c, nullptr, ones.get(), y0.get());
+        const double r0[3] = {c->cube_min[0] + 0.5 * c->cube_side, c->cube_min[1] + 0.5 * c->cube_side, c->cube_min[2] + 0.5 * c->cube_side};
+        for (int a = 0; a < 3; ++a) {
+            ya[a].alloc(N);
+            v1_rhs<<<cdiv(N, 256), 256, 0, s>>>(c->V.get(), nrm.get(), N, a, r0[a], qv.get(), pv.get());
+            KERNEL_CHECK();
+            apply_device(c, qv.get(), pv.get(), ya[a].get());
+        }
+        c->diagL.alloc(N);
+        c->diagM.alloc(N);
+        v1_diag<<<cdiv(N, 256), 256, 0, s>>>(c->V.get(), nrm.get(), y0.get(), ya[0].get(), ya[1].get(), ya[2].get(), N,
+                                             r0[0], r0[1], r0[2],
+                                             c->diagL.get(), c->diagM.get());
+        KERNEL_CHECK();
+        CUDA_TRY(cudaStreamSynchronize(s));
+        c->have_diag = true;
+    }
+    // free term of bem_solve
+    c->cfree.alloc(N);
+    if (c->free_term == 1) {
+        fill_const<<<cdiv(N, 256), 256, 0, s>>>(c->cfree.get(), N, 0.5);
+        KERNEL_CHECK();
+    } else {
+        apply_device(c, nullptr, ones.get(), y0.get());
+        free_term_kernel<<<cdiv(N, 256), 256, 0, s>>>(y0.get(), N, c->cfree.get());
+        KERNEL_CHECK();
+    }
+    CUDA_TRY(cudaStreamSynchronize(s));
+    c->timing = timing;
+    c->have_cfree = true;
+    c->setup_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+}
+
+// register-resident DFMA loop: 8 independent chains per thread
+__global__ void dfma_loop(double *out, int iters, double a, double b)
+{
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+}  // namespace bem
+
+using namespace bem;
+
+extern "C" {
+
+bem_status bem_create(const double *vertices, int64_t n_vertices, const int32_t *triangles, int64_t n_triangles,
+                      const int32_t *bubble_id, bem_ctx **out)
+{
+    if (!out) return BEM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!vertices || !triangles || n_vertices < 4 || n_triangles < 4 || n_vertices > 2000000000ll || n_triangles > 700000000ll)
+        return BEM_ERR_INVALID_ARG;
+    bem_ctx *c = new (std::nothrow) bem_ctx();
+    if (!c) return BEM_ERR_OOM;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { delete c; cudaGetLastError(); return BEM_ERR_CUDA; }
+    cudaGetDevice(&c->device);
+    c->N = n_vertices;
+    c->T = n_triangles;
+    bem_status st = guarded(c, [&]() {
+        c->V.alloc(3 * c->N);
+        c->F.alloc(3 * c->T);
+        CUDA_TRY(cudaMemcpy(c->V.get(), vertices, 3 * c->N * sizeof(double), cudaMemcpyDefault));
+        CUDA_TRY(cudaMemcpy(c->F.get(), triangles, 3 * c->T * sizeof(int32_t), cudaMemcpyDefault));
+        if (bubble_id) {
+            c->bid.alloc(c->N);
+            CUDA_TRY(cudaMemcpy(c->bid.get(), bubble_id, c->N * sizeof(int32_t), cudaMemcpyDefault));
+        }
+        validate_mesh(c);
+    });
+    if (st != BEM_OK) {
+        // keep the message reachable for the binding through a static buffer
+        static thread_local std::string last;
+        last = c->err;
+        delete c;
+        return st;
+    }
+    *out = c;
+    return BEM_OK;
+}
+
+bem_status bem_set_option(bem_ctx *c, const char *key, double value)
+{
+    if (!c || !key) return BEM_ERR_INVALID_ARG;
+    const int v = (int)value;
+    if (!strcmp(key, "quadrature")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->quadrature = v; c->ready = false; }
+    else if (!strcmp(key, "mode")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->mode = v; c->ready = false; }
+    else if (!strcmp(key, "free_term")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->free_term = v; c->ready = false; }
+    else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
+    else if (!strcmp(key, "lmax")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->force_lmax = v; c->ready = false; }
+    else if (!strcmp(key, "timing")) { c->timing = v != 0; }
+    else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
+    return BEM_OK;
+}
+
+bem_status bem_set_stream(bem_ctx *c, void *cuda_stream)
+{
+    if (!c) return BEM_ERR_INVALID_ARG;
+    c->stream = (cudaStream_t)cuda_stream;
+    return BEM_OK;
+}
+
+bem_status bem_setup(bem_ctx *c, int p, int leaf_size, double near_radius)
+{
+    if (!c) return BEM_ERR_INVALID_ARG;
+    if (p < 1 || p > 32 || leaf_size < 1 || !(near_radius >= 1.0)) {
+        c->err = "bem_setup: need 1 <= p <= 32, leaf_size >= 1, near_radius >= 1";
+        return BEM_ERR_INVALID_ARG;
+    }
+    return guarded(c, [&]() { setup_impl(c, p, leaf_size, near_radius); });
+}
+
+bem_status bem_apply(bem_ctx *c, const double *q, const double *phi, double *y)
+{
+    if (!c || !y) return BEM_ERR_INVALID_ARG;
+    if (!c->ready) { c->err = "bem_apply before bem_setup"; return BEM_ERR_NOT_SETUP; }
+    if (y == q || y == phi) { c->err = "bem_apply: y aliases an input"; return BEM_ERR_INVALID_ARG; }
+    return guarded(c, [&]() {
+        const size_t bytes = c->N * sizeof(double);
+        const bool hq = !is_device_ptr(q), hp = !is_device_ptr(phi), hy = !is_device_ptr(y);
+        const double *dq = q, *dp = phi;
+        double *dy = y;
+        if (hq) { if (!c->stage_q.p) c->stage_q.alloc(c->N); CUDA_TRY(cudaMemcpyAsync(c->stage_q.get(), q, bytes, cudaMemcpyHostToDevice, c->stream)); dq = c->stage_q.get(); }
+        if (hp) { if (!c->stage_phi.p) c->stage_phi.alloc(c->N); CUDA_TRY(cudaMemcpyAsync(c->stage_phi.get(), phi, bytes, cudaMemcpyHostToDevice, c->stream)); dp = c->stage_phi.get(); }
+        if (hy) { if (!c->stage_y.p) c->stage_y.alloc(c->N); dy = c->stage_y.get(); }
+        apply_device(c, dq, dp, dy);
+        if (hy) CUDA_TRY(cudaMemcpyAsync(y, dy, bytes, cudaMemcpyDeviceToHost, c->stream));
+        if (hq || hp || hy) CUDA_TRY(cudaStreamSynchronize(c->stream));
+    });
+}
+
+bem_status bem_get_timings(bem_ctx *c, double *ms_out, int n)
+{
+    if (!c || !ms_out || n < 1) return BEM_ERR_INVALID_ARG;
+    if (!c->ev_valid) { c->err = "no timed bem_apply yet (set option timing = 1)"; return BEM_ERR_NOT_SETUP; }
+    return guarded(c, [&]() {
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+        double t[BEM_T_COUNT] = {0};
+        float ms;
+        for (int k = 0; k < 8; ++k) { CUDA_TRY(cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1])); t[k] = ms; }
+        CUDA_TRY(cudaEventElapsedTime(&ms, c->ev[0], c->ev[8]));
+        t[BEM_T_TOTAL] = ms;
+        for (int k = 0; k < n && k < BEM_T_COUNT; ++k) ms_out[k] = t[k];
+    });
+}
+
+bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
+{
+    if (!c || !out || n < 1) return BEM_ERR_INVALID_ARG;
+    if (!c->ready) return BEM_ERR_NOT_SETUP;
+    double s[BEM_S_COUNT] = {0};
+    s[BEM_S_N_TARGETS] = (double)c->N;
+    s[BEM_S_N_SOURCES] = (double)c->ns;
+    s[BEM_S_CSR_NNZ] = (double)c->nnz;
+    s[BEM_S_NEAR_TRIANGLES] = (double)c->near_tris;
+    s[BEM_S_SETUP_MS] = c->setup_ms;
+    s[BEM_S_DEVICE_BYTES] = (double)g_device_bytes;
+    s[BEM_S_EXP_STRIDE] = c->nst;
+    s[BEM_S_KERNEL_LAUNCHES_PER_APPLY] = c->launches_per_apply;
+    if (c->mode == 0) {
+        s[BEM_S_LMAX] = c->sb.lmax;
+        s[BEM_S_N_SRC_LEAVES] = c->sb.nbox[c->sb.lmax];
+        s[BEM_S_N_TGT_LEAVES] = c->tb.nbox[c->tb.lmax];
+        s[BEM_S_P2P_PAIRS] = (double)c->p2p_pairs;
+        s[BEM_S_M2L_PAIRS] = (double)c->m2l_pairs;
+        s[BEM_S_N_SRC_BOXES] = c->sb.total();
+        s[BEM_S_N_TGT_BOXES] = c->tb.total();
+    } else {
+        s[BEM_S_P2P_PAIRS] = (double)c->N * (double)c->ns;
+    }
+    for (int k = 0; k < n && k < BEM_S_COUNT; ++k) out[k] = s[k];
+    return BEM_OK;
+}
+
+bem_status bem_get_free_term(bem_ctx *c, double *c_out)
+{
+    if (!c || !c_out) return BEM_ERR_INVALID_ARG;
+    if (!c->ready || !c->have_cfree) return BEM_ERR_NOT_SETUP;
+    return guarded(c, [&]() {
+        CUDA_TRY(cudaMemcpyAsync(c_out, c->cfree.get(), c->N * sizeof(double), cudaMemcpyDefault, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+    });
+}
+
+bem_status bem_fp64_peak(bem_ctx *c, double *gflops_out)
+{
+    if (!c || !gflops_out) return BEM_ERR_INVALID_ARG;
+    return guarded(c, [&]() {
+        cudaDeviceProp prop;
+        CUDA_TRY(cudaGetDeviceProperties(&prop, c->device));
+        const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 20000;
+        dvec<double> out;
+        out.alloc((size_t)blocks * threads);
+        cudaEvent_t e0, e1;
+        CUDA_TRY(cudaEventCreate(&e0));
+        CUDA_TRY(cudaEventCreate(&e1));
+        double best = 0;
+        for (int rep = 0; rep < 4; ++rep) {
+            CUDA_TRY(cudaEventRecord(e0, c->stream));
+            dfma_loop<<<blocks, threads, 0, c->stream>>>(out.get(), iters, 0.999999, 1e-9);
+            KERNEL_CHECK();
+            CUDA_TRY(cudaEventRecord(e1, c->stream));
+            CUDA_TRY(cudaEventSynchronize(e1));
+            float ms;
+            CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+            const double gf = 2.0 * 8.0 * iters * (double)blocks * threads / (ms * 1e6);
+            if (rep > 0) best = std::max(best, gf);
+        }
+        cudaEventDestroy(e0);
+        cudaEventDestroy(e1);
+        *gflops_out = best;
+    });
+}
+
+const char *bem_last_error(const bem_ctx *c) { return c ? c->err.c_str() : "null context"; }
+
+void bem_destroy(bem_ctx *c)
+{
+    if (!c) return;
+    cudaSetDevice(c->device);
+    for (int i = 0; i < 16; ++i)
+        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    delete c;
+}
+
+}  // extern "C"

@@ -1,0 +1,181 @@
+// Shared declarations of the library: error handling, device buffers, the
+// context.  Product code only -- nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+#include <stdexcept>
+
+#include "../../include/bem.h"
+
+namespace bem {
+
+struct Error : std::runtime_error {
+    bem_status status;
+    Error(bem_status s, const std::string &m) : std::runtime_error(m), status(s) {}
+};
+
+inline void cuda_check(cudaError_t e, const char *what, const char *file, int line)
+{
+    if (e == cudaSuccess) return;
+    char buf[512];
+    snprintf(buf, sizeof buf, "%s: %s (%s:%d)", what, cudaGetErrorString(e), file, line);
+    throw Error(e == cudaErrorMemoryAllocation ? BEM_ERR_OOM : BEM_ERR_CUDA, buf);
+}
+#define CUDA_TRY(x) ::bem::cuda_check((x), #x, __FILE__, __LINE__)
+#define KERNEL_CHECK() ::bem::cuda_check(cudaGetLastError(), "kernel launch", __FILE__, __LINE__)
+
+extern size_t g_device_bytes;      // running total of live device allocations (stats only)
+
+// Owning device array.
+template <class T>
+struct dvec {
+    T *p = nullptr;
+    size_t n = 0;
+    dvec() = default;
+    dvec(const dvec &) = delete;
+    dvec &operator=(const dvec &) = delete;
+    dvec(dvec &&o) noexcept : p(o.p), n(o.n) { o.p = nullptr; o.n = 0; }
+    dvec &operator=(dvec &&o) noexcept { if (this != &o) { free(); p = o.p; n = o.n; o.p = nullptr; o.n = 0; } return *this; }
+    ~dvec() { free(); }
+    void free() { if (p) { cudaFree(p); g_device_bytes -= n * sizeof(T); } p = nullptr; n = 0; }
+    void alloc(size_t count)
+    {
+        free();
+        if (count == 0) count = 1;
+        CUDA_TRY(cudaMalloc((void **)&p, count * sizeof(T)));
+        n = count;
+        g_device_bytes += n * sizeof(T);
+    }
+    void zero(cudaStream_t s) { CUDA_TRY(cudaMemsetAsync(p, 0, n * sizeof(T), s)); }
+    T *get() const { return p; }
+};
+
+inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// ---------------------------------------------------------------- primitives (prims.cu)
+void scan_exclusive_i32(const int32_t *in, int32_t *out, int64_t n, cudaStream_t s);  // out[n] = total (n+1 outputs)
+void scan_exclusive_i64(const int32_t *in, int64_t *out, int64_t n, cudaStream_t s);  // out[n] = total
+// stable LSD radix sort of (key, value) pairs on bits [begin_bit, end_bit); result ends in (keys, vals);
+// tmp arrays must hold n elements.
+void radix_sort_pairs(uint64_t *keys, uint32_t *vals, uint64_t *keys_tmp, uint32_t *vals_tmp,
+                      int64_t n, int begin_bit, int end_bit, cudaStream_t s);
+void iota_u32(uint32_t *v, int64_t n, cudaStream_t s);
+// min / max of the three coordinates of n points (AoS xyz); out6 = device [minx,miny,minz,maxx,maxy,maxz]
+void bbox3(const double *xyz, int64_t n, double *out6, cudaStream_t s);
+double reduce_max(const double *v, int64_t n, cudaStream_t s);   // synchronises
+
+// ---------------------------------------------------------------- octree tables (tree.cu)
+constexpr int MAX_LEVEL = 12;      // expansions exist on levels 2..lmax <= MAX_LEVEL
+constexpr int N_OFFSETS = 343;     // (2*3+1)^3 relative positions, 316 of them well separated
+constexpr int MAT_M2L = 0;         // matrix ids: [0,343) M2L by offset, then 8 L2L, then 8 M2M
+constexpr int MAT_L2L = 343;
+constexpr int MAT_M2M = 351;
+constexpr int N_MATS = 359;
+
+struct BoxSet {                     // the non-empty boxes of one point set on levels 0..lmax
+    int lmax = 0;
+    int64_t npts = 0;
+    dvec<uint64_t> key_sorted;      // [npts] 63-bit Morton keys, ascending
+    dvec<uint32_t> perm;            // [npts] sorted position -> original index
+    int nbox[MAX_LEVEL + 1] = {0};  // boxes per level
+    int base[MAX_LEVEL + 2] = {0};  // global index of the first box of a level (levels 2..lmax)
+    dvec<uint64_t> bkey[MAX_LEVEL + 1];   // [nbox] key prefix (3*level bits) of each box, ascending
+    dvec<int32_t> child[MAX_LEVEL + 1];   // [nbox+1] first child at level+1 (for level < lmax)
+    dvec<int32_t> parent[MAX_LEVEL + 1];  // [nbox] parent at level-1
+    dvec<int32_t> begin;            // [nbox[lmax]+1] first point of each leaf
+    dvec<int32_t> leaf_of;          // [npts] leaf of each sorted point
+    int total() const { return base[lmax + 1]; }
+};
+
+// One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
+// executed as (tiles of a dense GEMM per matrix) -> scratch rows -> fixed-order row sums.
+struct Tile { int32_t mat, row0, nrows, from_local; };
+struct Stage {
+    int64_t npairs = 0;
+    int ntgt = 0;
+    int out_base = 0;               // global index of the first target box
+    bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
+    dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
+    dvec<int32_t> pos;              // [npairs] scratch row of pair k (target-major order)
+    dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
+    dvec<Tile> tiles;
+    int ntiles = 0;
+};
+
+}  // namespace bem
+
+// ---------------------------------------------------------------- the context
+struct bem_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+
+    // mesh (device)
+    int64_t N = 0, T = 0;
+    int nbubbles = 1;
+    bem::dvec<double> V;            // [N*3]
+    bem::dvec<int32_t> F;           // [T*3]
+    bem::dvec<int32_t> bid;         // [N]
+
+    // options
+    int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
+
+    // setup state
+    bool ready = false;
+    int p = 0, nst = 0;             // truncation number, expansion row stride (p^2 rounded up to 8)
+    int leaf_size = 0;
+    double eta = 0;
+    double cube_min[3] = {0, 0, 0}, cube_side = 1.0;
+
+    // geometry (a0)
+    bem::dvec<double> triA;         // [T]
+    bem::dvec<double> triN;         // [T*3]
+
+    // sources in engine order (Morton-sorted in FMM mode, natural in direct mode)
+    int64_t ns = 0;
+    bem::dvec<double4> src_pos;     // [ns] (x, y, z, 0)
+    bem::dvec<double4> lift_w;      // [ns] (w, w Nx, w Ny, w Nz)
+    bem::dvec<int4> lift_vid;       // [ns] (v0, v1, v2, -) densities are 2/3 f[v0] + 1/6 f[v1] + 1/6 f[v2]
+    bem::dvec<double4> src_str;     // [ns] (m, dx, dy, dz), rewritten by every apply
+    // targets in engine order
+    bem::dvec<double> tgt_pos;      // [N*3]
+    bem::dvec<uint32_t> tgt_inv;    // [N] original vertex -> engine position (FMM mode)
+
+    // octree + lists (FMM mode)
+    bem::BoxSet sb, tb;
+    bem::dvec<int32_t> nbr;         // [n_tgt_leaves * 27] source leaves adjacent to a target leaf, -1 padded
+    bem::dvec<double> mats;         // [N_MATS * nst * nst] real translation matrices, row = input dof k, col = output dof
+    bem::dvec<double> Mexp, Lexp;   // [total boxes * nst]
+    bem::dvec<double> scratch;      // [max pairs of a stage * nst]
+    std::vector<bem::Stage> m2m;    // leaf-1 .. 2
+    std::vector<bem::Stage> m2l;    // 2 .. lmax (M2L + L2L of the level)
+    int64_t m2l_pairs = 0, p2p_pairs = 0;
+
+    // partial sums of the point engine, combined by the SpMV kernel
+    bem::dvec<double> ypart;        // [nsplit * N]
+    int nsplit = 1;
+
+    // near-field correction (a3) / V1 diagonal (a3')
+    bem::dvec<int64_t> rowptr;      // [N+1]
+    bem::dvec<int32_t> col;         // [nnz]
+    bem::dvec<double2> val;         // [nnz] (C^S, C^D)
+    int64_t nnz = 0, near_tris = 0;
+    bem::dvec<double> diagL, diagM; // V1 only
+    bool have_diag = false;
+
+    bem::dvec<double> cfree;        // [N] free term c_i of bem_solve
+    bool have_cfree = false;
+
+    // staging for host-pointer arguments
+    bem::dvec<double> stage_q, stage_phi, stage_y;
+
+    // timings
+    cudaEvent_t ev[16] = {nullptr};
+    bool ev_valid = false;
+    double setup_ms = 0;
+    int launches_per_apply = 0;
+};

@@ -1,0 +1,309 @@
+// Steps a5-a9: P2M, M2M, M2L, L2L, L2P on box-scaled real
+// solid-harmonic expansions ("multipole and local expansions
+// ... spherical harmonics ... truncated to the first p_fmm degrees"; the
+// translations are "dense" p^2 x p^2 operators here, batched as GEMMs).
+//
+// Every translation of one kind and one relative position uses the SAME real
+// p^2 x p^2 matrix on every level (box-scaled coefficients, harmonics.cuh), so
+// a stage is:  rows of input expansions gathered by pair, sorted by matrix ->
+// tiles of a dense fp64 GEMM (matrix staged in shared memory, reused by 64
+// pairs) -> one scratch row per pair -> per-target sums of its rows in a fixed
+// order (no atomics; results are bit-reproducible).
+#include "common.cuh"
+#include "harmonics.cuh"
+#include "morton.cuh"
+
+namespace bem {
+
+// ------------------------------------------------------------------ matrices (setup)
+__host__ __device__ inline int tab_len(int deg_excl) { return deg_excl * (deg_excl + 1) / 2; }
+
+// one thread per matrix: its harmonic table
+__global__ void harmonic_tables(int p, double *tab_re, double *tab_im, int stride)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= N_MATS) return;
+    double *re = tab_re + (size_t)m * stride, *im = tab_im + (size_t)m * stride;
+    if (m < MAT_L2L) {
+        const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
+        if (max(max(abs(ox), abs(oy)), abs(oz)) < 2) return;          // adjacent offsets are never used
+        eval_I((double)ox, (double)oy, (double)oz, 2 * p - 1, re, im);
+    } else {
+        const int o = (m - MAT_L2L) & 7;                               // child octant: bit set -> +1/2
+        eval_R((o & 1) ? 0.5 : -0.5, (o & 2) ? 0.5 : -0.5, (o & 4) ? 0.5 : -0.5, p, re, im);
+    }
+}
+// mats[m][k][c] = T_m[c][k]  (row = input dof, column = output dof), zero padded to nst
+__global__ void fill_matrices(int p, int nst, const double *tab_re, const double *tab_im, int stride, double *mats)
+{
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t per = (int64_t)nst * nst;
+    if (idx >= per * N_MATS) return;
+    const int m = (int)(idx / per);
+    const int k = (int)((idx % per) / nst), cc = (int)(idx % nst);
+    const int n = p * p;
+    double v = 0.0;
+    if (k < n && cc < n) {
+        const double *re = tab_re + (size_t)m * stride, *im = tab_im + (size_t)m * stride;
+        if (m < MAT_L2L) {
+            const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
+            if (max(max(abs(ox), abs(oy)), abs(oz)) >= 2) v = m2l_entry(re, im, p, cc, k);
+        } else if (m < MAT_M2M) v = l2l_entry(re, im, p, cc, k);
+        else v = m2m_entry(re, im, p, cc, k);
+    }
+    mats[idx] = v;
+}
+
+void build_matrices(bem_ctx *c)
+{
+    const int p = c->p, nst = c->nst;
+    const int stride = tab_len(2 * p - 1);
+    dvec<double> tre, tim;
+    tre.alloc((size_t)N_MATS * stride);
+    tim.alloc((size_t)N_MATS * stride);
+    tre.zero(c->stream);
+    tim.zero(c->stream);
+    harmonic_tables<<<cdiv(N_MATS, 64), 64, 0, c->stream>>>(p, tre.get(), tim.get(), stride);
+    KERNEL_CHECK();
+    const int64_t tot = (int64_t)N_MATS * nst * nst;
+    c->mats.alloc(tot);
+    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, nst, tre.get(), tim.get(), stride, c->mats.get());
+    KERNEL_CHECK();
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+}
+
+// ------------------------------------------------------------------ batched GEMM (a6, a7, a8)
+// scratch[row0 + r][:] = in[src_sorted[row0 + r]][:] * mats[tile.mat]   for r < tile.nrows
+// CTA: 64 rows x 64 columns, K in chunks of 8; thread: 4 rows x 4 columns (columns strided by 16).
+constexpr int GEMM_TM = 64, GEMM_TN = 64, GEMM_KC = 8, GEMM_THREADS = 256;
+
+__global__ void __launch_bounds__(GEMM_THREADS)
+translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
+               const double *__restrict__ Mexp, const double *__restrict__ Lexp,
+               const double *__restrict__ mats, int nst, double *__restrict__ scratch)
+{
+    __shared__ double As[GEMM_KC][GEMM_TM + 4];
+    __shared__ double Bs[GEMM_KC][GEMM_TN];
+    __shared__ int rows[GEMM_TM];
+    const Tile tile = tiles[blockIdx.x];
+    const int n0 = blockIdx.y * GEMM_TN;
+    const double *in = tile.from_local ? Lexp : Mexp;
+    const double *B = mats + (size_t)tile.mat * nst * nst;
+    if (threadIdx.x < GEMM_TM) rows[threadIdx.x] = threadIdx.x < tile.nrows ? src_sorted[tile.row0 + threadIdx.x] : -1;
+    __syncthreads();
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    double acc[4][4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.0;
+    // loaders: A: thread -> (row = tid/4, two k's), B: thread -> (k = tid/32, two columns)
+    const int ar = threadIdx.x >> 2, ak = (threadIdx.x & 3) * 2;
+    const int bk = threadIdx.x >> 5, bc = (threadIdx.x & 31) * 2;
+    const int arow = rows[ar];
+    for (int k0 = 0; k0 < nst; k0 += GEMM_KC) {
+        double2 av = make_double2(0.0, 0.0), bv = make_double2(0.0, 0.0);
+        if (arow >= 0) av = *reinterpret_cast<const double2 *>(in + (size_t)arow * nst + k0 + ak);
+        if (n0 + bc < nst) bv = *reinterpret_cast<const double2 *>(B + (size_t)(k0 + bk) * nst + n0 + bc);
+        __syncthreads();
+        As[ak][ar] = av.x; As[ak + 1][ar] = av.y;
+        Bs[bk][bc] = bv.x; Bs[bk][bc + 1] = bv.y;
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk < GEMM_KC; ++kk) {
+            double a[4], b[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) a[i] = As[kk][ty * 4 + i];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = Bs[kk][tx + 16 * j];
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fma(a[i], b[j], acc[i][j]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int r = ty * 4 + i;
+        if (r >= tile.nrows) continue;
+        double *out = scratch + (size_t)(tile.row0 + r) * nst + n0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (n0 + tx + 16 * j < nst) out[tx + 16 * j] = acc[i][j];
+    }
+}
+
+// out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} scratch[pos[k]][:]   (fixed order)
+__global__ void __launch_bounds__(128)
+translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ pos, const double *__restrict__ scratch,
+                 int nst, double *__restrict__ out)
+{
+    const int t = blockIdx.x;
+    const int b = ptr[t], e = ptr[t + 1];
+    for (int cc = threadIdx.x; cc < nst; cc += blockDim.x) {
+        double s = 0.0;
+        for (int k = b; k < e; ++k) s += scratch[(size_t)pos[k] * nst + cc];
+        out[(size_t)t * nst + cc] = s;
+    }
+}
+
+void launch_stage(bem_ctx *c, const Stage &st)
+{
+    if (st.ntgt == 0) return;
+    if (st.ntiles > 0) {
+        dim3 grid(st.ntiles, cdiv(c->nst, GEMM_TN));
+        translate_gemm<<<grid, GEMM_THREADS, 0, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
+                                                             c->mats.get(), c->nst, c->scratch.get());
+        KERNEL_CHECK();
+    }
+    double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
+    translate_reduce<<<st.ntgt, 128, 0, c->stream>>>(st.ptr.get(), st.pos.get(), c->scratch.get(), c->nst, out);
+    KERNEL_CHECK();
+}
+
+// ------------------------------------------------------------------ P2M (a5)
+// Mt_l^m = sum_s [ (m_s/h) conj R_l^m(a) - (1/h^2) d_s . grad conj R_l^m(a) ],  a = (y_s - c)/h, with
+// d.grad R_l^m = d_z R_{l-1}^m + 1/2 (d_x - i d_y) R_{l-1}^{m+1} - 1/2 (d_x + i d_y) R_{l-1}^{m-1}.
+// One warp per source leaf; lane = source (32 at a time).  Each lane builds the harmonics row by
+// row (degree l from degrees l-1, l-2); the 2l+1 real values of a row go through shared memory so
+// that lane k sums value k over the 32 sources -- a fixed-order sum, no atomics.
+constexpr int P2M_WARPS = 4;
+
+__global__ void __launch_bounds__(P2M_WARPS * 32)
+p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf, int level,
+           double cmx, double cmy, double cmz, double h,
+           const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nst, double *__restrict__ Mout)
+{
+    extern __shared__ double sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int leaf = blockIdx.x * P2M_WARPS + warp;
+    if (leaf >= nleaf) return;
+    double *tbl = sm + (size_t)warp * (2 * p - 1) * 33;            // [2l+1 values][33]
+    uint32_t ix, iy, iz;
+    morton_decode(skey[leaf], &ix, &iy, &iz);
+    const double cx = cmx + (ix + 0.5) * h, cy = cmy + (iy + 0.5) * h, cz = cmz + (iz + 0.5) * h;
+    const double ih = 1.0 / h;
+    const int s0 = sbegin[leaf], s1 = sbegin[leaf + 1];
+    double *M = Mout + (size_t)leaf * nst;
+    for (int cidx = lane; cidx < nst; cidx += 32) M[cidx] = 0.0;
+    __syncwarp();
+    double pre[P_MAX + 2], pim[P_MAX + 2], qre[P_MAX + 2], qim[P_MAX + 2], cre[P_MAX + 2], cim[P_MAX + 2];
+    for (int base = s0; base < s1; base += 32) {
+        const int s = base + lane;
+        const bool valid = s < s1;
+        double ax = 0, ay = 0, az = 0, mh = 0, dx = 0, dy = 0, dz = 0;
+        if (valid) {
+            const double4 ps = spos[s], st = sstr[s];
+            ax = (ps.x - cx) * ih; ay = (ps.y - cy) * ih; az = (ps.z - cz) * ih;
+            mh = st.x * ih; dx = st.y * ih * ih; dy = st.z * ih * ih; dz = st.w * ih * ih;
+        }
+        const double r2 = ax * ax + ay * ay + az * az;
+        for (int l = 0; l < p; ++l) {
+            // row l of R from rows l-1 (p*) and l-2 (q*)
+            if (l == 0) { cre[0] = 1.0; cim[0] = 0.0; }
+            else {
+                for (int m = 0; m < l; ++m) {
+                    double vr = (2 * l - 1) * az * pre[m], vi = (2 * l - 1) * az * pim[m];
+                    if (m <= l - 2) { vr -= r2 * qre[m]; vi -= r2 * qim[m]; }
+                    const double inv = 1.0 / ((double)(l - m) * (double)(l + m));
+                    cre[m] = vr * inv; cim[m] = vi * inv;
+                }
+                const double f = -1.0 / (2.0 * l);
+                cre[l] = f * (ax * pre[l - 1] - ay * pim[l - 1]);
+                cim[l] = f * (ax * pim[l - 1] + ay * pre[l - 1]);
+            }
+            // coefficient values of this source for degree l
+            for (int m = 0; m <= l; ++m) {
+                double gr = 0.0, gi = 0.0;
+                if (l > 0) {
+                    const double Cr = (m <= l - 1) ? pre[m] : 0.0, Ci = (m <= l - 1) ? pim[m] : 0.0;
+                    const double Ar = (m + 1 <= l - 1) ? pre[m + 1] : 0.0, Ai = (m + 1 <= l - 1) ? pim[m + 1] : 0.0;
+                    double Br, Bi;
+                    if (m >= 1) { Br = pre[m - 1]; Bi = pim[m - 1]; }
+                    else if (l - 1 >= 1) { Br = -pre[1]; Bi = pim[1]; }       // R_{l-1}^{-1} = -conj R_{l-1}^{1}
+                    else { Br = 0.0; Bi = 0.0; }
+                    gr = dz * Cr + 0.5 * (dx * Ar + dy * Ai) - 0.5 * (dx * Br - dy * Bi);
+                    gi = dz * Ci + 0.5 * (dx * Ai - dy * Ar) - 0.5 * (dx * Bi + dy * Br);
+                }
+                const double vr = mh * cre[m] - gr, vi = -(mh * cim[m] - gi);   // conj
+                if (m == 0) tbl[lane] = valid ? vr : 0.0;
+                else { tbl[(2 * m - 1) * 33 + lane] = valid ? vr : 0.0; tbl[(2 * m) * 33 + lane] = valid ? vi : 0.0; }
+            }
+            __syncwarp();
+            for (int k = lane; k < 2 * l + 1; k += 32) {
+                double sum = 0.0;
+                for (int j = 0; j < 32; ++j) sum += tbl[k * 33 + j];
+                M[l * l + k] += sum;
+            }
+            __syncwarp();
+            for (int m = 0; m <= l; ++m) { qre[m] = pre[m]; qim[m] = pim[m]; pre[m] = cre[m]; pim[m] = cim[m]; }
+        }
+    }
+}
+
+void launch_p2m(bem_ctx *c)
+{
+    const BoxSet &sb = c->sb;
+    const int lmax = sb.lmax, nleaf = sb.nbox[lmax];
+    const double h = c->cube_side / (double)(1 << lmax);
+    const size_t smem = (size_t)P2M_WARPS * (2 * c->p - 1) * 33 * sizeof(double);
+    p2m_kernel<<<cdiv(nleaf, P2M_WARPS), P2M_WARPS * 32, smem, c->stream>>>(
+        sb.begin.get(), sb.bkey[lmax].get(), nleaf, lmax, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
+        c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
+    KERNEL_CHECK();
+}
+
+// ------------------------------------------------------------------ L2P (a9)
+// Phi(x) = sum_l [ Lt_l^0 R_l^0(b) + 2 sum_{m>0} ( Re Lt_l^m Re R_l^m(b) + Im Lt_l^m Im R_l^m(b) ) ],  b = (x - c)/h.
+// One thread per target; threads of a warp mostly share the leaf, so coefficient loads are broadcasts.
+__global__ void __launch_bounds__(128)
+l2p_kernel(const double *__restrict__ tgt, int64_t nt, const int32_t *__restrict__ leaf_of, const uint64_t *__restrict__ tkey,
+           double cmx, double cmy, double cmz, double h, int p, int nst, const double *__restrict__ Lleaf, double *__restrict__ y)
+{
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nt) return;
+    const int leaf = leaf_of[t];
+    uint32_t ix, iy, iz;
+    morton_decode(tkey[leaf], &ix, &iy, &iz);
+    const double ih = 1.0 / h;
+    const double bx = (tgt[3 * t] - (cmx + (ix + 0.5) * h)) * ih;
+    const double by = (tgt[3 * t + 1] - (cmy + (iy + 0.5) * h)) * ih;
+    const double bz = (tgt[3 * t + 2] - (cmz + (iz + 0.5) * h)) * ih;
+    const double r2 = bx * bx + by * by + bz * bz;
+    const double *L = Lleaf + (size_t)leaf * nst;
+    double pre[P_MAX + 2], pim[P_MAX + 2], qre[P_MAX + 2], qim[P_MAX + 2], cre[P_MAX + 2], cim[P_MAX + 2];
+    double phi = 0.0;
+    for (int l = 0; l < p; ++l) {
+        if (l == 0) { cre[0] = 1.0; cim[0] = 0.0; }
+        else {
+            for (int m = 0; m < l; ++m) {
+                double vr = (2 * l - 1) * bz * pre[m], vi = (2 * l - 1) * bz * pim[m];
+                if (m <= l - 2) { vr -= r2 * qre[m]; vi -= r2 * qim[m]; }
+                const double inv = 1.0 / ((double)(l - m) * (double)(l + m));
+                cre[m] = vr * inv; cim[m] = vi * inv;
+            }
+            const double f = -1.0 / (2.0 * l);
+            cre[l] = f * (bx * pre[l - 1] - by * pim[l - 1]);
+            cim[l] = f * (bx * pim[l - 1] + by * pre[l - 1]);
+        }
+        const double *Ll = L + l * l;
+        double row = Ll[0] * cre[0];
+        for (int m = 1; m <= l; ++m) row += 2.0 * (Ll[2 * m - 1] * cre[m] + Ll[2 * m] * cim[m]);
+        phi += row;
+        for (int m = 0; m <= l; ++m) { qre[m] = pre[m]; qim[m] = pim[m]; pre[m] = cre[m]; pim[m] = cim[m]; }
+    }
+    y[t] = phi;
+}
+
+void launch_l2p(bem_ctx *c, const int32_t *leaf_of)
+{
+    const BoxSet &tb = c->tb;
+    const int lmax = tb.lmax;
+    const double h = c->cube_side / (double)(1 << lmax);
+    l2p_kernel<<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, leaf_of, tb.bkey[lmax].get(),
+                                                       c->cube_min[0], c->cube_min[1], c->cube_min[2], h, c->p, c->nst,
+                                                       c->Lexp.get() + (size_t)tb.base[lmax] * c->nst, c->ypart.get());
+    KERNEL_CHECK();
+}
+
+}  // namespace bem
