@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the BEM matrix-vector product (BASELINE.json metric:
+"BEM MVP ms/apply vs N nodes; P2P Gpairs/s; M2L/SpMV % of FP64/HBM roofline").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+A step = one bem_apply (the whole hot path: lift, P2M, M2M, M2L, L2L, L2P, P2P, correction SpMV)
+on a seeded synthetic bubble cluster.  Default workload: config 5 of BASELINE.json (4000 bubbles,
+2,568,000 nodes, p = 12, fp64) -- the >= 2.5M-node cluster the north_star's target names.
+
+  value     ms per bem_apply with q, phi, y resident in HBM (CUDA events on the context's stream)
+  e2e       the same call with HOST buffers: H2D of q and phi, D2H of y inside the timed region
+  roofline  the dominant kernel (M2L batched GEMM) against the FP64 peak
+  cpu_baseline  the CPU oracle, timed on a bounded sample of target rows of the same workload
+
+The path does not shard (BASELINE.json: one GPU, no collectives): --gpus N runs N independent
+replicas, one per rank ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from bem_inputs.configs import make_config, sample_rows  # noqa: E402
+
+METRIC = "bem_apply_ms"
+UNIT = "ms"
+# nominal FP64 FMA peak of B200 for the "alu" roofline: 148 SMs x 64 FP64
+# FMA lanes per SM per clock x 2 flop x 1.965 GHz (clocks.max.sm)
+FP64_NOMINAL_GFLOPS = 148 * 64 * 2 * 1.965
+
+
+def workload_name(c):
+    return c["name"]
+
+
+def oracle_sample(c, seconds_target=15.0):
+    """Time the oracle, as it stands, on a bounded sample of target rows; extrapolate to all rows
+    (rows are independent: the paper extrapolates its CPU brute-force reference the same way)."""
+    import oracle
+    V, F, q, phi = c["V"], c["F"], c["q"], c["phi"]
+    N = V.shape[0]
+    cores = oracle.num_threads()
+    probe = sample_rows(c["cfg"], N, min(N, 4 * cores))
+    t0 = time.perf_counter()
+    oracle.g3_apply(V, F, q, phi, eta=c["eta"], rows=probe)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    nrows = int(min(N, max(len(probe), seconds_target / dt * len(probe))))
+    rows = sample_rows(c["cfg"], N, nrows)
+    t0 = time.perf_counter()
+    y = oracle.g3_apply(V, F, q, phi, eta=c["eta"], rows=rows)
+    dt = time.perf_counter() - t0
+    ms_full = dt * 1e3 * N / len(rows)
+    return dict(value=ms_full, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{len(rows)} of {N} target rows x all {3 * F.shape[0]} sources in {dt:.2f} s, scaled by N/rows",
+                ns_per_pair=dt * 1e9 / (len(rows) * 3.0 * F.shape[0])), rows, y
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the same config/metric; each step is one bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    c = make_config(args.config)
+    per_step = []
+    info = None
+    for i in range(args.warmup + args.steps):
+        info, _, _ = oracle_sample(c, seconds_target=args.ref_seconds)
+        if i >= args.warmup:
+            per_step.append(info["value"])
+    v = float(np.mean(per_step))
+    line = dict(impl="reference", metric=METRIC, value=v, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=v, higher_is_better=False, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", config=dict(workload=workload_name(c), p=c["p"], n_nodes=int(c["V"].shape[0])),
+                cpu_baseline=dict(value=v, unit=UNIT, cores=info["cores"], kind="oracle", sample=info["sample"]),
+                e2e=dict(value=v, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.f.read().splitlines():
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        os.unlink(self.f.name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=float(max(mx)) if mx else None,
+                    samples=len(sm), reasons=sorted(reasons))
+
+
+def run_gpu(args):
+    import torch
+    import paper_1905_01341_b200 as bem
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the BEM library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    c = make_config(args.config)
+    V, F = c["V"], c["F"]
+    N, T = V.shape[0], F.shape[0]
+    p = args.p or c["p"]
+    stream = torch.cuda.current_stream()
+
+    t0 = time.perf_counter()
+    ctx = bem.bem_create(V, F, c["bubble_id"])
+    ctx.bem_set_stream(stream.cuda_stream)
+    ctx.bem_set_option("mode", 1 if args.direct else 0)
+    if args.lmax:
+        ctx.bem_set_option("lmax", args.lmax)
+    ctx.bem_setup(p, args.leaf_size or c["leaf_size"], c["eta"])
+    torch.cuda.synchronize()
+    setup_wall_ms = (time.perf_counter() - t0) * 1e3
+    stats = ctx.bem_get_stats()
+
+    qd = torch.tensor(c["q"], device="cuda"); pd = torch.tensor(c["phi"], device="cuda")
+    yd = torch.empty_like(qd)
+    qh = torch.tensor(c["q"]).pin_memory(); ph = torch.tensor(c["phi"]).pin_memory()
+    yh = torch.empty(N, dtype=torch.float64).pin_memory()
+
+    # L2 policy: the working set of one apply (sources, expansions, lists, CSR) is far above the 126 MB L2 for
+    # configs 3-5; for the small configs a 512 MB buffer is rewritten between timed iterations.
+    flush = stats["device_bytes"] < 4 * 126e6
+    fbuf = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda") if flush else None
+
+    def timed(fn, steps):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            if fbuf is not None:
+                fbuf.fill_(1.0)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    for _ in range(max(args.warmup, 3)):
+        ctx.bem_apply(qd, pd, yd)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    total_ms = timed(lambda: ctx.bem_apply(qd, pd, yd), args.steps)
+    barrier()
+    # end to end: host (pinned) q, phi -> y host, copies inside the call
+    for _ in range(2):
+        ctx.bem_apply(qh, ph, yh)
+    barrier()
+    e2e_ms = timed(lambda: ctx.bem_apply(qh, ph, yh), args.steps)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    if dist is not None:
+        t = torch.tensor([total_ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = t.tolist()
+    ms = total_ms / args.steps
+    e2e = e2e_ms / args.steps
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # per-kernel-class breakdown (CUDA events inside bem_apply, on the context's stream), averaged
+    ctx.bem_set_option("timing", 1)
+    acc = None
+    nb = max(3, min(args.steps, 10))
+    for _ in range(nb):
+        if fbuf is not None:
+            fbuf.fill_(1.0)
+        ctx.bem_apply(qd, pd, yd)
+        t = ctx.bem_get_timings()
+        acc = t if acc is None else {k: acc[k] + t[k] for k in t}
+    ctx.bem_set_option("timing", 0)
+    tm = {k: v / nb for k, v in acc.items()}
+    dfma = ctx.bem_fp64_peak()
+    hbm = None
+    try:
+        hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        pass
+    hbm_peak, hbm_src = (hbm, "measured") if hbm else (6650.0, "fallback")
+
+    kernels = {}
+    if not args.direct:
+        m2l_flops = stats["m2l_pairs"] * 2.0 * p ** 4
+        roof = dict(kernel="m2l_gemm", bound="alu", achieved=m2l_flops / (tm["m2l"] * 1e-3) / 1e12 if tm["m2l"] > 0 else 0.0,
+                    peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", traffic=None,
+                    peak_source="nominal: 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz", measured_dfma_tflops=dfma / 1e3,
+                    algorithmic="2 p^4 flop per M2L pair x %d pairs" % stats["m2l_pairs"], ms=tm["m2l"])
+    else:
+        roof = dict(kernel="p2p_direct", bound="alu", achieved=stats["p2p_pairs"] * 20.0 / (tm["p2p"] * 1e-3) / 1e12,
+                    peak=FP64_NOMINAL_GFLOPS / 2e3, unit="Tinstr/s", traffic=None,
+                    peak_source="nominal FP64 instruction rate: 148 x 64 x 1.965 GHz", measured_dfma_tflops=dfma / 1e3,
+                    algorithmic="20 FP64 instructions per pair x %d pairs" % stats["p2p_pairs"], ms=tm["p2p"])
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    kernels["p2p"] = dict(ms=tm["p2p"], gpairs_per_s=stats["p2p_pairs"] / (tm["p2p"] * 1e-3) / 1e9 if tm["p2p"] > 0 else None,
+                          pairs=stats["p2p_pairs"])
+    spmv_bytes = 20.0 * stats["csr_nnz"] + 32.0 * N
+    kernels["spmv"] = dict(ms=tm["spmv"], gbs=spmv_bytes / (tm["spmv"] * 1e-3) / 1e9, frac_hbm=spmv_bytes / (tm["spmv"] * 1e-3) / 1e9 / hbm_peak,
+                           hbm_peak_gbs=hbm_peak, hbm_peak_source=hbm_src, bytes=spmv_bytes)
+    breakdown = {k: round(v, 4) for k, v in tm.items()}
+
+    # parity in the same run + the oracle timed beside it (bounded sample of rows)
+    cpu, rows, yo = oracle_sample(c, seconds_target=args.ref_seconds)
+    y = yd.cpu().numpy()
+    parity = float(np.linalg.norm(y[rows] - yo) / np.linalg.norm(yo))
+
+    solve = None
+    if args.solve_iters > 0:
+        qs = torch.zeros_like(qd)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        st, it, rr = ctx.bem_solve(pd, qs, tol=args.solve_tol, max_iter=args.solve_iters)
+        torch.cuda.synchronize()
+        solve = dict(ms=(time.perf_counter() - t0) * 1e3, iterations=it, relres=rr, tol=args.solve_tol, max_iter=args.solve_iters,
+                     status=bem.STATUS_NAMES[st])
+
+    line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
+                higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=workload_name(c), mode="direct" if args.direct else "fmm", p=p, n_nodes=N, n_triangles=T,
+                            n_sources=int(stats["n_sources"]), leaf_size=args.leaf_size or c["leaf_size"], eta=c["eta"],
+                            lmax=int(stats["lmax"]), parallelism="replicas only" if world > 1 else "1 gpu",
+                            l2="flushed between iterations (512 MB write)" if flush else "working set larger than L2",
+                            device_bytes=int(stats["device_bytes"])),
+                e2e=dict(value=e2e, unit=UNIT, h2d_bytes_per_step=16 * N, d2h_bytes_per_step=8 * N),
+                gpu_launches=int(stats["kernel_launches_per_apply"]) * args.steps,
+                clocks=clocks, roofline=roof, cpu_baseline=cpu, parity_rel_l2_vs_oracle=parity,
+                breakdown_ms=breakdown, kernels=kernels, setup_ms=stats["setup_ms"], setup_wall_ms=setup_wall_ms,
+                m2l_pairs=int(stats["m2l_pairs"]), solve=solve,
+                paper_context="paper Table 3 (PAPER.md:606): 1 MVP = 4.0 s at N=2,629,632, p=12, double, Xeon 5660 x12 cores + Tesla K20")
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: 2.57M nodes)")
+    ap.add_argument("--p", type=int, default=0)
+    ap.add_argument("--leaf-size", type=int, default=0)
+    ap.add_argument("--lmax", type=int, default=0)
+    ap.add_argument("--direct", action="store_true", help="direct-sum mode (configs 1-3)")
+    ap.add_argument("--solve-iters", type=int, default=30, help="also run bem_solve with this max_iter (0: skip)")
+    ap.add_argument("--solve-tol", type=float, default=1e-6)
+    ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU time budget of one oracle sample")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

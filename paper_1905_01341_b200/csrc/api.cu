@@ -20,7 +20,7 @@ void boxset_build(BoxSet &bs, int lmax, const int counts[22], cudaStream_t s);
 void build_lists(bem_ctx *c);
 // translate.cu
 void build_matrices(bem_ctx *c);
-void launch_stage(bem_ctx *c, const Stage &st);
+void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce);
 void launch_p2m(bem_ctx *c);
 void launch_l2p(bem_ctx *c, const int32_t *leaf_of);
 // p2p.cu
@@ -109,38 +109,42 @@ __global__ void v1_diag(const double *V, const double *nrm, const double *y0, co
 }
 
 // ------------------------------------------------------------------ apply (device pointers)
+void mark(bem_ctx *c, int cls)
+{
+    if (!c->timing) return;
+    if (c->ev_n == (int)c->ev.size()) {
+        cudaEvent_t e;
+        CUDA_TRY(cudaEventCreate(&e));
+        c->ev.push_back(e);
+        c->ev_cls.push_back(cls);
+    }
+    c->ev_cls[c->ev_n] = cls;
+    CUDA_TRY(cudaEventRecord(c->ev[c->ev_n++], c->stream));
+}
+
 void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
 {
-    cudaStream_t s = c->stream;
-    const bool tm = c->timing != 0;
-    int e = 0;
-    auto mark = [&]() { if (tm) CUDA_TRY(cudaEventRecord(c->ev[e++], s)); };
-    if (tm && !c->ev[0])
-        for (int i = 0; i < 16; ++i) CUDA_TRY(cudaEventCreate(&c->ev[i]));
-    mark();                                   // 0
+    c->ev_n = 0;
+    mark(c, -1);
     launch_lift(c, q, phi);
-    mark();                                   // 1
+    mark(c, BEM_T_LIFT);
     if (c->mode == 1) {
-        mark(); mark(); mark(); mark(); mark();   // 2..6: no tree passes
         launch_p2p_direct(c);
-        mark();                               // 7
+        mark(c, BEM_T_P2P);
     } else {
         const int lmax = c->sb.lmax;
         launch_p2m(c);
-        mark();                               // 2
-        for (int l = lmax - 1; l >= 2; --l) launch_stage(c, c->m2m[l]);
-        mark();                               // 3
-        for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l]);
-        mark();                               // 4   (M2L GEMM + L2L + reduce)
-        mark();                               // 5
+        mark(c, BEM_T_P2M);
+        for (int l = lmax - 1; l >= 2; --l) launch_stage(c, c->m2m[l], BEM_T_M2M, BEM_T_M2M);
+        for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l], BEM_T_M2L, BEM_T_L2L_REDUCE);
         launch_l2p(c, c->tb.leaf_of.get());
-        mark();                               // 6
+        mark(c, BEM_T_L2P);
         launch_p2p_leaves(c);
-        mark();                               // 7
+        mark(c, BEM_T_P2P);
     }
     launch_spmv_combine(c, q, phi, y);
-    mark();                                   // 8
-    c->ev_valid = tm;
+    mark(c, BEM_T_SPMV);
+    c->ev_valid = c->timing != 0;
 }
 
 static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
@@ -371,13 +375,16 @@ bem_status bem_apply(bem_ctx *c, const double *q, const double *phi, double *y)
 bem_status bem_get_timings(bem_ctx *c, double *ms_out, int n)
 {
     if (!c || !ms_out || n < 1) return BEM_ERR_INVALID_ARG;
-    if (!c->ev_valid) { c->err = "no timed bem_apply yet (set option timing = 1)"; return BEM_ERR_NOT_SETUP; }
+    if (!c->ev_valid || c->ev_n < 2) { c->err = "no timed bem_apply yet (set option timing = 1)"; return BEM_ERR_NOT_SETUP; }
     return guarded(c, [&]() {
         CUDA_TRY(cudaStreamSynchronize(c->stream));
         double t[BEM_T_COUNT] = {0};
         float ms;
-        for (int k = 0; k < 8; ++k) { CUDA_TRY(cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1])); t[k] = ms; }
-        CUDA_TRY(cudaEventElapsedTime(&ms, c->ev[0], c->ev[8]));
+        for (int k = 1; k < c->ev_n; ++k) {
+            CUDA_TRY(cudaEventElapsedTime(&ms, c->ev[k - 1], c->ev[k]));
+            if (c->ev_cls[k] >= 0 && c->ev_cls[k] < BEM_T_TOTAL) t[c->ev_cls[k]] += ms;
+        }
+        CUDA_TRY(cudaEventElapsedTime(&ms, c->ev[0], c->ev[c->ev_n - 1]));
         t[BEM_T_TOTAL] = ms;
         for (int k = 0; k < n && k < BEM_T_COUNT; ++k) ms_out[k] = t[k];
     });
@@ -457,8 +464,7 @@ void bem_destroy(bem_ctx *c)
 {
     if (!c) return;
     cudaSetDevice(c->device);
-    for (int i = 0; i < 16; ++i)
-        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     delete c;
 }
 

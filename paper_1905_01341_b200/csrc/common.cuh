@@ -55,6 +55,11 @@ struct dvec {
 };
 
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+}  // namespace bem
+struct bem_ctx;
+namespace bem {
+// with option "timing": record an event on the context's stream; the time since the previous mark is charged to cls
+void mark(bem_ctx *c, int cls);
 
 // ---------------------------------------------------------------- primitives (prims.cu)
 void scan_exclusive_i32(const int32_t *in, int32_t *out, int64_t n, cudaStream_t s);  // out[n] = total (n+1 outputs)
@@ -173,8 +178,10 @@ struct bem_ctx {
     // staging for host-pointer arguments
     bem::dvec<double> stage_q, stage_phi, stage_y;
 
-    // timings
-    cudaEvent_t ev[16] = {nullptr};
+    // timings: event k closes an interval that belongs to kernel class ev_cls[k] (-1: start)
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> ev_cls;
+    int ev_n = 0;
     bool ev_valid = false;
     double setup_ms = 0;
     int launches_per_apply = 0;

@@ -147,7 +147,7 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ po
     }
 }
 
-void launch_stage(bem_ctx *c, const Stage &st)
+void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
 {
     if (st.ntgt == 0) return;
     if (st.ntiles > 0) {
@@ -155,10 +155,12 @@ void launch_stage(bem_ctx *c, const Stage &st)
         translate_gemm<<<grid, GEMM_THREADS, 0, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
                                                              c->mats.get(), c->nst, c->scratch.get());
         KERNEL_CHECK();
+        mark(c, cls_gemm);
     }
     double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
     translate_reduce<<<st.ntgt, 128, 0, c->stream>>>(st.ptr.get(), st.pos.get(), c->scratch.get(), c->nst, out);
     KERNEL_CHECK();
+    mark(c, cls_reduce);
 }
 
 // ------------------------------------------------------------------ P2M (a5)
@@ -247,6 +249,7 @@ void launch_p2m(bem_ctx *c)
     const int lmax = sb.lmax, nleaf = sb.nbox[lmax];
     const double h = c->cube_side / (double)(1 << lmax);
     const size_t smem = (size_t)P2M_WARPS * (2 * c->p - 1) * 33 * sizeof(double);
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(p2m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     p2m_kernel<<<cdiv(nleaf, P2M_WARPS), P2M_WARPS * 32, smem, c->stream>>>(
         sb.begin.get(), sb.bkey[lmax].get(), nleaf, lmax, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
         c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
