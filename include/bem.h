@@ -103,7 +103,10 @@ bem_status bem_create(const double *vertices, int64_t n_vertices,
  *                   (default); 1 = c_i = 1/2 literally (Eq. 15)
  *   "gmres_restart" 0 = no restart up to max_iter (default), else restart length
  *   "lmax"          0 = choose the octree depth from leaf_size (default), else force it
- *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply */
+ *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply
+ *   "gemm_path"     batched translations (M2M, M2L, L2L): 0 = FP64 tensor-core tiles (DMMA; p <= 16,
+ *                   default -- measured faster), 1 = plain FP64 FMA tiles (any p).
+ *                   May be changed between products. */
 bem_status bem_set_option(bem_ctx *ctx, const char *key, double value);
 
 /* bem_set_stream -- cuda_stream is a cudaStream_t (NULL = default stream).  All
@@ -158,6 +161,11 @@ bem_status bem_get_free_term(bem_ctx *ctx, double *c_out);
  * the achieved FP64 rate in GFLOP/s (2 flop per DFMA) in *gflops_out (HOST).
  * It is the measured denominator of the P2P / M2L roofline fractions. */
 bem_status bem_fp64_peak(bem_ctx *ctx, double *gflops_out);
+
+/* bem_fp64_tensor_peak -- the same with a register-resident mma.sync m8n8k4 f64 (DMMA) loop: the
+ * FP64 tensor-core rate, GFLOP/s (512 flop per warp instruction) in *gflops_out (HOST).  north_star:
+ * "tensor cores (FP64 DMMA) only if ... measured faster" -- this is that measurement. */
+bem_status bem_fp64_tensor_peak(bem_ctx *ctx, double *gflops_out);
 
 /* Last error text of this context (never NULL; valid until the next call). */
 const char *bem_last_error(const bem_ctx *ctx);

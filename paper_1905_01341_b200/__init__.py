@@ -30,7 +30,7 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
 
 # every symbol include/bem.h declares
 EXPORTS = ["bem_create", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
-           "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_last_error", "bem_destroy"]
+           "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy"]
 
 
 class BemError(RuntimeError):
@@ -62,6 +62,7 @@ def load_library() -> ctypes.CDLL:
     lib.bem_get_stats.argtypes = [vp, vp, i32]
     lib.bem_get_free_term.argtypes = [vp, vp]
     lib.bem_fp64_peak.argtypes = [vp, ctypes.POINTER(dbl)]
+    lib.bem_fp64_tensor_peak.argtypes = [vp, ctypes.POINTER(dbl)]
     lib.bem_last_error.argtypes = [vp]
     lib.bem_last_error.restype = ctypes.c_char_p
     lib.bem_destroy.argtypes = [vp]
@@ -154,6 +155,11 @@ class Bem:
     def bem_fp64_peak(self) -> float:
         g = ctypes.c_double(0.0)
         self._check(self._lib.bem_fp64_peak(self._ctx, ctypes.byref(g)))
+        return g.value
+
+    def bem_fp64_tensor_peak(self) -> float:
+        g = ctypes.c_double(0.0)
+        self._check(self._lib.bem_fp64_tensor_peak(self._ctx, ctypes.byref(g)))
         return g.value
 
     def bem_destroy(self):

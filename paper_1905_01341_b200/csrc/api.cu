@@ -280,6 +280,50 @@ __global__ void dfma_loop(double *out, int iters, double a, double b)
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// register-resident DMMA loop: 8 independent m8n8k4 accumulator tiles per warp
+__global__ void dmma_loop(double *out, int iters, double a, double b)
+{
+    double c[8][2];
+    for (int i = 0; i < 8; ++i) { c[i][0] = threadIdx.x; c[i][1] = i; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    }
+    double s = 0;
+    for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1];
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+template <class K>
+static double time_loop(bem_ctx *c, K kern, double flop_per_thread_iter)
+{
+    cudaDeviceProp prop;
+    CUDA_TRY(cudaGetDeviceProperties(&prop, c->device));
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 20000;
+    dvec<double> out;
+    out.alloc((size_t)blocks * threads);
+    cudaEvent_t e0, e1;
+    CUDA_TRY(cudaEventCreate(&e0));
+    CUDA_TRY(cudaEventCreate(&e1));
+    double best = 0;
+    for (int rep = 0; rep < 4; ++rep) {
+        CUDA_TRY(cudaEventRecord(e0, c->stream));
+        kern<<<blocks, threads, 0, c->stream>>>(out.get(), iters, 0.999999, 1e-9);
+        KERNEL_CHECK();
+        CUDA_TRY(cudaEventRecord(e1, c->stream));
+        CUDA_TRY(cudaEventSynchronize(e1));
+        float ms;
+        CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        const double gf = flop_per_thread_iter * iters * (double)blocks * threads / (ms * 1e6);
+        if (rep > 0) best = std::max(best, gf);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return best;
+}
+
 }  // namespace bem
 
 using namespace bem;
@@ -332,6 +376,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
     else if (!strcmp(key, "lmax")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->force_lmax = v; c->ready = false; }
     else if (!strcmp(key, "timing")) { c->timing = v != 0; }
+    else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
     return BEM_OK;
 }
@@ -431,31 +476,13 @@ bem_status bem_get_free_term(bem_ctx *c, double *c_out)
 bem_status bem_fp64_peak(bem_ctx *c, double *gflops_out)
 {
     if (!c || !gflops_out) return BEM_ERR_INVALID_ARG;
-    return guarded(c, [&]() {
-        cudaDeviceProp prop;
-        CUDA_TRY(cudaGetDeviceProperties(&prop, c->device));
-        const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 20000;
-        dvec<double> out;
-        out.alloc((size_t)blocks * threads);
-        cudaEvent_t e0, e1;
-        CUDA_TRY(cudaEventCreate(&e0));
-        CUDA_TRY(cudaEventCreate(&e1));
-        double best = 0;
-        for (int rep = 0; rep < 4; ++rep) {
-            CUDA_TRY(cudaEventRecord(e0, c->stream));
-            dfma_loop<<<blocks, threads, 0, c->stream>>>(out.get(), iters, 0.999999, 1e-9);
-            KERNEL_CHECK();
-            CUDA_TRY(cudaEventRecord(e1, c->stream));
-            CUDA_TRY(cudaEventSynchronize(e1));
-            float ms;
-            CUDA_TRY(cudaEventElapsedTime(&ms, e0, e1));
-            const double gf = 2.0 * 8.0 * iters * (double)blocks * threads / (ms * 1e6);
-            if (rep > 0) best = std::max(best, gf);
-        }
-        cudaEventDestroy(e0);
-        cudaEventDestroy(e1);
-        *gflops_out = best;
-    });
+    return guarded(c, [&]() { *gflops_out = time_loop(c, dfma_loop, 2.0 * 8.0); });
+}
+
+bem_status bem_fp64_tensor_peak(bem_ctx *c, double *gflops_out)
+{
+    if (!c || !gflops_out) return BEM_ERR_INVALID_ARG;
+    return guarded(c, [&]() { *gflops_out = time_loop(c, dmma_loop, 8.0 * 512.0 / 32.0); });
 }
 
 const char *bem_last_error(const bem_ctx *c) { return c ? c->err.c_str() : "null context"; }

@@ -128,6 +128,7 @@ struct bem_ctx {
 
     // options
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
+    int gemm_path = 0;              // translations: 0 = FP64 tensor path (DMMA) where p <= 16, 1 = plain-FMA tiles
 
     // setup state
     bool ready = false;

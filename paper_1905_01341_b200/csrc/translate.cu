@@ -133,6 +133,124 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
     }
 }
 
+// ------------------------------------------------------------------ the same product on the FP64 tensor path
+// Measured on B200 (profiles/r1_02_dmma_vs_dfma.md): mma.sync m8n8k4 f64 (SASS DMMA) sustains 37.15 TFLOP/s,
+// a register-resident DFMA loop 33.8; more important, one DMMA needs ONE 8-byte shared-memory operand per
+// thread for 512 flop per warp, so the GEMM is no longer bound by shared-memory operand traffic.
+//
+// CTA = 8 warps = 64 scratch rows (pairs) of one matrix.  Each warp owns 8 rows and keeps their whole A
+// operand (8 x K input expansion coefficients, gathered straight from global memory) in registers as KS
+// m8n8k4 A-fragments; the translation matrix streams through shared memory in chunks of DM_NC columns
+// (cp.async, double buffered), shared by the 8 warps.  K is padded to 4 KS (zero A, zero B rows).
+constexpr int DM_NC = 24;            // columns of B per chunk (3 n-tiles)
+constexpr int DM_S = 28;             // row stride of a chunk in doubles: 28 = 12 (mod 16) -> conflict-free fragment loads
+constexpr int DM_THREADS = 256;
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+template <int KS>
+__global__ void __launch_bounds__(DM_THREADS)
+translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
+               const double *__restrict__ Mexp, const double *__restrict__ Lexp,
+               const double *__restrict__ mats, int nst, double *__restrict__ scratch)
+{
+    extern __shared__ __align__(16) double dm_smem[];          // [2][4 KS][DM_S]
+    constexpr int KP = 4 * KS;
+    double *Bs0 = dm_smem, *Bs1 = dm_smem + KP * DM_S;
+    const Tile tile = tiles[blockIdx.x];
+    const double *in = tile.from_local ? Lexp : Mexp;
+    const double *B = mats + (size_t)tile.mat * nst * nst;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lr = lane >> 2, lk = lane & 3;                   // fragment row / k (A), n / k (B)
+    const int row = warp * 8 + lr;
+    const bool rvalid = row < tile.nrows;
+
+    // zero the K-padding rows of both buffers once (cp.async never touches them)
+    for (int i = nst * DM_S + threadIdx.x; i < KP * DM_S; i += DM_THREADS) { Bs0[i] = 0.0; Bs1[i] = 0.0; }
+
+    const int nchunks = (nst + DM_NC - 1) / DM_NC;
+    auto issue = [&](int ch, double *dst) {
+        const int c0 = ch * DM_NC;
+        const int ncol = min(DM_NC, nst - c0);                  // multiple of 8
+        const int per_row = ncol >> 1;                          // 16-byte pieces per row
+        for (int i = threadIdx.x; i < nst * per_row; i += DM_THREADS) {
+            const int k = i / per_row, j = (i - k * per_row) * 2;
+            cp_async16(dst + k * DM_S + j, B + (size_t)k * nst + c0 + j);
+        }
+        cp_async_commit();
+    };
+    issue(0, Bs0);
+
+    // A operand -> registers
+    double a[KS];
+    {
+        const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
+        const double *ap = in + (size_t)(arow < 0 ? 0 : arow) * nst + lk;
+#pragma unroll
+        for (int s = 0; s < KS; ++s) a[s] = (arow >= 0 && 4 * s + lk < nst) ? ap[4 * s] : 0.0;
+    }
+    double *orow = scratch + (size_t)(tile.row0 + row) * nst + 2 * lk;
+
+    for (int ch = 0; ch < nchunks; ++ch) {
+        double *cur = (ch & 1) ? Bs1 : Bs0;
+        cp_async_wait<0>();
+        __syncthreads();                                        // chunk ch landed; everyone left chunk ch-1
+        if (ch + 1 < nchunks) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
+        const int c0 = ch * DM_NC;
+        const int nt = min(DM_NC, nst - c0) >> 3;               // n-tiles in this chunk: 1..3
+        const double *bp = cur + lk * DM_S + lr;
+        double c00 = 0, c01 = 0, c10 = 0, c11 = 0, c20 = 0, c21 = 0;
+        if (nt == 3) {
+#pragma unroll
+            for (int s = 0; s < KS; ++s) {
+                const double *b = bp + 4 * s * DM_S;
+                dmma884(c00, c01, a[s], b[0]);
+                dmma884(c10, c11, a[s], b[8]);
+                dmma884(c20, c21, a[s], b[16]);
+            }
+        } else {
+#pragma unroll
+            for (int s = 0; s < KS; ++s) {
+                const double *b = bp + 4 * s * DM_S;
+                dmma884(c00, c01, a[s], b[0]);
+                if (nt > 1) dmma884(c10, c11, a[s], b[8]);
+            }
+        }
+        if (rvalid) {
+            *reinterpret_cast<double2 *>(orow + c0) = make_double2(c00, c01);
+            if (nt > 1) *reinterpret_cast<double2 *>(orow + c0 + 8) = make_double2(c10, c11);
+            if (nt > 2) *reinterpret_cast<double2 *>(orow + c0 + 16) = make_double2(c20, c21);
+        }
+    }
+}
+
+template <int KS>
+static void launch_dmma(bem_ctx *c, const Stage &st)
+{
+    const size_t smem = (size_t)2 * 4 * KS * DM_S * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    translate_dmma<KS><<<st.ntiles, DM_THREADS, smem, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
+                                                                  c->mats.get(), c->nst, c->scratch.get());
+}
+
 // out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} scratch[pos[k]][:]   (fixed order)
 __global__ void __launch_bounds__(128)
 translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ pos, const double *__restrict__ scratch,
@@ -151,9 +269,19 @@ void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
 {
     if (st.ntgt == 0) return;
     if (st.ntiles > 0) {
-        dim3 grid(st.ntiles, cdiv(c->nst, GEMM_TN));
-        translate_gemm<<<grid, GEMM_THREADS, 0, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                             c->mats.get(), c->nst, c->scratch.get());
+        const int ks = c->nst / 4;                              // k-steps of the tensor path; nst is a multiple of 8
+        if (c->gemm_path == 1 || ks > 64) {                     // plain-FMA tiles: p > 16, or forced (option "gemm_path")
+            dim3 grid(st.ntiles, cdiv(c->nst, GEMM_TN));
+            translate_gemm<<<grid, GEMM_THREADS, 0, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
+                                                                 c->mats.get(), c->nst, c->scratch.get());
+        }
+        else if (ks <= 4) launch_dmma<4>(c, st);
+        else if (ks <= 10) launch_dmma<10>(c, st);
+        else if (ks <= 16) launch_dmma<16>(c, st);
+        else if (ks <= 26) launch_dmma<26>(c, st);
+        else if (ks <= 36) launch_dmma<36>(c, st);
+        else if (ks <= 50) launch_dmma<50>(c, st);
+        else launch_dmma<64>(c, st);
         KERNEL_CHECK();
         mark(c, cls_gemm);
     }
