@@ -18,8 +18,8 @@ CONFIG_PARAMS = {
     1: dict(p=8, leaf_size=64, eta=2.5),
     2: dict(p=10, leaf_size=64, eta=2.5),
     3: dict(p=10, leaf_size=64, eta=2.5),
-    4: dict(p=10, leaf_size=64, eta=2.5),
-    5: dict(p=12, leaf_size=64, eta=2.5),
+    4: dict(p=10, leaf_size=96, eta=2.5),
+    5: dict(p=12, leaf_size=96, eta=2.5),
 }
 
 

@@ -182,10 +182,10 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         build_sources(c, nullptr);
         c->tgt_pos.alloc(3 * N);
         CUDA_TRY(cudaMemcpyAsync(c->tgt_pos.get(), c->V.get(), 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, s));
-        const int tb = cdiv(N, 128);
+        const int tb = cdiv(N, 256);
         int nsplit = cdiv(592, tb);
         nsplit = std::max(1, std::min(nsplit, 64));
-        nsplit = (int)std::max<int64_t>(1, std::min<int64_t>(nsplit, c->ns / 128));
+        nsplit = (int)std::max<int64_t>(1, std::min<int64_t>(nsplit, c->ns / 256));
         c->nsplit = nsplit;
         c->ypart.alloc((size_t)nsplit * N);
         c->launches_per_apply = 3;

@@ -36,57 +36,80 @@ void launch_lift(bem_ctx *c, const double *q, const double *phi)
 }
 
 // ------------------------------------------------------------------ pair kernel
+// 1/sqrt(x) for x > 0 (0 for x == 0) to ~1 ulp: the hardware seed (MUFU.RSQ64H, relative error d ~ 2^-22)
+// followed by ONE third-order step  y1 = y0 (1 + e/2 + 3 e^2/8),  e = 1 - x y0^2, whose residual is
+// 5 e^3/16 ~ 2.5 d^3 < 1e-19 -- 5 FP64 instructions instead of the two Newton steps and the
+// slow-path branch of the library rsqrt (P2P).
+__device__ __forceinline__ double rsqrt_pos(double x)
+{
+    double y0;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+    y0 = __double2hiint(x) > 0 ? y0 : 0.0;        // x >= 0 here; x == 0 (and subnormal x) -> 0, an integer test off the FP64 pipe
+    const double e = fma(-x, y0 * y0, 1.0);
+    const double pe = fma(0.375, e, 0.5) * e;
+    return fma(y0, pe, y0);
+}
+
 // one (target, source) interaction; r2 == 0 (V1: source j = target i; "i != j") adds nothing
-__device__ __forceinline__ double pair_term(double tx, double ty, double tz, const double4 &sp, const double4 &ss)
+// acc += that interaction (the last multiply and the accumulation are one FMA)
+__device__ __forceinline__ double pair_acc(double acc, double tx, double ty, double tz, const double4 &sp, const double4 &ss)
 {
     const double dx = tx - sp.x, dy = ty - sp.y, dz = tz - sp.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
-    const double inv = r2 > 0.0 ? rsqrt(r2) : 0.0;
-    const double dd = ss.y * dx + ss.z * dy + ss.w * dz;
+    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    const double inv = rsqrt_pos(r2);
+    const double dd = fma(ss.y, dx, fma(ss.z, dy, ss.w * dz));
     // m/r - (d.dx)/r^3 = inv * (m - dd * inv^2)
-    return inv * (ss.x - dd * (inv * inv));
+    return fma(inv, fma(-dd, inv * inv, ss.x), acc);
 }
 
 constexpr int P2P_THREADS = 128;
-constexpr int P2P_TILE = 128;
+constexpr int P2P_TILE = 256;
 
 // ------------------------------------------------------------------ direct mode (a10')
-// grid = (target blocks, source splits); thread = one target; sources staged through shared memory
+// grid = (target blocks, source splits); thread = TWO targets (one shared-memory source read feeds
+// two pairs); sources staged through shared memory in tiles of 256
 __global__ void __launch_bounds__(P2P_THREADS)
 p2p_direct_kernel(const double *__restrict__ tgt, int64_t nt, const double4 *__restrict__ spos,
                   const double4 *__restrict__ sstr, int64_t ns, int64_t chunk, double *__restrict__ ypart)
 {
     __shared__ double4 sp[P2P_TILE], ss[P2P_TILE];
-    const int64_t t = (int64_t)blockIdx.x * P2P_THREADS + threadIdx.x;
-    double tx = 0, ty = 0, tz = 0;
-    if (t < nt) { tx = tgt[3 * t]; ty = tgt[3 * t + 1]; tz = tgt[3 * t + 2]; }
+    const int64_t ta = (int64_t)blockIdx.x * (2 * P2P_THREADS) + threadIdx.x, tb = ta + P2P_THREADS;
+    double ax = 0, ay = 0, az = 0, bx = 0, by = 0, bz = 0;
+    if (ta < nt) { ax = tgt[3 * ta]; ay = tgt[3 * ta + 1]; az = tgt[3 * ta + 2]; }
+    if (tb < nt) { bx = tgt[3 * tb]; by = tgt[3 * tb + 1]; bz = tgt[3 * tb + 2]; }
     const int64_t s0 = (int64_t)blockIdx.y * chunk, s1 = min(s0 + chunk, ns);
-    double acc = 0.0;
+    double acca = 0.0, accb = 0.0;
     for (int64_t base = s0; base < s1; base += P2P_TILE) {
         const int n = (int)min((int64_t)P2P_TILE, s1 - base);
         __syncthreads();
-        if (threadIdx.x < n) { sp[threadIdx.x] = spos[base + threadIdx.x]; ss[threadIdx.x] = sstr[base + threadIdx.x]; }
+        for (int i = threadIdx.x; i < n; i += P2P_THREADS) { sp[i] = spos[base + i]; ss[i] = sstr[base + i]; }
         __syncthreads();
 #pragma unroll 4
-        for (int j = 0; j < n; ++j) acc += pair_term(tx, ty, tz, sp[j], ss[j]);
+        for (int j = 0; j < n; ++j) {
+            const double4 p = sp[j], q = ss[j];
+            acca = pair_acc(acca, ax, ay, az, p, q);
+            accb = pair_acc(accb, bx, by, bz, p, q);
+        }
     }
-    if (t < nt) ypart[(int64_t)blockIdx.y * nt + t] = acc;
+    if (ta < nt) ypart[(int64_t)blockIdx.y * nt + ta] = acca;
+    if (tb < nt) ypart[(int64_t)blockIdx.y * nt + tb] = accb;
 }
 
 void launch_p2p_direct(bem_ctx *c)
 {
     const int64_t chunk = (c->ns + c->nsplit - 1) / c->nsplit;
-    dim3 grid(cdiv(c->N, P2P_THREADS), c->nsplit);
+    dim3 grid(cdiv(c->N, 2 * P2P_THREADS), c->nsplit);
     p2p_direct_kernel<<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
                                                            c->ns, chunk, c->ypart.get());
     KERNEL_CHECK();
 }
 
 // ------------------------------------------------------------------ FMM near field (a10)
-// One CTA per target leaf.  The 128 threads are arranged as TT targets x SS source
-// slices (TT * SS = 128, SS the largest power of two with TT >= targets in the leaf,
-// at most 32): lanes of a warp hold different targets and read the same source from shared
-// memory (a broadcast), slices are summed at the end in a fixed order -- no atomics,
+// One CTA per target leaf.  The sources of its (up to 27) neighbouring source leaves are treated
+// as ONE concatenated list and staged through shared memory in tiles of 256, whatever the leaf
+// boundaries.  The 128 threads are arranged as TT targets x SS source slices with TT = number of
+// targets of the leaf (chunks of 128) and SS = floor(128 / TT): lanes that hold different targets
+// read the same source (a broadcast); slices are summed at the end in a fixed order -- no atomics,
 // so two runs agree bit for bit.  y (engine order) already holds the far field (L2P).
 __global__ void __launch_bounds__(P2P_THREADS)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
@@ -95,38 +118,59 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
 {
     __shared__ double4 sp[P2P_TILE], ss[P2P_TILE];
     __shared__ double red[P2P_THREADS];
-    __shared__ int nb_s[27];
+    __shared__ int seg_s0[32], seg_pre[33];
     const int leaf = blockIdx.x;
     const int t0 = tbegin[leaf], nt = tbegin[leaf + 1] - t0;
-    if (threadIdx.x < 27) nb_s[threadIdx.x] = nbr[(int64_t)leaf * 27 + threadIdx.x];
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x;
+        const int b = lane < 27 ? nbr[(int64_t)leaf * 27 + lane] : -1;
+        int s0 = 0, cnt = 0;
+        if (b >= 0) { s0 = sbegin[b]; cnt = sbegin[b + 1] - s0; }
+        int inc = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        seg_s0[lane] = s0;
+        seg_pre[lane + 1] = inc;
+        if (lane == 0) seg_pre[0] = 0;
+    }
+    __syncthreads();
+    const int S = seg_pre[32];
     for (int c0 = 0; c0 < nt; c0 += P2P_THREADS) {
-        const int ntc = min(nt - c0, P2P_THREADS);
-        int SS = 1;
-        while (SS < 32 && ntc * (SS * 2) <= P2P_THREADS) SS *= 2;
-        const int TT = P2P_THREADS / SS;
-        const int tl = threadIdx.x % TT, sl = threadIdx.x / TT;
-        const bool active = tl < ntc;
+        const int TT = min(nt - c0, P2P_THREADS);
+        const int SS = P2P_THREADS / TT;
+        const int sl = threadIdx.x / TT, tl = threadIdx.x - sl * TT;
+        const bool active = sl < SS;
         double tx = 0, ty = 0, tz = 0;
         if (active) { const int64_t t = t0 + c0 + tl; tx = tgt[3 * t]; ty = tgt[3 * t + 1]; tz = tgt[3 * t + 2]; }
-        double acc = 0.0;
-        __syncthreads();
-        for (int k = 0; k < 27; ++k) {
-            const int sbx = nb_s[k];
-            if (sbx < 0) break;
-            const int s0 = sbegin[sbx], s1 = sbegin[sbx + 1];
-            for (int base = s0; base < s1; base += P2P_TILE) {
-                const int n = min(P2P_TILE, s1 - base);
-                __syncthreads();
-                if (threadIdx.x < n) { sp[threadIdx.x] = spos[base + threadIdx.x]; ss[threadIdx.x] = sstr[base + threadIdx.x]; }
-                __syncthreads();
-                if (active)
-                    for (int j = sl; j < n; j += SS) acc += pair_term(tx, ty, tz, sp[j], ss[j]);
+        double acc0 = 0.0, acc1 = 0.0;
+        for (int base = 0; base < S; base += P2P_TILE) {
+            const int n = min(P2P_TILE, S - base);
+            __syncthreads();
+            for (int i = threadIdx.x; i < n; i += P2P_THREADS) {
+                const int g = base + i;
+                int k = seg_pre[16] <= g ? 16 : 0;                     // last k with seg_pre[k] <= g
+                if (seg_pre[k + 8] <= g) k += 8;
+                if (seg_pre[k + 4] <= g) k += 4;
+                if (seg_pre[k + 2] <= g) k += 2;
+                if (seg_pre[k + 1] <= g) k += 1;
+                const int idx = seg_s0[k] + (g - seg_pre[k]);
+                sp[i] = spos[idx];
+                ss[i] = sstr[idx];
+            }
+            __syncthreads();
+            if (active) {
+                int j = sl;
+                for (; j + SS < n; j += 2 * SS) {
+                    acc0 = pair_acc(acc0, tx, ty, tz, sp[j], ss[j]);
+                    acc1 = pair_acc(acc1, tx, ty, tz, sp[j + SS], ss[j + SS]);
+                }
+                if (j < n) acc0 = pair_acc(acc0, tx, ty, tz, sp[j], ss[j]);
             }
         }
         __syncthreads();
-        red[threadIdx.x] = acc;
+        red[threadIdx.x] = acc0 + acc1;
         __syncthreads();
-        if (sl == 0 && active) {
+        if (sl == 0) {
             double sum = 0.0;
             for (int s = 0; s < SS; ++s) sum += red[s * TT + tl];
             y[t0 + c0 + tl] += sum;

@@ -297,16 +297,16 @@ void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
 // One warp per source leaf; lane = source (32 at a time).  Each lane builds the harmonics row by
 // row (degree l from degrees l-1, l-2); the 2l+1 real values of a row go through shared memory so
 // that lane k sums value k over the 32 sources -- a fixed-order sum, no atomics.
-constexpr int P2M_WARPS = 4;
+constexpr int P2M_WARPS_G = 4;
 
-__global__ void __launch_bounds__(P2M_WARPS * 32)
+__global__ void __launch_bounds__(P2M_WARPS_G * 32)
 p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf, int level,
            double cmx, double cmy, double cmz, double h,
            const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nst, double *__restrict__ Mout)
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int leaf = blockIdx.x * P2M_WARPS + warp;
+    const int leaf = blockIdx.x * P2M_WARPS_G + warp;
     if (leaf >= nleaf) return;
     double *tbl = sm + (size_t)warp * (2 * p - 1) * 33;            // [2l+1 values][33]
     uint32_t ix, iy, iz;
@@ -371,14 +371,14 @@ p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey
     }
 }
 
-void launch_p2m(bem_ctx *c)
+void launch_p2m_generic(bem_ctx *c)
 {
     const BoxSet &sb = c->sb;
     const int lmax = sb.lmax, nleaf = sb.nbox[lmax];
     const double h = c->cube_side / (double)(1 << lmax);
-    const size_t smem = (size_t)P2M_WARPS * (2 * c->p - 1) * 33 * sizeof(double);
+    const size_t smem = (size_t)P2M_WARPS_G * (2 * c->p - 1) * 33 * sizeof(double);
     if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(p2m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    p2m_kernel<<<cdiv(nleaf, P2M_WARPS), P2M_WARPS * 32, smem, c->stream>>>(
+    p2m_kernel<<<cdiv(nleaf, P2M_WARPS_G), P2M_WARPS_G * 32, smem, c->stream>>>(
         sb.begin.get(), sb.bkey[lmax].get(), nleaf, lmax, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
         c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
     KERNEL_CHECK();
@@ -426,7 +426,7 @@ l2p_kernel(const double *__restrict__ tgt, int64_t nt, const int32_t *__restrict
     y[t] = phi;
 }
 
-void launch_l2p(bem_ctx *c, const int32_t *leaf_of)
+void launch_l2p_generic(bem_ctx *c, const int32_t *leaf_of)
 {
     const BoxSet &tb = c->tb;
     const int lmax = tb.lmax;
