@@ -271,7 +271,8 @@ def run_gpu(args):
                 higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
                 config=dict(workload=workload_name(c), mode="direct" if args.direct else "fmm", p=p, n_nodes=N, n_triangles=T,
                             n_sources=int(stats["n_sources"]), leaf_size=args.leaf_size or c["leaf_size"], eta=c["eta"],
-                            lmax=int(stats["lmax"]), parallelism="replicas only" if world > 1 else "1 gpu",
+                            lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]), n_tgt_leaves=int(stats["n_tgt_leaves"]),
+                            parallelism="replicas only" if world > 1 else "1 gpu",
                             l2="flushed between iterations (512 MB write)" if flush else "working set larger than L2",
                             device_bytes=int(stats["device_bytes"])),
                 e2e=dict(value=e2e, unit=UNIT, h2d_bytes_per_step=16 * N, d2h_bytes_per_step=8 * N),

@@ -182,7 +182,7 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         build_sources(c, nullptr);
         c->tgt_pos.alloc(3 * N);
         CUDA_TRY(cudaMemcpyAsync(c->tgt_pos.get(), c->V.get(), 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, s));
-        const int tb = cdiv(N, 256);
+        const int tb = cdiv(N, 512);
         int nsplit = cdiv(592, tb);
         nsplit = std::max(1, std::min(nsplit, 64));
         nsplit = (int)std::max<int64_t>(1, std::min<int64_t>(nsplit, c->ns / 256));

@@ -64,65 +64,86 @@ __device__ __forceinline__ double pair_acc(double acc, double tx, double ty, dou
 
 constexpr int P2P_THREADS = 128;
 constexpr int P2P_TILE = 256;
+constexpr int P2P_TPT = 4;            // direct mode: targets per thread
 
 // ------------------------------------------------------------------ direct mode (a10')
-// grid = (target blocks, source splits); thread = TWO targets (one shared-memory source read feeds
-// two pairs); sources staged through shared memory in tiles of 256
+// grid = (target blocks, source splits); thread = FOUR targets, so one shared-memory source read
+// (4 x LDS.128, a broadcast) feeds four pairs -- measured with ncu, one target per thread is bound by
+// the shared-memory pipe (88% LSU wavefronts at 48% FP64), not by FP64; sources staged in tiles of 256
 __global__ void __launch_bounds__(P2P_THREADS)
 p2p_direct_kernel(const double *__restrict__ tgt, int64_t nt, const double4 *__restrict__ spos,
                   const double4 *__restrict__ sstr, int64_t ns, int64_t chunk, double *__restrict__ ypart)
 {
     __shared__ double4 sp[P2P_TILE], ss[P2P_TILE];
-    const int64_t ta = (int64_t)blockIdx.x * (2 * P2P_THREADS) + threadIdx.x, tb = ta + P2P_THREADS;
-    double ax = 0, ay = 0, az = 0, bx = 0, by = 0, bz = 0;
-    if (ta < nt) { ax = tgt[3 * ta]; ay = tgt[3 * ta + 1]; az = tgt[3 * ta + 2]; }
-    if (tb < nt) { bx = tgt[3 * tb]; by = tgt[3 * tb + 1]; bz = tgt[3 * tb + 2]; }
+    const int64_t tfirst = (int64_t)blockIdx.x * (P2P_TPT * P2P_THREADS) + threadIdx.x;
+    double tx[P2P_TPT], ty[P2P_TPT], tz[P2P_TPT], acc[P2P_TPT];
+#pragma unroll
+    for (int k = 0; k < P2P_TPT; ++k) {
+        const int64_t t = tfirst + (int64_t)k * P2P_THREADS;
+        tx[k] = ty[k] = tz[k] = 0.0;
+        acc[k] = 0.0;
+        if (t < nt) { tx[k] = tgt[3 * t]; ty[k] = tgt[3 * t + 1]; tz[k] = tgt[3 * t + 2]; }
+    }
     const int64_t s0 = (int64_t)blockIdx.y * chunk, s1 = min(s0 + chunk, ns);
-    double acca = 0.0, accb = 0.0;
     for (int64_t base = s0; base < s1; base += P2P_TILE) {
         const int n = (int)min((int64_t)P2P_TILE, s1 - base);
         __syncthreads();
         for (int i = threadIdx.x; i < n; i += P2P_THREADS) { sp[i] = spos[base + i]; ss[i] = sstr[base + i]; }
         __syncthreads();
-#pragma unroll 4
+#pragma unroll 2
         for (int j = 0; j < n; ++j) {
             const double4 p = sp[j], q = ss[j];
-            acca = pair_acc(acca, ax, ay, az, p, q);
-            accb = pair_acc(accb, bx, by, bz, p, q);
+#pragma unroll
+            for (int k = 0; k < P2P_TPT; ++k) acc[k] = pair_acc(acc[k], tx[k], ty[k], tz[k], p, q);
         }
     }
-    if (ta < nt) ypart[(int64_t)blockIdx.y * nt + ta] = acca;
-    if (tb < nt) ypart[(int64_t)blockIdx.y * nt + tb] = accb;
+#pragma unroll
+    for (int k = 0; k < P2P_TPT; ++k) {
+        const int64_t t = tfirst + (int64_t)k * P2P_THREADS;
+        if (t < nt) ypart[(int64_t)blockIdx.y * nt + t] = acc[k];
+    }
 }
 
 void launch_p2p_direct(bem_ctx *c)
 {
     const int64_t chunk = (c->ns + c->nsplit - 1) / c->nsplit;
-    dim3 grid(cdiv(c->N, 2 * P2P_THREADS), c->nsplit);
+    dim3 grid(cdiv(c->N, P2P_TPT * P2P_THREADS), c->nsplit);
     p2p_direct_kernel<<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
                                                            c->ns, chunk, c->ypart.get());
     KERNEL_CHECK();
 }
 
 // ------------------------------------------------------------------ FMM near field (a10)
-// One CTA per target leaf.  The sources of its (up to 27) neighbouring source leaves are treated
-// as ONE concatenated list and staged through shared memory in tiles of 256, whatever the leaf
-// boundaries.  The 128 threads are arranged as TT targets x SS source slices with TT = number of
-// targets of the leaf (chunks of 128) and SS = floor(128 / TT): lanes that hold different targets
-// read the same source (a broadcast); slices are summed at the end in a fixed order -- no atomics,
-// so two runs agree bit for bit.  y (engine order) already holds the far field (L2P).
-__global__ void __launch_bounds__(P2P_THREADS)
+// One CTA (4 warps) per target leaf.  The sources of its (up to 27) neighbouring source leaves are
+// treated as ONE concatenated list of S sources; LANES HOLD SOURCES (one per lane and round, read
+// straight from global memory into registers, 128 per CTA round) and loop over the targets of the
+// leaf, 32 at a time, which are broadcast from shared memory (2 x LDS.128 per pair instead of 4, and
+// with a warp-uniform address).  Every lane keeps 32 partial sums acc[t] in registers over all its
+// rounds; one transposed butterfly (31 shuffle steps) at the end leaves the sum of acc[t] over the
+// lanes in lane t, and the 4 warps are added through shared memory -- a fixed order, no atomics, so
+// two runs agree bit for bit.  Work is ~ (targets) x ceil(S/128) x 128 pairs whatever the leaf sizes.
+// y (engine order) already holds the far field (L2P).
+constexpr int P2P_WARPS = P2P_THREADS / 32;
+
+// (x, y, z) of a shared-memory point.  volatile: the targets do not change inside the round loop, and the
+// compiler would otherwise hoist all 32 of them (96 doubles) out of it and spill them to local memory.
+__device__ __forceinline__ void lds_point(unsigned addr, double &x, double &y, double &z)
+{
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%3];\n\tld.shared.f64 %2, [%3+16];" : "=d"(x), "=d"(y), "=d"(z) : "r"(addr));
+}
+
+__global__ void __launch_bounds__(P2P_THREADS, 4)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
                 const int32_t *__restrict__ sbegin, const double4 *__restrict__ spos, const double4 *__restrict__ sstr,
                 double *__restrict__ y)
 {
-    __shared__ double4 sp[P2P_TILE], ss[P2P_TILE];
-    __shared__ double red[P2P_THREADS];
+    __shared__ double4 tg[32];
+    __shared__ double red[P2P_WARPS][32];
     __shared__ int seg_s0[32], seg_pre[33];
     const int leaf = blockIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int t0 = tbegin[leaf], nt = tbegin[leaf + 1] - t0;
-    if (threadIdx.x < 32) {
-        const int lane = threadIdx.x;
+    if (warp == 0) {
         const int b = lane < 27 ? nbr[(int64_t)leaf * 27 + lane] : -1;
         int s0 = 0, cnt = 0;
         if (b >= 0) { s0 = sbegin[b]; cnt = sbegin[b + 1] - s0; }
@@ -135,45 +156,72 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
     }
     __syncthreads();
     const int S = seg_pre[32];
-    for (int c0 = 0; c0 < nt; c0 += P2P_THREADS) {
-        const int TT = min(nt - c0, P2P_THREADS);
-        const int SS = P2P_THREADS / TT;
-        const int sl = threadIdx.x / TT, tl = threadIdx.x - sl * TT;
-        const bool active = sl < SS;
-        double tx = 0, ty = 0, tz = 0;
-        if (active) { const int64_t t = t0 + c0 + tl; tx = tgt[3 * t]; ty = tgt[3 * t + 1]; tz = tgt[3 * t + 2]; }
-        double acc0 = 0.0, acc1 = 0.0;
-        for (int base = 0; base < S; base += P2P_TILE) {
-            const int n = min(P2P_TILE, S - base);
-            __syncthreads();
-            for (int i = threadIdx.x; i < n; i += P2P_THREADS) {
-                const int g = base + i;
-                int k = seg_pre[16] <= g ? 16 : 0;                     // last k with seg_pre[k] <= g
-                if (seg_pre[k + 8] <= g) k += 8;
-                if (seg_pre[k + 4] <= g) k += 4;
-                if (seg_pre[k + 2] <= g) k += 2;
-                if (seg_pre[k + 1] <= g) k += 1;
-                const int idx = seg_s0[k] + (g - seg_pre[k]);
-                sp[i] = spos[idx];
-                ss[i] = sstr[idx];
-            }
-            __syncthreads();
-            if (active) {
-                int j = sl;
-                for (; j + SS < n; j += 2 * SS) {
-                    acc0 = pair_acc(acc0, tx, ty, tz, sp[j], ss[j]);
-                    acc1 = pair_acc(acc1, tx, ty, tz, sp[j + SS], ss[j + SS]);
-                }
-                if (j < n) acc0 = pair_acc(acc0, tx, ty, tz, sp[j], ss[j]);
-            }
+    const int rounds = (S + P2P_THREADS - 1) / P2P_THREADS;
+    const unsigned tg_base = (unsigned)__cvta_generic_to_shared(tg);
+
+    // source g of the concatenated list; beyond the end a far-away point of zero strength (adds exactly 0)
+    auto load_source = [&](int g, double4 &p, double4 &q) {
+        if (g < S) {
+            int k = seg_pre[16] <= g ? 16 : 0;                         // last k with seg_pre[k] <= g
+            if (seg_pre[k + 8] <= g) k += 8;
+            if (seg_pre[k + 4] <= g) k += 4;
+            if (seg_pre[k + 2] <= g) k += 2;
+            if (seg_pre[k + 1] <= g) k += 1;
+            const int idx = seg_s0[k] + (g - seg_pre[k]);
+            p = spos[idx];
+            q = sstr[idx];
+        } else {
+            p = make_double4(1e100, 0.0, 0.0, 0.0);
+            q = make_double4(0.0, 0.0, 0.0, 0.0);
+        }
+    };
+
+    for (int c0 = 0; c0 < nt; c0 += 32) {
+        const int ntc = min(32, nt - c0);
+        __syncthreads();                                                // tg / red of the previous group are free
+        if (threadIdx.x < 32) {
+            double4 v = make_double4(0.0, 0.0, 0.0, 0.0);
+            if (threadIdx.x < ntc) { const int64_t t = t0 + c0 + threadIdx.x; v = make_double4(tgt[3 * t], tgt[3 * t + 1], tgt[3 * t + 2], 0.0); }
+            tg[threadIdx.x] = v;
         }
         __syncthreads();
-        red[threadIdx.x] = acc0 + acc1;
+        double acc[32];
+#pragma unroll
+        for (int t = 0; t < 32; ++t) acc[t] = 0.0;
+        double4 p, q, pn, qn;
+        load_source(threadIdx.x, pn, qn);
+        for (int r = 0; r < rounds; ++r) {
+            p = pn; q = qn;
+            if (r + 1 < rounds) load_source((r + 1) * P2P_THREADS + threadIdx.x, pn, qn);   // prefetch the next round
+#pragma unroll
+            for (int tb = 0; tb < 32; tb += 4) {                        // 4 independent chains at a time
+                if (tb >= ntc) break;                                   // warp-uniform; targets beyond ntc are zero points of tg
+#pragma unroll
+                for (int t = tb; t < tb + 4; ++t) {
+                    double Tx, Ty, Tz;
+                    lds_point(tg_base + 32u * t, Tx, Ty, Tz);
+                    acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                }
+            }
+        }
+        // transposed butterfly: afterwards acc[0] of lane L = sum over lanes of acc[L]
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            const bool up = (lane & off) != 0;
+#pragma unroll
+            for (int i = 0; i < off; ++i) {
+                const double send = up ? acc[i] : acc[i + off];
+                const double keep = up ? acc[i + off] : acc[i];
+                acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+            }
+        }
+        red[warp][lane] = acc[0];
         __syncthreads();
-        if (sl == 0) {
-            double sum = 0.0;
-            for (int s = 0; s < SS; ++s) sum += red[s * TT + tl];
-            y[t0 + c0 + tl] += sum;
+        if (threadIdx.x < ntc) {
+            double sum = red[0][threadIdx.x];
+#pragma unroll
+            for (int w = 1; w < P2P_WARPS; ++w) sum += red[w][threadIdx.x];
+            y[t0 + c0 + threadIdx.x] += sum;
         }
     }
 }
