@@ -183,7 +183,7 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         c->tgt_pos.alloc(3 * N);
         CUDA_TRY(cudaMemcpyAsync(c->tgt_pos.get(), c->V.get(), 3 * N * sizeof(double), cudaMemcpyDeviceToDevice, s));
         const int tb = cdiv(N, 512);
-        int nsplit = cdiv(592, tb);
+        int nsplit = cdiv(148 * 14, tb);             // >= 14 CTAs (56 warps) per SM: the pair loop is latency-bound below that
         nsplit = std::max(1, std::min(nsplit, 64));
         nsplit = (int)std::max<int64_t>(1, std::min<int64_t>(nsplit, c->ns / 256));
         c->nsplit = nsplit;

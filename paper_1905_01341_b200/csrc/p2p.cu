@@ -124,6 +124,7 @@ void launch_p2p_direct(bem_ctx *c)
 // two runs agree bit for bit.  Work is ~ (targets) x ceil(S/128) x 128 pairs whatever the leaf sizes.
 // y (engine order) already holds the far field (L2P).
 constexpr int P2P_WARPS = P2P_THREADS / 32;
+constexpr int P2P_NT = 16;           // targets per pass (register accumulators per lane); 8, 16 or 32
 
 // (x, y, z) of a shared-memory point.  volatile: the targets do not change inside the round loop, and the
 // compiler would otherwise hoist all 32 of them (96 doubles) out of it and spill them to local memory.
@@ -132,13 +133,13 @@ __device__ __forceinline__ void lds_point(unsigned addr, double &x, double &y, d
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%3];\n\tld.shared.f64 %2, [%3+16];" : "=d"(x), "=d"(y), "=d"(z) : "r"(addr));
 }
 
-__global__ void __launch_bounds__(P2P_THREADS, 4)
+__global__ void __launch_bounds__(P2P_THREADS, 5)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
                 const int32_t *__restrict__ sbegin, const double4 *__restrict__ spos, const double4 *__restrict__ sstr,
                 double *__restrict__ y)
 {
-    __shared__ double4 tg[32];
-    __shared__ double red[P2P_WARPS][32];
+    __shared__ double4 tg[P2P_NT];
+    __shared__ double red[P2P_WARPS][P2P_NT];
     __shared__ int seg_s0[32], seg_pre[33];
     const int leaf = blockIdx.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -176,37 +177,70 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
         }
     };
 
-    for (int c0 = 0; c0 < nt; c0 += 32) {
-        const int ntc = min(32, nt - c0);
+    for (int c0 = 0; c0 < nt; c0 += P2P_NT) {
+        const int ntc = min(P2P_NT, nt - c0);
         __syncthreads();                                                // tg / red of the previous group are free
-        if (threadIdx.x < 32) {
+        if (threadIdx.x < P2P_NT) {
             double4 v = make_double4(0.0, 0.0, 0.0, 0.0);
             if (threadIdx.x < ntc) { const int64_t t = t0 + c0 + threadIdx.x; v = make_double4(tgt[3 * t], tgt[3 * t + 1], tgt[3 * t + 2], 0.0); }
             tg[threadIdx.x] = v;
         }
         __syncthreads();
-        double acc[32];
+        double acc[P2P_NT];
 #pragma unroll
-        for (int t = 0; t < 32; ++t) acc[t] = 0.0;
+        for (int t = 0; t < P2P_NT; ++t) acc[t] = 0.0;
         double4 p, q, pn, qn;
         load_source(threadIdx.x, pn, qn);
+#pragma unroll 1
         for (int r = 0; r < rounds; ++r) {
             p = pn; q = qn;
             if (r + 1 < rounds) load_source((r + 1) * P2P_THREADS + threadIdx.x, pn, qn);   // prefetch the next round
 #pragma unroll
-            for (int tb = 0; tb < 32; tb += 4) {                        // 4 independent chains at a time
-                if (tb >= ntc) break;                                   // warp-uniform; targets beyond ntc are zero points of tg
+            for (int tb = 0; tb < P2P_NT; tb += 8) {                    // 8 independent chains at a time
+                if (tb + 8 <= ntc) {                                    // warp-uniform
 #pragma unroll
-                for (int t = tb; t < tb + 4; ++t) {
-                    double Tx, Ty, Tz;
-                    lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                    acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                    for (int t = tb; t < tb + 8; ++t) {
+                        double Tx, Ty, Tz;
+                        lds_point(tg_base + 32u * t, Tx, Ty, Tz);
+                        acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                    }
+                } else if (tb < ntc) {                                  // the last 1..7 targets: 4 + singles
+                    if (tb + 4 <= ntc) {
+#pragma unroll
+                        for (int t = tb; t < tb + 4; ++t) {
+                            double Tx, Ty, Tz;
+                            lds_point(tg_base + 32u * t, Tx, Ty, Tz);
+                            acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                        }
+#pragma unroll
+                        for (int t = tb + 4; t < tb + 7; ++t) {
+                            if (t < ntc) {
+                                double Tx, Ty, Tz;
+                                lds_point(tg_base + 32u * t, Tx, Ty, Tz);
+                                acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                            }
+                        }
+                    } else {
+#pragma unroll
+                        for (int t = tb; t < tb + 3; ++t) {
+                            if (t < ntc) {
+                                double Tx, Ty, Tz;
+                                lds_point(tg_base + 32u * t, Tx, Ty, Tz);
+                                acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                            }
+                        }
+                    }
                 }
             }
         }
-        // transposed butterfly: afterwards acc[0] of lane L = sum over lanes of acc[L]
+        // transposed butterfly: afterwards acc[0] of lane L = sum over the 32 lanes of acc[L % P2P_NT]
 #pragma unroll
-        for (int off = 16; off >= 1; off >>= 1) {
+        for (int off = 16; off >= P2P_NT; off >>= 1) {
+#pragma unroll
+            for (int i = 0; i < P2P_NT; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], off);
+        }
+#pragma unroll
+        for (int off = P2P_NT / 2; off >= 1; off >>= 1) {
             const bool up = (lane & off) != 0;
 #pragma unroll
             for (int i = 0; i < off; ++i) {
@@ -215,7 +249,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                 acc[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
             }
         }
-        red[warp][lane] = acc[0];
+        if (lane < P2P_NT) red[warp][lane] = acc[0];
         __syncthreads();
         if (threadIdx.x < ntc) {
             double sum = red[0][threadIdx.x];
