@@ -1,6 +1,7 @@
 // The C-ABI boundary (include/bem.h): context, bem_create, bem_setup, bem_apply and the
 // small query calls.  bem_solve lives in solve.cu.
 #include "common.cuh"
+#include "harmonics.cuh"
 
 #include <chrono>
 #include <cmath>
@@ -155,7 +156,9 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     c->have_diag = false;
     c->have_cfree = false;
     c->p = p;
-    c->nst = ((p * p + 7) / 8) * 8;
+    c->pl = p <= 16 ? std::max(4, 2 * ((p + 1) / 2)) : p;     // template buckets 4, 6, .., 16 of the P2M / L2P / DMMA kernels
+    c->nre = lay_nre(c->pl);
+    c->nst = lay_nst(c->pl);
     c->leaf_size = leaf_size;
     c->eta = eta;
     compute_geometry(c);

@@ -80,6 +80,7 @@ constexpr int MAT_M2L = 0;         // matrix ids: [0,343) M2L by offset, then 8 
 constexpr int MAT_L2L = 343;
 constexpr int MAT_M2M = 351;
 constexpr int N_MATS = 359;
+constexpr int ROT_M = 32;          // entries per matrix in the azimuth table (m < P_MAX = 32)
 
 struct BoxSet {                     // the non-empty boxes of one point set on levels 0..lmax
     int lmax = 0;
@@ -98,7 +99,7 @@ struct BoxSet {                     // the non-empty boxes of one point set on l
 
 // One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
 // executed as (tiles of a dense GEMM per matrix) -> scratch rows -> fixed-order row sums.
-struct Tile { int32_t mat, row0, nrows, from_local; };
+struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split)
 struct Stage {
     int64_t npairs = 0;
     int ntgt = 0;
@@ -106,6 +107,7 @@ struct Stage {
     bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
     dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
     dvec<int32_t> pos;              // [npairs] scratch row of pair k (target-major order)
+    dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order): the reduce pass rotates back by its azimuth
     dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
     dvec<Tile> tiles;
     int ntiles = 0;
@@ -132,7 +134,8 @@ struct bem_ctx {
 
     // setup state
     bool ready = false;
-    int p = 0, nst = 0;             // truncation number, expansion row stride (p^2 rounded up to 8)
+    int p = 0, nst = 0;             // truncation number, expansion row stride (harmonics.cuh: nre + nim)
+    int pl = 0, nre = 0;            // layout degree count (kernel template bucket >= p), size of the real-part block
     int leaf_size = 0;
     double eta = 0;
     double cube_min[3] = {0, 0, 0}, cube_side = 1.0;
@@ -155,6 +158,8 @@ struct bem_ctx {
     bem::BoxSet sb, tb;
     bem::dvec<int32_t> nbr;         // [n_tgt_leaves * 27] source leaves adjacent to a target leaf, -1 padded
     bem::dvec<double> mats;         // [N_MATS * nst * nst] real translation matrices, row = input dof k, col = output dof
+    bem::dvec<double2> rot;         // [N_MATS * ROT_M] (cos m a, sin m a): azimuth a of the M2L offset, identity for M2M / L2L
+    bem::dvec<int32_t> kinfo;       // [nst] order m of every stored dof (0 for padding)
     bem::dvec<double> Mexp, Lexp;   // [total boxes * nst]
     bem::dvec<double> scratch;      // [max pairs of a stage * nst]
     std::vector<bem::Stage> m2m;    // leaf-1 .. 2

@@ -7,7 +7,14 @@
 // with the Condon-Shortley phase, R_l^{-m} = (-1)^m conj R_l^m (same for I), so
 // that 1/|x-y| = sum_{l,m} conj R_l^m(y-c) I_l^m(x-c).  Only m >= 0 is stored;
 // a real field has C_l^{-m} = (-1)^m conj C_l^m, so an expansion is p^2 real
-// numbers, laid out as  idx(l,0) = l^2,  idx(l,m,Re) = l^2+2m-1,  idx(l,m,Im) = l^2+2m.
+// numbers.  Layout of a stored expansion (row of nst = 2 nre doubles): all REAL parts first,
+// idx(l,m,Re) = l(l+1)/2 + m  (0 <= m <= l), padded to nre = a multiple of 8, then all
+// IMAGINARY parts at the same place of the second half, idx(l,m,Im) = nre + l(l+1)/2 + m
+// (the m = 0 slots stay zero), so that the two parts of a coefficient are exactly nre apart.
+// The split is what makes the M2L matrices block diagonal:
+// for an offset in the xz-plane every I_n^m(T) is real, so real parts map to real parts
+// and imaginary parts to imaginary parts.  The layout is sized for pl >= p (the template
+// bucket of the kernels); degrees p..pl-1 are kept zero.
 //
 // Box-scaled coefficients (h = box edge):  Mt_l^m = M_l^m / h^(l+1),
 // Lt_l^m = L_l^m h^l.  With them every translation matrix depends only on the
@@ -25,7 +32,9 @@ namespace bem {
 constexpr int P_MAX = 32;          // bem_setup rejects p > 32
 
 BEM_HD int tri_idx(int l, int m) { return l * (l + 1) / 2 + m; }
-BEM_HD int real_idx(int l, int m, int part) { return l * l + (m == 0 ? 0 : 2 * m - 1 + part); }
+BEM_HD int lay_nre(int pl) { return ((pl * (pl + 1) / 2 + 7) / 8) * 8; }
+BEM_HD int lay_nst(int pl) { return 2 * lay_nre(pl); }
+BEM_HD int real_idx(int l, int m, int part, int nre) { return part * nre + l * (l + 1) / 2 + m; }
 
 // R_l^m(x,y,z) for 0 <= m <= l < p at tri_idx(l,m).
 BEM_HD void eval_R(double x, double y, double z, int p, double *re, double *im)
@@ -94,15 +103,18 @@ BEM_HD cplx tab_get(const double *re, const double *im, int lmax_excl, int l, in
     return v;
 }
 
-// decode a real-basis index c in [0, p^2) into (l, m, part)
-BEM_HD void real_decode(int c, int *l, int *m, int *part)
+// decode a stored index c in [0, nst) into (l, m, part); false for padding entries, degrees >= p and Im of m = 0
+BEM_HD bool real_decode(int c, int p, int nre, int *l, int *m, int *part)
 {
-    int ll = (int)sqrt((double)c);
-    while (ll * ll > c) --ll;
-    while ((ll + 1) * (ll + 1) <= c) ++ll;
-    const int k = c - ll * ll;
-    *l = ll;
-    if (k == 0) { *m = 0; *part = 0; } else { *m = (k + 1) / 2; *part = (k + 1) & 1; }
+    const int im = c >= nre ? 1 : 0;
+    const int t = im ? c - nre : c;
+    int lt = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
+    while (lt * (lt + 1) / 2 > t) --lt;
+    while ((lt + 1) * (lt + 2) / 2 <= t) ++lt;
+    *l = lt;
+    *m = t - lt * (lt + 1) / 2;
+    *part = im;
+    return lt < p && !(im && *m == 0);
 }
 
 // One entry of a real translation matrix: the response at output dof
@@ -124,11 +136,10 @@ BEM_HD double real_entry(cplx Wp, cplx Wm, int mi, int pi, int po, double scale)
 
 // M2L:  Lt_l^m = (-1)^l sum_{j<p,k} Mt_j^k I_{j+l}^{k+m}(That),
 // That = (c_target - c_source)/h.  Ire/Iim hold I up to degree 2p-2.
-BEM_HD double m2l_entry(const double *Ire, const double *Iim, int p, int cout, int cin)
+BEM_HD double m2l_entry(const double *Ire, const double *Iim, int p, int nre, int cout, int cin)
 {
     int l, m, po, j, k, pi;
-    real_decode(cout, &l, &m, &po);
-    real_decode(cin, &j, &k, &pi);
+    if (!real_decode(cout, p, nre, &l, &m, &po) || !real_decode(cin, p, nre, &j, &k, &pi)) return 0.0;
     const cplx Wp = tab_get(Ire, Iim, 2 * p - 1, j + l, k + m);
     const cplx Wm = tab_get(Ire, Iim, 2 * p - 1, j + l, -k + m);
     return real_entry(Wp, Wm, k, pi, po, (l & 1) ? -1.0 : 1.0);
@@ -136,11 +147,10 @@ BEM_HD double m2l_entry(const double *Ire, const double *Iim, int p, int cout, i
 
 // M2M:  Mt'_l^m = 2^-(l+1) sum_{j<=l,k} Mt_j^k conj R_{l-j}^{m-k}(that),
 // that = (c_child - c_parent)/h_child.
-BEM_HD double m2m_entry(const double *Rre, const double *Rim, int p, int cout, int cin)
+BEM_HD double m2m_entry(const double *Rre, const double *Rim, int p, int nre, int cout, int cin)
 {
     int l, m, po, j, k, pi;
-    real_decode(cout, &l, &m, &po);
-    real_decode(cin, &j, &k, &pi);
+    if (!real_decode(cout, p, nre, &l, &m, &po) || !real_decode(cin, p, nre, &j, &k, &pi)) return 0.0;
     if (j > l) return 0.0;
     cplx Wp = tab_get(Rre, Rim, p, l - j, m - k); Wp.im = -Wp.im;
     cplx Wm = tab_get(Rre, Rim, p, l - j, m + k); Wm.im = -Wm.im;
@@ -149,11 +159,10 @@ BEM_HD double m2m_entry(const double *Rre, const double *Rim, int p, int cout, i
 
 // L2L:  Lt'_j^k = sum_{l>=j,m} 2^-l Lt_l^m conj R_{l-j}^{m-k}(that),
 // that = (c_child - c_parent)/h_child.  Output dof (j,k), input dof (l,m).
-BEM_HD double l2l_entry(const double *Rre, const double *Rim, int p, int cout, int cin)
+BEM_HD double l2l_entry(const double *Rre, const double *Rim, int p, int nre, int cout, int cin)
 {
     int l, m, pi, j, k, po;
-    real_decode(cout, &j, &k, &po);
-    real_decode(cin, &l, &m, &pi);
+    if (!real_decode(cout, p, nre, &j, &k, &po) || !real_decode(cin, p, nre, &l, &m, &pi)) return 0.0;
     if (l < j) return 0.0;
     cplx Wp = tab_get(Rre, Rim, p, l - j, m - k); Wp.im = -Wp.im;
     cplx Wm = tab_get(Rre, Rim, p, l - j, -m - k); Wm.im = -Wm.im;

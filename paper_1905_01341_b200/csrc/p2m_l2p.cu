@@ -132,8 +132,12 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
             }
         }
     }
+    // group-local value k of group g is (l, m, part) in degree-major order l^2 + (0 | 2m-1 | 2m); store it at its
+    // place in the split layout (harmonics.cuh); everything else of the row (padding, degrees >= p) is zero
     double *M = Mout + (size_t)leaf * nst;
-    const int n = p * p;
+    constexpr int NRE = ((P * (P + 1) / 2 + 7) / 8) * 8;
+    for (int k = lane; k < nst; k += 32) M[k] = 0.0;
+    __syncwarp();
 #pragma unroll
     for (int l = 0; l < P; ++l) {
         const bool last = (l == P - 1) || (grp_start(l + 1) != grp_start(l));
@@ -142,11 +146,17 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
 #pragma unroll
             for (int slot = 0; slot < 2; ++slot) {
                 const int k = lane + 32 * slot;
-                if (32 * slot < nval && k < nval && g0 + k < n) M[g0 + k] = acc[2 * g + slot];
+                if (32 * slot < nval && k < nval) {
+                    const int o = g0 + k;
+                    int ll = (int)sqrt((double)o);
+                    while (ll * ll > o) --ll;
+                    while ((ll + 1) * (ll + 1) <= o) ++ll;
+                    const int r = o - ll * ll, m = (r + 1) >> 1, part = (r > 0 && !(r & 1)) ? 1 : 0;
+                    if (ll < p) M[real_idx(ll, m, part, NRE)] = acc[2 * g + slot];
+                }
             }
         }
     }
-    for (int k = n + lane; k < nst; k += 32) M[k] = 0.0;                // row padding: the tiles read nst entries
 }
 
 template <int P>
@@ -204,12 +214,13 @@ l2p_kernel_t(const double *__restrict__ tgt, int64_t nt, const int32_t *__restri
         next_row<P>(l, bx, by, bz, r2, Rre, Rim);
         if (l < p) {
             const int cur = l & 1;
-            const double *Ll = L + l * l;
+            constexpr int NRE = ((P * (P + 1) / 2 + 7) / 8) * 8;
+            const double *Lre = L + l * (l + 1) / 2, *Lim = Lre + NRE;                        // split layout (harmonics.cuh)
             double row = 0.0;
 #pragma unroll
             for (int m = 1; m < P; ++m)
-                if (m <= l) row = fma(__ldg(Ll + 2 * m - 1), Rre[cur][m], fma(__ldg(Ll + 2 * m), Rim[cur][m], row));
-            phi += fma(2.0, row, __ldg(Ll) * Rre[cur][0]);
+                if (m <= l) row = fma(__ldg(Lre + m), Rre[cur][m], fma(__ldg(Lim + m), Rim[cur][m], row));
+            phi += fma(2.0, row, __ldg(Lre) * Rre[cur][0]);
         }
     }
     y[t] = phi;

@@ -13,12 +13,18 @@
 #include "harmonics.cuh"
 #include "morton.cuh"
 
+#include <cmath>
+
 namespace bem {
 
 // ------------------------------------------------------------------ matrices (setup)
 __host__ __device__ inline int tab_len(int deg_excl) { return deg_excl * (deg_excl + 1) / 2; }
 
-// one thread per matrix: its harmonic table
+// one thread per matrix: its harmonic table.  An M2L offset (ox, oy, oz) is first turned about the z axis
+// into the xz-plane, T' = (sqrt(ox^2 + oy^2), 0, oz): there every I_n^m(T') is REAL, so the real p^2 x p^2
+// matrix splits into a (real parts -> real parts) and an (imaginary -> imaginary) block -- half the flops.
+// The azimuth is applied to the coefficients instead: Mt'_j^k = e^{ik a} Mt_j^k going in (gather of the tile
+// kernels) and Lt_l^m = e^{im a} Lt'_l^m coming out (reduce pass), a = atan2(oy, ox).
 __global__ void harmonic_tables(int p, double *tab_re, double *tab_im, int stride)
 {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;
@@ -27,30 +33,27 @@ __global__ void harmonic_tables(int p, double *tab_re, double *tab_im, int strid
     if (m < MAT_L2L) {
         const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
         if (max(max(abs(ox), abs(oy)), abs(oz)) < 2) return;          // adjacent offsets are never used
-        eval_I((double)ox, (double)oy, (double)oz, 2 * p - 1, re, im);
+        eval_I(sqrt((double)(ox * ox + oy * oy)), 0.0, (double)oz, 2 * p - 1, re, im);
     } else {
         const int o = (m - MAT_L2L) & 7;                               // child octant: bit set -> +1/2
         eval_R((o & 1) ? 0.5 : -0.5, (o & 2) ? 0.5 : -0.5, (o & 4) ? 0.5 : -0.5, p, re, im);
     }
 }
-// mats[m][k][c] = T_m[c][k]  (row = input dof, column = output dof), zero padded to nst
-__global__ void fill_matrices(int p, int nst, const double *tab_re, const double *tab_im, int stride, double *mats)
+// mats[m][k][c] = T_m[c][k]  (row = input dof, column = output dof); padding dofs and degrees >= p are zero
+__global__ void fill_matrices(int p, int nre, int nst, const double *tab_re, const double *tab_im, int stride, double *mats)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t per = (int64_t)nst * nst;
     if (idx >= per * N_MATS) return;
     const int m = (int)(idx / per);
     const int k = (int)((idx % per) / nst), cc = (int)(idx % nst);
-    const int n = p * p;
     double v = 0.0;
-    if (k < n && cc < n) {
-        const double *re = tab_re + (size_t)m * stride, *im = tab_im + (size_t)m * stride;
-        if (m < MAT_L2L) {
-            const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
-            if (max(max(abs(ox), abs(oy)), abs(oz)) >= 2) v = m2l_entry(re, im, p, cc, k);
-        } else if (m < MAT_M2M) v = l2l_entry(re, im, p, cc, k);
-        else v = m2m_entry(re, im, p, cc, k);
-    }
+    const double *re = tab_re + (size_t)m * stride, *im = tab_im + (size_t)m * stride;
+    if (m < MAT_L2L) {
+        const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
+        if (max(max(abs(ox), abs(oy)), abs(oz)) >= 2 && ((k < nre) == (cc < nre))) v = m2l_entry(re, im, p, nre, cc, k);
+    } else if (m < MAT_M2M) v = l2l_entry(re, im, p, nre, cc, k);
+    else v = m2m_entry(re, im, p, nre, cc, k);
     mats[idx] = v;
 }
 
@@ -67,28 +70,60 @@ void build_matrices(bem_ctx *c)
     KERNEL_CHECK();
     const int64_t tot = (int64_t)N_MATS * nst * nst;
     c->mats.alloc(tot);
-    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, nst, tre.get(), tim.get(), stride, c->mats.get());
+    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, c->nre, nst, tre.get(), tim.get(), stride, c->mats.get());
     KERNEL_CHECK();
+    // azimuth table (cos m a, sin m a) and the per-dof table (m, partner = the other part of the same (l, m), part)
+    std::vector<double2> rot((size_t)N_MATS * ROT_M);
+    for (int m = 0; m < N_MATS; ++m) {
+        double a = 0.0;
+        if (m < MAT_L2L) {
+            const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3;
+            if (ox != 0 || oy != 0) a = atan2((double)oy, (double)ox);
+        }
+        for (int k = 0; k < ROT_M; ++k) rot[(size_t)m * ROT_M + k] = make_double2(cos(k * a), sin(k * a));
+    }
+    c->rot.alloc(rot.size());
+    CUDA_TRY(cudaMemcpyAsync(c->rot.get(), rot.data(), rot.size() * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+    std::vector<int32_t> kin(nst);
+    for (int k = 0; k < nst; ++k) {
+        int l, m, part;
+        kin[k] = real_decode(k, c->pl, c->nre, &l, &m, &part) ? m : 0;
+    }
+    c->kinfo.alloc(nst);
+    CUDA_TRY(cudaMemcpyAsync(c->kinfo.get(), kin.data(), nst * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
+}
+
+// e^{i m a} applied to one coefficient (re, im) in place:  Re' = cos Re - sin Im,  Im' = cos Im + sin Re
+__device__ __forceinline__ void azimuth(double2 cs, double &re, double &im)
+{
+    const double r = fma(cs.x, re, -cs.y * im);
+    im = fma(cs.x, im, cs.y * re);
+    re = r;
 }
 
 // ------------------------------------------------------------------ batched GEMM (a6, a7, a8)
 // scratch[row0 + r][:] = in[src_sorted[row0 + r]][:] * mats[tile.mat]   for r < tile.nrows
+// (M2L tiles: the input row is first turned by the azimuth of the offset, see harmonic_tables)
+// Plain-FMA version (any p; the fallback for p > 16 and option gemm_path = 1).
 // CTA: 64 rows x 64 columns, K in chunks of 8; thread: 4 rows x 4 columns (columns strided by 16).
 constexpr int GEMM_TM = 64, GEMM_TN = 64, GEMM_KC = 8, GEMM_THREADS = 256;
 
 __global__ void __launch_bounds__(GEMM_THREADS)
 translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
-               const double *__restrict__ mats, int nst, double *__restrict__ scratch)
+               const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+               int nst, double *__restrict__ scratch)
 {
     __shared__ double As[GEMM_KC][GEMM_TM + 4];
     __shared__ double Bs[GEMM_KC][GEMM_TN];
     __shared__ int rows[GEMM_TM];
     const Tile tile = tiles[blockIdx.x];
     const int n0 = blockIdx.y * GEMM_TN;
-    const double *in = tile.from_local ? Lexp : Mexp;
+    const double *in = (tile.flags & 1) ? Lexp : Mexp;
+    const bool split = (tile.flags & 2) != 0;
     const double *B = mats + (size_t)tile.mat * nst * nst;
+    const double2 *rcs = rot + (size_t)tile.mat * ROT_M;
     if (threadIdx.x < GEMM_TM) rows[threadIdx.x] = threadIdx.x < tile.nrows ? src_sorted[tile.row0 + threadIdx.x] : -1;
     __syncthreads();
     const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
@@ -103,7 +138,21 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
     const int arow = rows[ar];
     for (int k0 = 0; k0 < nst; k0 += GEMM_KC) {
         double2 av = make_double2(0.0, 0.0), bv = make_double2(0.0, 0.0);
-        if (arow >= 0) av = *reinterpret_cast<const double2 *>(in + (size_t)arow * nst + k0 + ak);
+        if (arow >= 0) {
+            const double *ap = in + (size_t)arow * nst;
+            av = *reinterpret_cast<const double2 *>(ap + k0 + ak);
+            if (split) {                                        // partner = the other part of the same (l, m), nre away
+                const int nre = nst >> 1, k = k0 + ak;
+                const bool im = k >= nre;
+                const double2 w = *reinterpret_cast<const double2 *>(ap + (im ? k - nre : k + nre));
+                const double2 c0 = rcs[kinfo[k]], c1 = rcs[kinfo[k + 1]];
+                double re0 = im ? w.x : av.x, im0 = im ? av.x : w.x, re1 = im ? w.y : av.y, im1 = im ? av.y : w.y;
+                azimuth(c0, re0, im0);
+                azimuth(c1, re1, im1);
+                av.x = im ? im0 : re0;
+                av.y = im ? im1 : re1;
+            }
+        }
         if (n0 + bc < nst) bv = *reinterpret_cast<const double2 *>(B + (size_t)(k0 + bk) * nst + n0 + bc);
         __syncthreads();
         As[ak][ar] = av.x; As[ak + 1][ar] = av.y;
@@ -134,16 +183,23 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
 }
 
 // ------------------------------------------------------------------ the same product on the FP64 tensor path
-// Measured on B200 (profiles/r1_02_dmma_vs_dfma.md): mma.sync m8n8k4 f64 (SASS DMMA) sustains 37.15 TFLOP/s,
-// a register-resident DFMA loop 33.8; more important, one DMMA needs ONE 8-byte shared-memory operand per
-// thread for 512 flop per warp, so the GEMM is no longer bound by shared-memory operand traffic.
+// Measured on B200 (profiles/): mma.sync m8n8k4 f64 (SASS DMMA) sustains 37.15 TFLOP/s, a register-resident
+// DFMA loop 33.9; more important, one DMMA needs ONE 8-byte shared-memory operand per thread for 512 flop per
+// warp, so the GEMM is no longer bound by shared-memory operand traffic.
 //
 // CTA = 8 warps = 64 scratch rows (pairs) of one matrix.  Each warp owns 8 rows and keeps their whole A
-// operand (8 x K input expansion coefficients, gathered straight from global memory) in registers as KS
-// m8n8k4 A-fragments; the translation matrix streams through shared memory in chunks of DM_NC columns
-// (cp.async, double buffered), shared by the 8 warps.  K is padded to 4 KS (zero A, zero B rows).
-constexpr int DM_NC = 24;            // columns of B per chunk (3 n-tiles)
-constexpr int DM_S = 28;             // row stride of a chunk in doubles: 28 = 12 (mod 16) -> conflict-free fragment loads
+// operand (8 x nst input coefficients, gathered straight from global memory and, for M2L, turned by the
+// azimuth of the offset in registers: the two parts of a coefficient sit in a[s] and a[s + KSH] of the same
+// lane) as 2 KSH m8n8k4 A-fragments; the matrix streams through shared memory in chunks of up to DM_NT
+// n-tiles (cp.async, double buffered), shared by the 8 warps.
+// KSH = k-steps (4 dofs each) of the real-part block = of the imaginary-part block.  An M2L matrix is block
+// diagonal in that split: its real-part columns only take the real-part k-steps and its imaginary-part
+// columns the others -- KSH^2 DMMA per warp instead of 2 KSH^2.
+// M2M / L2L matrices (8 + 8 of them, a few % of the work) are dense and take all k-steps.
+constexpr int DM_NT = 5;             // n-tiles (8 columns of B) per chunk = independent accumulator chains per warp
+constexpr int DM_S = 44;             // row stride of a chunk in doubles: 44 = 12 (mod 16) -> conflict-free fragment loads
+constexpr int DM_NT_DENSE = 2;       // dense (M2M / L2L) tiles: twice the rows, so narrower chunks with row stride
+constexpr int DM_S_DENSE = 20;       // 20 = 4 (mod 16): 2 nre x 20 doubles fit the nre x 44 buffer of the split tiles
 constexpr int DM_THREADS = 256;
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
@@ -162,106 +218,165 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                  : "d"(a), "d"(b));
 }
 
+// one chunk of NT n-tiles over the k-steps [KB, KE): cur = chunk buffer, whose row 0 is dof 4 KR
+template <int KS, int KB, int KE, int KR, int NT, int S>
+__device__ __forceinline__ void dm_chunk_nt(const double (&a)[KS], const double *cur, int lr, int lk, bool rvalid, double *orow_c0)
+{
+    const double *bp = cur + lk * S + lr;
+    double c[NT][2];
+#pragma unroll
+    for (int j = 0; j < NT; ++j) c[j][0] = c[j][1] = 0.0;
+#pragma unroll
+    for (int s = KB; s < KE; ++s) {
+        const double *b = bp + 4 * (s - KR) * S;
+#pragma unroll
+        for (int j = 0; j < NT; ++j) dmma884(c[j][0], c[j][1], a[s], b[8 * j]);
+    }
+    if (rvalid) {
+#pragma unroll
+        for (int j = 0; j < NT; ++j) *reinterpret_cast<double2 *>(orow_c0 + 8 * j) = make_double2(c[j][0], c[j][1]);
+    }
+}
+template <int KS, int KB, int KE, int KR>
+__device__ __forceinline__ void dm_chunk(const double (&a)[KS], const double *cur, int nt, int lr, int lk,
+                                         bool rvalid, double *orow_c0)
+{
+    switch (nt) {                                               // warp-uniform
+    case 5: dm_chunk_nt<KS, KB, KE, KR, 5, DM_S>(a, cur, lr, lk, rvalid, orow_c0); break;
+    case 4: dm_chunk_nt<KS, KB, KE, KR, 4, DM_S>(a, cur, lr, lk, rvalid, orow_c0); break;
+    case 3: dm_chunk_nt<KS, KB, KE, KR, 3, DM_S>(a, cur, lr, lk, rvalid, orow_c0); break;
+    case 2: dm_chunk_nt<KS, KB, KE, KR, 2, DM_S>(a, cur, lr, lk, rvalid, orow_c0); break;
+    default: dm_chunk_nt<KS, KB, KE, KR, 1, DM_S>(a, cur, lr, lk, rvalid, orow_c0); break;
+    }
+}
 template <int KS>
+__device__ __forceinline__ void dm_chunk_dense(const double (&a)[KS], const double *cur, int nt, int lr, int lk,
+                                               bool rvalid, double *orow_c0)
+{
+    if (nt == 2) dm_chunk_nt<KS, 0, KS, 0, 2, DM_S_DENSE>(a, cur, lr, lk, rvalid, orow_c0);
+    else dm_chunk_nt<KS, 0, KS, 0, 1, DM_S_DENSE>(a, cur, lr, lk, rvalid, orow_c0);
+}
+
+template <int KSH>
 __global__ void __launch_bounds__(DM_THREADS)
 translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
-               const double *__restrict__ mats, int nst, double *__restrict__ scratch)
+               const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+               double *__restrict__ scratch)
 {
-    extern __shared__ __align__(16) double dm_smem[];          // [2][4 KS][DM_S]
-    constexpr int KP = 4 * KS;
-    double *Bs0 = dm_smem, *Bs1 = dm_smem + KP * DM_S;
+    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S] (dense tiles: [2][2 NRE][DM_S_DENSE])
+    __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
+    constexpr int KS = 2 * KSH, NRE = 4 * KSH, NST = 4 * KS;
+    constexpr int NTH = KSH / 2;                               // n-tiles (8 columns) of one block
     const Tile tile = tiles[blockIdx.x];
-    const double *in = tile.from_local ? Lexp : Mexp;
-    const double *B = mats + (size_t)tile.mat * nst * nst;
+    const double *in = (tile.flags & 1) ? Lexp : Mexp;
+    const bool split = (tile.flags & 2) != 0;
+    const int brows = split ? NRE : NST;                       // rows of B a chunk needs
+    double *Bs0 = dm_smem, *Bs1 = dm_smem + NRE * DM_S;
+    const int bstride = split ? DM_S : DM_S_DENSE;
+    const double *B = mats + (size_t)tile.mat * NST * NST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int lr = lane >> 2, lk = lane & 3;                   // fragment row / k (A), n / k (B)
     const int row = warp * 8 + lr;
     const bool rvalid = row < tile.nrows;
 
-    // zero the K-padding rows of both buffers once (cp.async never touches them)
-    for (int i = nst * DM_S + threadIdx.x; i < KP * DM_S; i += DM_THREADS) { Bs0[i] = 0.0; Bs1[i] = 0.0; }
-
-    const int nchunks = (nst + DM_NC - 1) / DM_NC;
+    // chunks of balanced width: per block of ntb n-tiles, ceil(ntb / DM_NT) chunks
+    const int ntb = split ? NTH : 2 * NTH;                      // n-tiles per block (dense: one block = everything)
+    const int wmax = split ? DM_NT : DM_NT_DENSE;
+    const int cpb = (ntb + wmax - 1) / wmax;                    // chunks per block
+    const int cw = (ntb + cpb - 1) / cpb;                       // chunk width in n-tiles
+    const int nchunks = split ? 2 * cpb : cpb;
+    auto chunk = [&](int ch, int &blk, int &t0, int &nt) {
+        blk = ch >= cpb;
+        const int cl = blk ? ch - cpb : ch;
+        t0 = blk * NTH + cw * cl;
+        nt = min(cw, blk * NTH + ntb - t0);
+    };
     auto issue = [&](int ch, double *dst) {
-        const int c0 = ch * DM_NC;
-        const int ncol = min(DM_NC, nst - c0);                  // multiple of 8
-        const int per_row = ncol >> 1;                          // 16-byte pieces per row
-        for (int i = threadIdx.x; i < nst * per_row; i += DM_THREADS) {
-            const int k = i / per_row, j = (i - k * per_row) * 2;
-            cp_async16(dst + k * DM_S + j, B + (size_t)k * nst + c0 + j);
+        int blk, t0, nt;
+        chunk(ch, blk, t0, nt);
+        const int c0 = 8 * t0, per_row = 4 * nt;                // 16-byte pieces per row
+        const int k0 = blk ? NRE : 0;                           // the block's own rows (dense: all rows)
+        for (int i = threadIdx.x; i < brows * per_row; i += DM_THREADS) {
+            const int k = i / per_row, j = (i % per_row) * 2;
+            cp_async16(dst + k * bstride + j, B + (size_t)(k0 + k) * NST + c0 + j);
         }
         cp_async_commit();
     };
     issue(0, Bs0);
+    if (split) {
+        for (int k = threadIdx.x; k < NRE; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
+    }
 
     // A operand -> registers
     double a[KS];
     {
         const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
-        const double *ap = in + (size_t)(arow < 0 ? 0 : arow) * nst + lk;
+        const double *ap = in + (size_t)(arow < 0 ? 0 : arow) * NST + lk;
 #pragma unroll
-        for (int s = 0; s < KS; ++s) a[s] = (arow >= 0 && 4 * s + lk < nst) ? ap[4 * s] : 0.0;
+        for (int s = 0; s < KS; ++s) a[s] = arow >= 0 ? ap[4 * s] : 0.0;
     }
-    double *orow = scratch + (size_t)(tile.row0 + row) * nst + 2 * lk;
+    double *orow = scratch + (size_t)(tile.row0 + row) * NST + 2 * lk;
 
     for (int ch = 0; ch < nchunks; ++ch) {
         double *cur = (ch & 1) ? Bs1 : Bs0;
         cp_async_wait<0>();
-        __syncthreads();                                        // chunk ch landed; everyone left chunk ch-1
+        __syncthreads();                                        // chunk ch landed; everyone left chunk ch-1; cs_k visible
+        if (ch == 0 && split) {
+#pragma unroll
+            for (int s = 0; s < KSH; ++s) azimuth(cs_k[4 * s + lk], a[s], a[s + KSH]);
+        }
         if (ch + 1 < nchunks) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
-        const int c0 = ch * DM_NC;
-        const int nt = min(DM_NC, nst - c0) >> 3;               // n-tiles in this chunk: 1..3
-        const double *bp = cur + lk * DM_S + lr;
-        double c00 = 0, c01 = 0, c10 = 0, c11 = 0, c20 = 0, c21 = 0;
-        if (nt == 3) {
-#pragma unroll
-            for (int s = 0; s < KS; ++s) {
-                const double *b = bp + 4 * s * DM_S;
-                dmma884(c00, c01, a[s], b[0]);
-                dmma884(c10, c11, a[s], b[8]);
-                dmma884(c20, c21, a[s], b[16]);
-            }
-        } else {
-#pragma unroll
-            for (int s = 0; s < KS; ++s) {
-                const double *b = bp + 4 * s * DM_S;
-                dmma884(c00, c01, a[s], b[0]);
-                if (nt > 1) dmma884(c10, c11, a[s], b[8]);
-            }
-        }
-        if (rvalid) {
-            *reinterpret_cast<double2 *>(orow + c0) = make_double2(c00, c01);
-            if (nt > 1) *reinterpret_cast<double2 *>(orow + c0 + 8) = make_double2(c10, c11);
-            if (nt > 2) *reinterpret_cast<double2 *>(orow + c0 + 16) = make_double2(c20, c21);
-        }
+        int blk, t0, nt;
+        chunk(ch, blk, t0, nt);
+        // chunk buffers hold the block's rows from row 0: the imaginary block reads its k-steps KSH.. at rows 0..
+        if (!split) dm_chunk_dense<KS>(a, cur, nt, lr, lk, rvalid, orow + 8 * t0);
+        else if (blk == 0) dm_chunk<KS, 0, KSH, 0>(a, cur, nt, lr, lk, rvalid, orow + 8 * t0);
+        else dm_chunk<KS, KSH, KS, KSH>(a, cur, nt, lr, lk, rvalid, orow + 8 * t0);
     }
 }
 
-template <int KS>
+template <int KSH>
 static void launch_dmma(bem_ctx *c, const Stage &st)
 {
-    const size_t smem = (size_t)2 * 4 * KS * DM_S * sizeof(double);
+    const size_t smem = (size_t)2 * 4 * KSH * DM_S * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    translate_dmma<KS><<<st.ntiles, DM_THREADS, smem, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                                  c->mats.get(), c->nst, c->scratch.get());
+    translate_dmma<KSH><<<st.ntiles, DM_THREADS, smem, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
+                                                                   c->mats.get(), c->kinfo.get(), c->rot.get(), c->scratch.get());
 }
 
-// out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} scratch[pos[k]][:]   (fixed order)
-__global__ void __launch_bounds__(128)
-translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ pos, const double *__restrict__ scratch,
-                 int nst, double *__restrict__ out)
+// out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[pos[k]][:]   (fixed order; a_k = azimuth of
+// pair k's matrix, the identity for M2M / L2L pairs).  One CTA per target box, one thread per coefficient (l, m):
+// it reads the real and the imaginary part (nre apart) of every row once and writes both.
+__global__ void __launch_bounds__(160)
+translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ pos, const int32_t *__restrict__ mat_t,
+                 const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+                 int nre, double *__restrict__ out)
 {
     const int t = blockIdx.x;
     const int b = ptr[t], e = ptr[t + 1];
-    for (int cc = threadIdx.x; cc < nst; cc += blockDim.x) {
-        double s = 0.0;
-        for (int k = b; k < e; ++k) s += scratch[(size_t)pos[k] * nst + cc];
-        out[(size_t)t * nst + cc] = s;
+    const int nst = 2 * nre;
+    double *o = out + (size_t)t * nst;
+    for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
+        const int m = kinfo[cc];
+        double sr = 0.0, si = 0.0;
+        if (m == 0) {
+            for (int k = b; k < e; ++k) sr += scratch[(size_t)pos[k] * nst + cc];
+        } else {
+            for (int k = b; k < e; ++k) {
+                const double *row = scratch + (size_t)pos[k] * nst + cc;
+                double vr = row[0], vi = row[nre];
+                azimuth(__ldg(rot + (size_t)mat_t[k] * ROT_M + m), vr, vi);
+                sr += vr;
+                si += vi;
+            }
+        }
+        o[cc] = sr;
+        o[cc + nre] = si;
     }
 }
 
@@ -269,24 +384,25 @@ void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
 {
     if (st.ntgt == 0) return;
     if (st.ntiles > 0) {
-        const int ks = c->nst / 4;                              // k-steps of the tensor path; nst is a multiple of 8
-        if (c->gemm_path == 1 || ks > 64) {                     // plain-FMA tiles: p > 16, or forced (option "gemm_path")
+        const int pl = c->pl;
+        if (c->gemm_path == 1 || pl > 16) {                     // plain-FMA tiles: p > 16, or forced (option "gemm_path")
             dim3 grid(st.ntiles, cdiv(c->nst, GEMM_TN));
             translate_gemm<<<grid, GEMM_THREADS, 0, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                                 c->mats.get(), c->nst, c->scratch.get());
+                                                                 c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, c->scratch.get());
         }
-        else if (ks <= 4) launch_dmma<4>(c, st);
-        else if (ks <= 10) launch_dmma<10>(c, st);
-        else if (ks <= 16) launch_dmma<16>(c, st);
-        else if (ks <= 26) launch_dmma<26>(c, st);
-        else if (ks <= 36) launch_dmma<36>(c, st);
-        else if (ks <= 50) launch_dmma<50>(c, st);
-        else launch_dmma<64>(c, st);
+        else if (pl == 4) launch_dmma<4>(c, st);                // nre / 4 of the layout for pl = 4, 6, .., 16
+        else if (pl == 6) launch_dmma<6>(c, st);
+        else if (pl == 8) launch_dmma<10>(c, st);
+        else if (pl == 10) launch_dmma<14>(c, st);
+        else if (pl == 12) launch_dmma<20>(c, st);
+        else if (pl == 14) launch_dmma<28>(c, st);
+        else launch_dmma<34>(c, st);
         KERNEL_CHECK();
         mark(c, cls_gemm);
     }
     double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
-    translate_reduce<<<st.ntgt, 128, 0, c->stream>>>(st.ptr.get(), st.pos.get(), c->scratch.get(), c->nst, out);
+    translate_reduce<<<st.ntgt, std::min(160, ((c->nre + 31) / 32) * 32), 0, c->stream>>>(st.ptr.get(), st.pos.get(), st.mat_t.get(), c->scratch.get(),
+                                                     c->kinfo.get(), c->rot.get(), c->nre, out);
     KERNEL_CHECK();
     mark(c, cls_reduce);
 }
@@ -302,7 +418,7 @@ constexpr int P2M_WARPS_G = 4;
 __global__ void __launch_bounds__(P2M_WARPS_G * 32)
 p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf, int level,
            double cmx, double cmy, double cmz, double h,
-           const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nst, double *__restrict__ Mout)
+           const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nre, int nst, double *__restrict__ Mout)
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -363,7 +479,7 @@ p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey
             for (int k = lane; k < 2 * l + 1; k += 32) {
                 double sum = 0.0;
                 for (int j = 0; j < 32; ++j) sum += tbl[k * 33 + j];
-                M[l * l + k] += sum;
+                M[real_idx(l, (k + 1) >> 1, (k > 0 && !(k & 1)) ? 1 : 0, nre)] += sum;
             }
             __syncwarp();
             for (int m = 0; m <= l; ++m) { qre[m] = pre[m]; qim[m] = pim[m]; pre[m] = cre[m]; pim[m] = cim[m]; }
@@ -380,7 +496,7 @@ void launch_p2m_generic(bem_ctx *c)
     if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(p2m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     p2m_kernel<<<cdiv(nleaf, P2M_WARPS_G), P2M_WARPS_G * 32, smem, c->stream>>>(
         sb.begin.get(), sb.bkey[lmax].get(), nleaf, lmax, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
-        c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
+        c->src_pos.get(), c->src_str.get(), c->p, c->nre, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
     KERNEL_CHECK();
 }
 
@@ -389,7 +505,7 @@ void launch_p2m_generic(bem_ctx *c)
 // One thread per target; threads of a warp mostly share the leaf, so coefficient loads are broadcasts.
 __global__ void __launch_bounds__(128)
 l2p_kernel(const double *__restrict__ tgt, int64_t nt, const int32_t *__restrict__ leaf_of, const uint64_t *__restrict__ tkey,
-           double cmx, double cmy, double cmz, double h, int p, int nst, const double *__restrict__ Lleaf, double *__restrict__ y)
+           double cmx, double cmy, double cmz, double h, int p, int nre, int nst, const double *__restrict__ Lleaf, double *__restrict__ y)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nt) return;
@@ -417,9 +533,9 @@ l2p_kernel(const double *__restrict__ tgt, int64_t nt, const int32_t *__restrict
             cre[l] = f * (bx * pre[l - 1] - by * pim[l - 1]);
             cim[l] = f * (bx * pim[l - 1] + by * pre[l - 1]);
         }
-        const double *Ll = L + l * l;
-        double row = Ll[0] * cre[0];
-        for (int m = 1; m <= l; ++m) row += 2.0 * (Ll[2 * m - 1] * cre[m] + Ll[2 * m] * cim[m]);
+        const double *Lre = L + l * (l + 1) / 2, *Lim = Lre + nre;
+        double row = Lre[0] * cre[0];
+        for (int m = 1; m <= l; ++m) row += 2.0 * (Lre[m] * cre[m] + Lim[m] * cim[m]);
         phi += row;
         for (int m = 0; m <= l; ++m) { qre[m] = pre[m]; qim[m] = pim[m]; pre[m] = cre[m]; pim[m] = cim[m]; }
     }
@@ -432,7 +548,7 @@ void launch_l2p_generic(bem_ctx *c, const int32_t *leaf_of)
     const int lmax = tb.lmax;
     const double h = c->cube_side / (double)(1 << lmax);
     l2p_kernel<<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, leaf_of, tb.bkey[lmax].get(),
-                                                       c->cube_min[0], c->cube_min[1], c->cube_min[2], h, c->p, c->nst,
+                                                       c->cube_min[0], c->cube_min[1], c->cube_min[2], h, c->p, c->nre, c->nst,
                                                        c->Lexp.get() + (size_t)tb.base[lmax] * c->nst, c->ypart.get());
     KERNEL_CHECK();
 }

@@ -240,11 +240,12 @@ static void finish_stage(Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cuda
             t.mat = m;
             t.row0 = row + r;
             t.nrows = std::min(GEMM_TM, h[m] - r);
-            t.from_local = (m >= MAT_L2L && m < MAT_M2M) ? 1 : 0;
+            t.flags = ((m >= MAT_L2L && m < MAT_M2M) ? 1 : 0) | (m < MAT_L2L ? 2 : 0);
             tiles.push_back(t);
         }
         row += h[m];
     }
+    st.mat_t = std::move(mat);
     st.ntiles = (int)tiles.size();
     st.tiles.alloc(tiles.size());
     if (!tiles.empty()) CUDA_TRY(cudaMemcpy(st.tiles.get(), tiles.data(), tiles.size() * sizeof(Tile), cudaMemcpyHostToDevice));
