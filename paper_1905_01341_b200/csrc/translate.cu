@@ -197,9 +197,9 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
 // columns the others -- KSH^2 DMMA per warp instead of 2 KSH^2.
 // M2M / L2L matrices (8 + 8 of them, a few % of the work) are dense and take all k-steps.
 constexpr int DM_NT = 5;             // n-tiles (8 columns of B) per chunk = independent accumulator chains per warp
-constexpr int DM_S = 44;             // row stride of a chunk in doubles: 44 = 12 (mod 16) -> conflict-free fragment loads
+constexpr int DM_S = 46;             // row stride of a chunk in doubles: 2 x 46 = 12 (mod 16) -> conflict-free fragment loads
 constexpr int DM_NT_DENSE = 2;       // dense (M2M / L2L) tiles: twice the rows, so narrower chunks with row stride
-constexpr int DM_S_DENSE = 20;       // 20 = 4 (mod 16): 2 nre x 20 doubles fit the nre x 44 buffer of the split tiles
+constexpr int DM_S_DENSE = 22;       // 2 x 22 = 12 (mod 16); 2 nre x 22 doubles fit the nre x 46 buffer of the split tiles
 constexpr int DM_THREADS = 256;
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
@@ -222,13 +222,13 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 template <int KS, int KB, int KE, int KR, int NT, int S>
 __device__ __forceinline__ void dm_chunk_nt(const double (&a)[KS], const double *cur, int lr, int lk, bool rvalid, double *orow_c0)
 {
-    const double *bp = cur + lk * S + lr;
+    const double *bp = cur + 2 * lk * S + lr;          // dof of fragment position (s, lk): 8 (s / 2) + 2 lk + (s & 1)
     double c[NT][2];
 #pragma unroll
     for (int j = 0; j < NT; ++j) c[j][0] = c[j][1] = 0.0;
 #pragma unroll
     for (int s = KB; s < KE; ++s) {
-        const double *b = bp + 4 * (s - KR) * S;
+        const double *b = bp + (8 * ((s - KR) >> 1) + ((s - KR) & 1)) * S;
 #pragma unroll
         for (int j = 0; j < NT; ++j) dmma884(c[j][0], c[j][1], a[s], b[8 * j]);
     }
@@ -308,13 +308,18 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
         for (int k = threadIdx.x; k < NRE; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
     }
 
-    // A operand -> registers
+    // A operand -> registers.  K is permuted so that the fragments of the k-steps 2j and 2j+1 of a lane are the
+    // two ADJACENT dofs 8j + 2 lk and 8j + 2 lk + 1: one 16-byte load per pair of k-steps.
     double a[KS];
     {
         const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
-        const double *ap = in + (size_t)(arow < 0 ? 0 : arow) * NST + lk;
+        const double2 *ap = reinterpret_cast<const double2 *>(in + (size_t)(arow < 0 ? 0 : arow) * NST) + lk;
 #pragma unroll
-        for (int s = 0; s < KS; ++s) a[s] = arow >= 0 ? ap[4 * s] : 0.0;
+        for (int j = 0; j < KS / 2; ++j) {
+            const double2 v = arow >= 0 ? ap[4 * j] : make_double2(0.0, 0.0);
+            a[2 * j] = v.x;
+            a[2 * j + 1] = v.y;
+        }
     }
     double *orow = scratch + (size_t)(tile.row0 + row) * NST + 2 * lk;
 
@@ -324,7 +329,7 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
         __syncthreads();                                        // chunk ch landed; everyone left chunk ch-1; cs_k visible
         if (ch == 0 && split) {
 #pragma unroll
-            for (int s = 0; s < KSH; ++s) azimuth(cs_k[4 * s + lk], a[s], a[s + KSH]);
+            for (int s = 0; s < KSH; ++s) azimuth(cs_k[8 * (s >> 1) + 2 * lk + (s & 1)], a[s], a[s + KSH]);
         }
         if (ch + 1 < nchunks) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
         int blk, t0, nt;
