@@ -88,6 +88,7 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
             mh = st.x * ih; dx = st.y * ih * ih; dy = st.z * ih * ih; dz = st.w * ih * ih;
         }
         const double r2 = ax * ax + ay * ay + az * az;
+        const double hx = 0.5 * dx, hy = 0.5 * dy;
         double Rre[2][P], Rim[2][P];
 #pragma unroll
         for (int l = 0; l < P; ++l) {
@@ -105,10 +106,10 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
                         double Br = 0.0, Bi = 0.0;
                         if (m >= 1) { Br = Rre[prv][m - 1]; Bi = Rim[prv][m - 1]; }
                         else if (l - 1 >= 1) { Br = -Rre[prv][1]; Bi = Rim[prv][1]; }      // R_{l-1}^{-1} = -conj R_{l-1}^{1}
-                        gr = dz * Cr + 0.5 * (dx * Ar + dy * Ai) - 0.5 * (dx * Br - dy * Bi);
-                        gi = dz * Ci + 0.5 * (dx * Ai - dy * Ar) - 0.5 * (dx * Bi + dy * Br);
+                        gr = fma(hx, Ar - Br, fma(hy, Ai + Bi, dz * Cr));           // hx = dx / 2, hy = dy / 2
+                        gi = fma(hx, Ai - Bi, fma(-hy, Ar + Br, dz * Ci));
                     }
-                    const double vr = mh * Rre[cur][m] - gr, vi = -(mh * Rim[cur][m] - gi);   // conj
+                    const double vr = fma(mh, Rre[cur][m], -gr), vi = fma(-mh, Rim[cur][m], gi);   // conj
                     if (m == 0) col[0] = vr;
                     else { col[(2 * m - 1) * 33] = vr; col[(2 * m) * 33] = vi; }
                 }

@@ -224,3 +224,31 @@ def test_fmm_leaf_size_one_and_huge():
         ctx = _ctx(c, p=12, leaf=leaf)
         y = _apply(ctx, c["q"], c["phi"])
         assert _rel(y, yo) <= 3e-5, (leaf, ctx.bem_get_stats()["lmax"], _rel(y, yo))
+
+
+def test_fmm_every_truncation_number_cfg1():
+    """Odd p (stored in the layout of the next even template bucket), the buckets themselves and the run-time-p
+    kernels (p > 16): the single-layer error falls monotonically (to rounding) and follows Table 1's decay."""
+    c = cfg(1)
+    rows = np.arange(c["V"].shape[0], dtype=np.int64)
+    yo = oracle_rows(c, rows, 0, "q", None)
+    errs = {}
+    for p in (1, 2, 3, 4, 5, 7, 9, 11, 13, 15, 16, 17, 19):
+        ctx = _ctx(c, p=p, lmax=3)
+        errs[p] = _rel(_apply(ctx, c["q"], None), yo)
+        ctx.bem_destroy()
+    print({p: f"{e:.2e}" for p, e in errs.items()})
+    ps = sorted(errs)
+    assert all(errs[b] < 1.05 * errs[a] for a, b in zip(ps, ps[1:]))
+    assert errs[4] < 5e-3 and errs[9] < 3e-5 and errs[13] < 1e-6 and errs[17] < 5e-8 and errs[19] < 1e-8
+
+
+def test_gemm_paths_agree():
+    """Option gemm_path: the FP64 tensor tiles and the plain-FMA tiles compute the same translations."""
+    c = cfg(2)
+    ctx = _ctx(c, p=10)
+    y0 = _apply(ctx, c["q"], c["phi"])
+    ctx.bem_set_option("gemm_path", 1)
+    y1 = _apply(ctx, c["q"], c["phi"])
+    ctx.bem_destroy()
+    assert _rel(y1, y0) <= 1e-13
