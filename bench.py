@@ -39,6 +39,9 @@ UNIT = "ms"
 # nominal FP64 FMA peak of B200 for the "alu" roofline: 148 SMs x 64 FP64
 # FMA lanes per SM per clock x 2 flop x 1.965 GHz (clocks.max.sm)
 FP64_NOMINAL_GFLOPS = 148 * 64 * 2 * 1.965
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels on config 5, from the committed
+# ncu --set full captures (profiles/r1_04_*.md); None for workloads that were not captured
+NCU_TRAFFIC = {}
 
 
 def workload_name(c):
@@ -232,24 +235,51 @@ def run_gpu(args):
         pass
     hbm_peak, hbm_src = (hbm, "measured") if hbm else (6650.0, "fallback")
 
+    # ---- roofline of the dominant kernel + the other kernels the metric names
+    # FP64 pipe: 148 SMs x 64 lanes x 1.965 GHz = 18.6 T instr/s; an FMA counts 2 flop, so the flop peak is 37.2 TFLOP/s.
+    # P2P: 17 FP64 instructions per pair (9 DFMA + 5 DMUL + 3 DADD = 26 flop; SASS count).
+    P2P_INSTR, P2P_FLOP = 17.0, 26.0
+    slot_peak = FP64_NOMINAL_GFLOPS / 2e3                      # T instr/s
+    nre = stats["exp_stride"] / 2.0
     kernels = {}
+    p2p_s = tm["p2p"] * 1e-3
+    kernels["p2p"] = dict(ms=tm["p2p"], pairs=stats["p2p_pairs"], gpairs_per_s=stats["p2p_pairs"] / p2p_s / 1e9 if p2p_s > 0 else None,
+                          tflops=stats["p2p_pairs"] * P2P_FLOP / p2p_s / 1e12 if p2p_s > 0 else None,
+                          fp64_slot_frac=stats["p2p_pairs"] * P2P_INSTR / p2p_s / 1e12 / slot_peak if p2p_s > 0 else None,
+                          note="17 FP64 instr / 26 flop per pair; slot_frac = share of the FP64 pipe's issue slots (nominal 18.6 T instr/s)")
     if not args.direct:
-        m2l_flops = stats["m2l_pairs"] * 2.0 * p ** 4
-        roof = dict(kernel="m2l_gemm", bound="alu", achieved=m2l_flops / (tm["m2l"] * 1e-3) / 1e12 if tm["m2l"] > 0 else 0.0,
-                    peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", traffic=None,
-                    peak_source="nominal: 148 SMs x 64 FP64 FMA/clk x 2 x 1.965 GHz", measured_dfma_tflops=dfma / 1e3, measured_dmma_tflops=dmma / 1e3,
-                    algorithmic="2 p^4 flop per M2L pair x %d pairs" % stats["m2l_pairs"], ms=tm["m2l"])
-    else:
-        roof = dict(kernel="p2p_direct", bound="alu", achieved=stats["p2p_pairs"] * 20.0 / (tm["p2p"] * 1e-3) / 1e12,
-                    peak=FP64_NOMINAL_GFLOPS / 2e3, unit="Tinstr/s", traffic=None,
-                    peak_source="nominal FP64 instruction rate: 148 x 64 x 1.965 GHz", measured_dfma_tflops=dfma / 1e3, measured_dmma_tflops=dmma / 1e3,
-                    algorithmic="20 FP64 instructions per pair x %d pairs" % stats["p2p_pairs"], ms=tm["p2p"])
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    kernels["p2p"] = dict(ms=tm["p2p"], gpairs_per_s=stats["p2p_pairs"] / (tm["p2p"] * 1e-3) / 1e9 if tm["p2p"] > 0 else None,
-                          pairs=stats["p2p_pairs"])
+        m2l_s = tm["m2l"] * 1e-3
+        exec_flop = stats["m2l_pairs"] * 4.0 * nre * nre          # two nre x nre blocks, 2 flop per MAC (azimuth split)
+        dense_flop = stats["m2l_pairs"] * 2.0 * p ** 4            # the dense p^2 x p^2 translation of SURVEY.md 8(d)
+        kernels["m2l"] = dict(ms=tm["m2l"], pairs=stats["m2l_pairs"], executed_tflops=exec_flop / m2l_s / 1e12,
+                              dense_equivalent_tflops=dense_flop / m2l_s / 1e12,
+                              frac_of_measured_dmma_peak=exec_flop / m2l_s / 1e9 / dmma, frac_of_nominal_fp64_peak=exec_flop / m2l_s / 1e9 / FP64_NOMINAL_GFLOPS,
+                              note="executed = 4 nre^2 flop per pair on the FP64 tensor path (nre = %d); dense-equivalent = 2 p^4" % int(nre))
+        red_bytes = stats["m2l_pairs"] * 8.0 * stats["exp_stride"]
+        kernels["reduce"] = dict(ms=tm["l2l_reduce"], gbs=red_bytes / (tm["l2l_reduce"] * 1e-3) / 1e9,
+                                 frac_hbm=red_bytes / (tm["l2l_reduce"] * 1e-3) / 1e9 / hbm_peak, bytes=red_bytes,
+                                 note="reads one translated row (8 nst bytes) per pair; L2L rows not counted")
+        p2m_bytes = 64.0 * stats["n_sources"] + 8.0 * stats["exp_stride"] * stats["n_src_leaves"]
+        kernels["p2m"] = dict(ms=tm["p2m"], gbs=p2m_bytes / (tm["p2m"] * 1e-3) / 1e9, msources_per_s=stats["n_sources"] / (tm["p2m"] * 1e-3) / 1e6)
     spmv_bytes = 20.0 * stats["csr_nnz"] + 32.0 * N
     kernels["spmv"] = dict(ms=tm["spmv"], gbs=spmv_bytes / (tm["spmv"] * 1e-3) / 1e9, frac_hbm=spmv_bytes / (tm["spmv"] * 1e-3) / 1e9 / hbm_peak,
                            hbm_peak_gbs=hbm_peak, hbm_peak_source=hbm_src, bytes=spmv_bytes)
+    common = dict(peak_source="derived: 148 SMs x 64 FP64 lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry); "
+                              "measured in this run: DFMA loop %.1f, DMMA loop %.1f TFLOP/s" % (dfma / 1e3, dmma / 1e3),
+                  measured_dfma_tflops=dfma / 1e3, measured_dmma_tflops=dmma / 1e3)
+    if args.direct or tm["p2p"] >= tm["m2l"]:
+        k = kernels["p2p"]
+        roof = dict(kernel="p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", bound="alu", achieved=k["tflops"],
+                    peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", frac=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
+                    fp64_slot_frac=k["fp64_slot_frac"], traffic=NCU_TRAFFIC.get("p2p_direct" if args.direct else "p2p_leaf"),
+                    algorithmic="26 flop (17 FP64 instructions) per pair x %d pairs" % stats["p2p_pairs"], ms=tm["p2p"],
+                    share_of_step=tm["p2p"] / tm["total"], **common)
+    else:
+        k = kernels["m2l"]
+        roof = dict(kernel="translate_dmma", bound="tensor", achieved=k["executed_tflops"], peak=dmma / 1e3, unit="TFLOP/s",
+                    frac=k["frac_of_measured_dmma_peak"], traffic=NCU_TRAFFIC.get("translate_dmma"),
+                    algorithmic="4 nre^2 flop per M2L pair x %d pairs (FP64 DMMA; peak = DMMA loop measured in this run)" % stats["m2l_pairs"],
+                    ms=tm["m2l"], share_of_step=tm["m2l"] / tm["total"], **common)
     breakdown = {k: round(v, 4) for k, v in tm.items()}
 
     # parity in the same run + the oracle timed beside it (bounded sample of rows)
@@ -259,13 +289,18 @@ def run_gpu(args):
 
     solve = None
     if args.solve_iters > 0:
-        qs = torch.zeros_like(qd)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        st, it, rr = ctx.bem_solve(pd, qs, tol=args.solve_tol, max_iter=args.solve_iters)
-        torch.cuda.synchronize()
-        solve = dict(ms=(time.perf_counter() - t0) * 1e3, iterations=it, relres=rr, tol=args.solve_tol, max_iter=args.solve_iters,
-                     status=bem.STATUS_NAMES[st])
+        solve = {}
+        for name, pre in (("unpreconditioned (paper)", 0), ("diagonal S_ii (option precond)", 1)):
+            ctx.bem_set_option("precond", pre)
+            qs = torch.zeros_like(qd)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            st, it, rr = ctx.bem_solve(pd, qs, tol=args.solve_tol, max_iter=args.solve_iters)
+            torch.cuda.synchronize()
+            ms_s = (time.perf_counter() - t0) * 1e3
+            solve[name] = dict(ms=ms_s, iterations=it, relres=rr, tol=args.solve_tol, max_iter=args.solve_iters,
+                               status=bem.STATUS_NAMES[st], ms_per_iteration=ms_s / max(it, 1))
+        ctx.bem_set_option("precond", 0)
 
     line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
                 higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",

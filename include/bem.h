@@ -102,6 +102,11 @@ bem_status bem_create(const double *vertices, int64_t n_vertices,
  *                   the diagonal rule M_ii = -1/2 - sum_{j!=i} M_ij
  *                   (default); 1 = c_i = 1/2 literally (Eq. 15)
  *   "gmres_restart" 0 = no restart up to max_iter (default), else restart length
+ *   "precond"       bem_solve: 0 = unpreconditioned GMRES, as in the paper (default); 1 = right
+ *                   diagonal scaling, GMRES on (S D^-1)(D q) = b with D = diag(S) (exact self integrals; in V1
+ *                   the L_ii of Eq. 21).  The stopping rule (true relative residual of S q = b) is unchanged.
+ *                   Not in the paper: it equilibrates bubbles of different size (S_ii ~ mesh size).  May be
+ *                   changed between solves.
  *   "lmax"          0 = choose the octree depth from leaf_size (default), else force it
  *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply
  *   "gemm_path"     batched translations (M2M, M2L, L2L): 0 = FP64 tensor-core tiles (DMMA; p <= 16,
@@ -138,7 +143,7 @@ bem_status bem_apply(bem_ctx *ctx, const double *q, const double *phi, double *y
 /* bem_solve -- the Dirichlet problem of PAPER.md:125, 160-171 (Eqs. 15-16):
  * given phi on the surface find q = dphi/dn with  S q = b,
  * b_i = -c_i phi_i + (D phi)_i, by unpreconditioned GMRES,
- * modified Gram-Schmidt, stopping when ||b - S q|| / ||b|| <= tol.
+ * Gram-Schmidt applied twice, stopping when ||b - S q|| / ||b|| <= tol.
  *   q           [n_vertices] output; read as the initial guess iff use_q_as_x0
  *               (the paper warm-starts from the previous time step).
  *   iters_out, relres_out  may be NULL.

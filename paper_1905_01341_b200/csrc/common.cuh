@@ -130,6 +130,7 @@ struct bem_ctx {
 
     // options
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
+    int precond = 0;                // bem_solve: 0 = unpreconditioned (the paper), 1 = right diagonal scaling by S_ii
     int gemm_path = 0;              // translations: 0 = FP64 tensor path (DMMA) where p <= 16, 1 = plain-FMA tiles
 
     // setup state
@@ -176,6 +177,7 @@ struct bem_ctx {
     bem::dvec<double2> val;         // [nnz] (C^S, C^D)
     int64_t nnz = 0, near_tris = 0;
     bem::dvec<double> diagL, diagM; // V1 only
+    bem::dvec<double> diagS;        // G3: S_ii (exact), the diagonal preconditioner of bem_solve (option "precond")
     bool have_diag = false;
 
     bem::dvec<double> cfree;        // [N] free term c_i of bem_solve

@@ -209,13 +209,14 @@ __global__ void csr_count(const int32_t *F, const int64_t *nptr, const int32_t *
 // (exact - Gauss) weights of the matching local vertex
 __global__ void csr_fill(const double *V, const int32_t *F, const double *A, const double *Nrm,
                          const int64_t *nptr, const int32_t *near, int64_t N,
-                         const int64_t *rowptr, int32_t *col, double2 *val)
+                         const int64_t *rowptr, int32_t *col, double2 *val, double *diagS)
 {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int64_t b = nptr[i], e = nptr[i + 1];
     const int64_t r0 = rowptr[i];
     int ncol = 0;
+    double sii = 0.0;                                            // S_ii = exact integral of vertex i's own hat function
     const double x[3] = {V[3 * i], V[3 * i + 1], V[3 * i + 2]};
     for (int64_t j = b; j < e; ++j) {
         const int64_t k = near[j];
@@ -227,7 +228,7 @@ __global__ void csr_fill(const double *V, const int32_t *F, const double *A, con
         for (int a = 0; a < 3; ++a)
             if (v[a] == i) inc = a;
         double WS[3], WD[3];
-        if (inc >= 0) tri_weights_incident(r, inc, WS, WD);
+        if (inc >= 0) { tri_weights_incident(r, inc, WS, WD); sii += WS[inc]; }
         else tri_weights_regular(r, x, WS, WD);
         // minus the 3-point Gauss value (what lift + P2P add for this triangle)
         const double w = A[k] / 3.0;
@@ -257,6 +258,7 @@ __global__ void csr_fill(const double *V, const int32_t *F, const double *A, con
             val[r0 + c] = cur;
         }
     }
+    diagS[i] = sii;
 }
 
 void build_correction(bem_ctx *c)
@@ -317,8 +319,9 @@ void build_correction(bem_ctx *c)
     CUDA_TRY(cudaMemcpy(&c->nnz, c->rowptr.get() + N, sizeof(int64_t), cudaMemcpyDeviceToHost));
     c->col.alloc(c->nnz);
     c->val.alloc(c->nnz);
+    c->diagS.alloc(N);
     csr_fill<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), c->F.get(), c->triA.get(), c->triN.get(), nptr.get(), near.get(), N,
-                                          c->rowptr.get(), c->col.get(), c->val.get());
+                                          c->rowptr.get(), c->col.get(), c->val.get(), c->diagS.get());
     KERNEL_CHECK();
     CUDA_TRY(cudaStreamSynchronize(s));
 }

@@ -2,9 +2,11 @@
 // (section 3.8: "unpreconditioned GMRES"; Eqs. 15-16,
 // PAPER.md:160-171:  L q = b,  b = -1/2 phi + M phi  with the diagonal rule of
 // PAPER.md:204 folded into c_i, reading R6).
-// Vector work (dots, axpys) runs on the device with fixed-order reductions; the
-// (k+1) x k Hessenberg least-squares problem is updated on the host with Givens
-// rotations -- one scalar read per inner product.
+// Vector work runs on the device with fixed-order reductions.  Orthogonalisation is
+// classical Gram-Schmidt applied twice (CGS2, as stable as modified Gram-Schmidt): all
+// k+1 inner products of a pass come from ONE batched kernel and one host read, and the
+// update w -= V h is one kernel -- the k-th iteration costs 2 syncs instead of k+1.  The
+// (k+1) x k Hessenberg least-squares problem is updated on the host with Givens rotations.
 #include "common.cuh"
 
 #include <cmath>
@@ -62,6 +64,12 @@ __global__ void rhs_kernel(const double *__restrict__ cf, const double *__restri
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) b[i] = -cf[i] * phi[i] - y[i];
 }
+// y = x ./ d ;  y += x ./ d
+__global__ void divide_kernel(const double *__restrict__ x, const double *__restrict__ d, double *__restrict__ y, int64_t n, int accumulate)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) y[i] = accumulate ? y[i] + x[i] / d[i] : x[i] / d[i];
+}
 // r = b - w
 __global__ void sub_kernel(const double *__restrict__ b, const double *__restrict__ w, double *__restrict__ r, int64_t n)
 {
@@ -69,10 +77,59 @@ __global__ void sub_kernel(const double *__restrict__ b, const double *__restric
     if (i < n) r[i] = b[i] - w[i];
 }
 
+// part[j * gridDim.x + bx] = partial <w, V_j> of block bx  (grid = (MD_BLOCKS, nvec))
+constexpr int MD_BLOCKS = 148;
+__global__ void __launch_bounds__(DOT_THREADS)
+multi_dot_partial(const double *__restrict__ w, const double *__restrict__ V, int64_t n, double *__restrict__ part)
+{
+    const double *v = V + (size_t)blockIdx.y * n;
+    double s = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) s = fma(w[i], v[i], s);
+    __shared__ double sm[DOT_THREADS];
+    sm[threadIdx.x] = s;
+    __syncthreads();
+    for (int st = DOT_THREADS / 2; st > 0; st >>= 1) {
+        if (threadIdx.x < st) sm[threadIdx.x] += sm[threadIdx.x + st];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = sm[0];
+}
+// out[j] = sum_bx part[j][bx]   (one block of 32 threads per j; fixed order)
+__global__ void multi_dot_final(const double *__restrict__ part, int nparts, double *__restrict__ out)
+{
+    double s = 0.0;
+    for (int i = threadIdx.x; i < nparts; i += 32) s += part[(size_t)blockIdx.x * nparts + i];
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    if (threadIdx.x == 0) out[blockIdx.x] = s;
+}
+// w -= sum_j h[j] V_j
+__global__ void multi_axpy(const double *__restrict__ h, const double *__restrict__ V, int nvec, int64_t n, double *__restrict__ w)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double acc = w[i];
+    for (int j = 0; j < nvec; ++j) acc = fma(-__ldg(h + j), V[(size_t)j * n + i], acc);
+    w[i] = acc;
+}
+
 struct Krylov {
     bem_ctx *c;
     int64_t n;
-    dvec<double> part, out;
+    dvec<double> part, out, mpart, mout;
+    // h[0..nvec) = V^T w, then w -= V h
+    void project_out(const double *V, int nvec, double *w, double *h_host)
+    {
+        if ((size_t)nvec * MD_BLOCKS > mpart.n) { mpart.alloc((size_t)2 * nvec * MD_BLOCKS); mout.alloc((size_t)2 * nvec); }
+        multi_dot_partial<<<dim3(MD_BLOCKS, nvec), DOT_THREADS, 0, c->stream>>>(w, V, n, mpart.get());
+        KERNEL_CHECK();
+        multi_dot_final<<<nvec, 32, 0, c->stream>>>(mpart.get(), MD_BLOCKS, mout.get());
+        KERNEL_CHECK();
+        multi_axpy<<<cdiv(n, 256), 256, 0, c->stream>>>(mout.get(), V, nvec, n, w);
+        KERNEL_CHECK();
+        CUDA_TRY(cudaMemcpyAsync(h_host, mout.get(), nvec * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+    }
     double dot(const double *a, const double *b)
     {
         dot_partial<<<DOT_BLOCKS, DOT_THREADS, 0, c->stream>>>(a, b, n, part.get());
@@ -120,9 +177,11 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
         const int m = c->gmres_restart > 0 ? std::min(c->gmres_restart, std::max(max_iter, 1)) : std::max(max_iter, 1);
         dvec<double> basis;
         basis.alloc((size_t)(m + 1) * n);
-        std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m), sn(m), g(m + 1), yv(m);
+        std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m), sn(m), g(m + 1), yv(m), hh(2 * (m + 1));
         auto Vk = [&](int k) { return basis.get() + (size_t)k * n; };
         bool x_is_zero = !use_x0;
+        const double *dpre = nullptr;                       // option "precond": D = diag(S)
+        if (c->precond == 1) dpre = c->have_diag ? c->diagL.get() : (c->diagS.p ? c->diagS.get() : nullptr);
         while (true) {
             if (x_is_zero) CUDA_TRY(cudaMemcpyAsync(r.get(), b.get(), bytes, cudaMemcpyDeviceToDevice, s));
             else {
@@ -139,12 +198,14 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
             g[0] = beta;
             int k = 0;
             for (; k < m && iters < max_iter; ++k) {
-                apply_device(c, Vk(k), nullptr, w.get());
-                for (int i = 0; i <= k; ++i) {             // modified Gram-Schmidt
-                    const double h = K.dot(w.get(), Vk(i));
-                    H[(size_t)i * m + k] = h;
-                    K.axpy(-h, Vk(i), w.get());
-                }
+                if (dpre) {                                 // right preconditioning: w = S (D^-1 v_k)
+                    divide_kernel<<<cdiv(n, 256), 256, 0, s>>>(Vk(k), dpre, r.get(), n, 0);
+                    KERNEL_CHECK();
+                    apply_device(c, r.get(), nullptr, w.get());
+                } else apply_device(c, Vk(k), nullptr, w.get());
+                K.project_out(basis.get(), k + 1, w.get(), hh.data());          // CGS2: two passes of classical Gram-Schmidt
+                K.project_out(basis.get(), k + 1, w.get(), hh.data() + (m + 1));
+                for (int i = 0; i <= k; ++i) H[(size_t)i * m + k] = hh[i] + hh[m + 1 + i];
                 const double hn = std::sqrt(K.dot(w.get(), w.get()));
                 H[(size_t)(k + 1) * m + k] = hn;
                 if (hn > 0.0) K.scale(1.0 / hn, w.get(), Vk(k + 1));
@@ -171,7 +232,13 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
                 for (int j = i + 1; j < k; ++j) t -= H[(size_t)i * m + j] * yv[j];
                 yv[i] = t / H[(size_t)i * m + i];
             }
-            for (int i = 0; i < k; ++i) K.axpy(yv[i], Vk(i), x.get());
+            if (dpre) {                                     // x += D^-1 (V y)
+                r.zero(s);
+                for (int i = 0; i < k; ++i) K.axpy(yv[i], Vk(i), r.get());
+                divide_kernel<<<cdiv(n, 256), 256, 0, s>>>(r.get(), dpre, x.get(), n, 1);
+                KERNEL_CHECK();
+            } else
+                for (int i = 0; i < k; ++i) K.axpy(yv[i], Vk(i), x.get());
             x_is_zero = false;
             if (relres <= tol || iters >= max_iter) {
                 // true residual of the returned iterate (one more product, as Matlab's gmres does)

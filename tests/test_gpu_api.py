@@ -253,3 +253,22 @@ def test_timings_and_stats():
     t = ctx.bem_get_timings()
     assert t["total"] > 0 and abs(sum(v for k, v in t.items() if k != "total") - t["total"]) < 0.2 * t["total"] + 0.05
     assert ctx.bem_fp64_peak() > 1000.0           # GFLOP/s
+
+
+def test_solve_diagonal_preconditioner_same_solution_fewer_iterations():
+    """Option precond = 1 (right scaling by S_ii) solves the same system: same q to the tolerance, and on a
+    polydisperse cluster (config 4 recipe, radii spread 3x) in fewer iterations."""
+    c = make_config(4, n_bubbles=12)
+    V, F, bid, phi = c["V"], c["F"], c["bubble_id"], c["phi"]
+    ctx = _mk(V, F, bid, p=12)
+    res = {}
+    for pre in (0, 1):
+        ctx.bem_set_option("precond", pre)
+        q = np.zeros(V.shape[0])
+        st, it, rr = ctx.bem_solve(phi, q, tol=1e-8, max_iter=400)
+        assert st == 0 and rr <= 1e-8
+        res[pre] = (q, it)
+    ctx.bem_destroy()
+    print("iterations", res[0][1], res[1][1])
+    assert _rel(res[1][0], res[0][0]) <= 1e-5          # cond(S) ~ 1e2-1e3 times the residual tolerance
+    assert res[1][1] < res[0][1]
