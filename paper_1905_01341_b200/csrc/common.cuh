@@ -151,6 +151,7 @@ struct bem_ctx {
     bem::dvec<double4> lift_w;      // [ns] (w, w Nx, w Ny, w Nz)
     bem::dvec<int4> lift_vid;       // [ns] (v0, v1, v2, -) densities are 2/3 f[v0] + 1/6 f[v1] + 1/6 f[v2]
     bem::dvec<double4> src_str;     // [ns] (m, dx, dy, dz), rewritten by every apply
+    bool has_dipole = true;         // false while phi == NULL: dipole strengths are all zero
     // targets in engine order
     bem::dvec<double> tgt_pos;      // [N*3]
     bem::dvec<uint32_t> tgt_inv;    // [N] original vertex -> engine position (FMM mode)

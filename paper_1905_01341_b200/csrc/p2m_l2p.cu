@@ -58,7 +58,7 @@ __device__ __forceinline__ void next_row(int l, double ax, double ay, double az,
 constexpr int P2M_WARPS = 4;
 constexpr int P2M_TBL = 64 * 33;
 
-template <int P>
+template <int P, bool DIP>
 __global__ void __launch_bounds__(P2M_WARPS * 32)
 p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf,
              double cmx, double cmy, double cmz, double h,
@@ -100,7 +100,7 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
             for (int m = 0; m < P; ++m) {
                 if (m <= l) {
                     double gr = 0.0, gi = 0.0;
-                    if (l > 0) {
+                    if (DIP && l > 0) {
                         const double Cr = (m <= l - 1) ? Rre[prv][m] : 0.0, Ci = (m <= l - 1) ? Rim[prv][m] : 0.0;
                         const double Ar = (m + 1 <= l - 1) ? Rre[prv][m + 1] : 0.0, Ai = (m + 1 <= l - 1) ? Rim[prv][m + 1] : 0.0;
                         double Br = 0.0, Bi = 0.0;
@@ -168,8 +168,13 @@ static void p2m_launch(bem_ctx *c)
     const double h = c->cube_side / (double)(1 << lmax);
     const size_t smem = (size_t)P2M_WARPS * P2M_TBL * sizeof(double);
     static bool attr = false;
-    if (!attr) { CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-    p2m_kernel_t<P><<<cdiv(nleaf, P2M_WARPS), P2M_WARPS * 32, smem, c->stream>>>(
+    if (!attr) {
+        CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr = true;
+    }
+    auto kern = c->has_dipole ? p2m_kernel_t<P, true> : p2m_kernel_t<P, false>;
+    kern<<<cdiv(nleaf, P2M_WARPS), P2M_WARPS * 32, smem, c->stream>>>(
         sb.begin.get(), sb.bkey[lmax].get(), nleaf, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
         c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
     KERNEL_CHECK();

@@ -31,6 +31,7 @@ __global__ void lift_kernel(const double *__restrict__ q, const double *__restri
 
 void launch_lift(bem_ctx *c, const double *q, const double *phi)
 {
+    c->has_dipole = phi != nullptr;                 // the pair and P2M kernels skip the dipole terms otherwise
     lift_kernel<<<cdiv(c->ns, 256), 256, 0, c->stream>>>(q, phi, c->lift_w.get(), c->lift_vid.get(), c->ns, c->src_str.get());
     KERNEL_CHECK();
 }
@@ -52,11 +53,14 @@ __device__ __forceinline__ double rsqrt_pos(double x)
 
 // one (target, source) interaction; r2 == 0 (V1: source j = target i; "i != j") adds nothing
 // acc += that interaction (the last multiply and the accumulation are one FMA)
+// DIP = false: monopole sources only (phi == NULL, every product of a GMRES iteration): 12 FP64 instructions instead of 17
+template <bool DIP>
 __device__ __forceinline__ double pair_acc(double acc, double tx, double ty, double tz, const double4 &sp, const double4 &ss)
 {
     const double dx = tx - sp.x, dy = ty - sp.y, dz = tz - sp.z;
     const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
     const double inv = rsqrt_pos(r2);
+    if (!DIP) return fma(inv, ss.x, acc);
     const double dd = fma(ss.y, dx, fma(ss.z, dy, ss.w * dz));
     // m/r - (d.dx)/r^3 = inv * (m - dd * inv^2)
     return fma(inv, fma(-dd, inv * inv, ss.x), acc);
@@ -70,6 +74,7 @@ constexpr int P2P_TPT = 4;            // direct mode: targets per thread
 // grid = (target blocks, source splits); thread = FOUR targets, so one shared-memory source read
 // (4 x LDS.128, a broadcast) feeds four pairs -- measured with ncu, one target per thread is bound by
 // the shared-memory pipe (88% LSU wavefronts at 48% FP64), not by FP64; sources staged in tiles of 256
+template <bool DIP>
 __global__ void __launch_bounds__(P2P_THREADS)
 p2p_direct_kernel(const double *__restrict__ tgt, int64_t nt, const double4 *__restrict__ spos,
                   const double4 *__restrict__ sstr, int64_t ns, int64_t chunk, double *__restrict__ ypart)
@@ -94,7 +99,7 @@ p2p_direct_kernel(const double *__restrict__ tgt, int64_t nt, const double4 *__r
         for (int j = 0; j < n; ++j) {
             const double4 p = sp[j], q = ss[j];
 #pragma unroll
-            for (int k = 0; k < P2P_TPT; ++k) acc[k] = pair_acc(acc[k], tx[k], ty[k], tz[k], p, q);
+            for (int k = 0; k < P2P_TPT; ++k) acc[k] = pair_acc<DIP>(acc[k], tx[k], ty[k], tz[k], p, q);
         }
     }
 #pragma unroll
@@ -108,8 +113,12 @@ void launch_p2p_direct(bem_ctx *c)
 {
     const int64_t chunk = (c->ns + c->nsplit - 1) / c->nsplit;
     dim3 grid(cdiv(c->N, P2P_TPT * P2P_THREADS), c->nsplit);
-    p2p_direct_kernel<<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
-                                                           c->ns, chunk, c->ypart.get());
+    if (c->has_dipole)
+        p2p_direct_kernel<true><<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
+                                                                     c->ns, chunk, c->ypart.get());
+    else
+        p2p_direct_kernel<false><<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
+                                                                      c->ns, chunk, c->ypart.get());
     KERNEL_CHECK();
 }
 
@@ -133,6 +142,7 @@ __device__ __forceinline__ void lds_point(unsigned addr, double &x, double &y, d
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%3];\n\tld.shared.f64 %2, [%3+16];" : "=d"(x), "=d"(y), "=d"(z) : "r"(addr));
 }
 
+template <bool DIP>
 __global__ void __launch_bounds__(P2P_THREADS, 5)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
                 const int32_t *__restrict__ sbegin, const double4 *__restrict__ spos, const double4 *__restrict__ sstr,
@@ -202,7 +212,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                     for (int t = tb; t < tb + 8; ++t) {
                         double Tx, Ty, Tz;
                         lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                        acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                        acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
                     }
                 } else if (tb < ntc) {                                  // the last 1..7 targets: 4 + singles
                     if (tb + 4 <= ntc) {
@@ -210,14 +220,14 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                         for (int t = tb; t < tb + 4; ++t) {
                             double Tx, Ty, Tz;
                             lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                            acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                            acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
                         }
 #pragma unroll
                         for (int t = tb + 4; t < tb + 7; ++t) {
                             if (t < ntc) {
                                 double Tx, Ty, Tz;
                                 lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                                acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                                acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
                             }
                         }
                     } else {
@@ -226,7 +236,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                             if (t < ntc) {
                                 double Tx, Ty, Tz;
                                 lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                                acc[t] = pair_acc(acc[t], Tx, Ty, Tz, p, q);
+                                acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
                             }
                         }
                     }
@@ -263,8 +273,12 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
 void launch_p2p_leaves(bem_ctx *c)
 {
     const int nleaf = c->tb.nbox[c->tb.lmax];
-    p2p_leaf_kernel<<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
-                                                          c->src_pos.get(), c->src_str.get(), c->ypart.get());
+    if (c->has_dipole)
+        p2p_leaf_kernel<true><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
+                                                                    c->src_pos.get(), c->src_str.get(), c->ypart.get());
+    else
+        p2p_leaf_kernel<false><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
+                                                                     c->src_pos.get(), c->src_str.get(), c->ypart.get());
     KERNEL_CHECK();
 }
 
