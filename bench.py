@@ -40,8 +40,8 @@ UNIT = "ms"
 # FMA lanes per SM per clock x 2 flop x 1.965 GHz (clocks.max.sm)
 FP64_NOMINAL_GFLOPS = 148 * 64 * 2 * 1.965
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels on config 5, from the committed
-# ncu --set full captures (profiles/r1_04_*.md); None for workloads that were not captured
-NCU_TRAFFIC = {}
+# ncu --set full capture (profiles/r1_03_launches_split_m2l.md); None for workloads that were not captured
+NCU_TRAFFIC = {"p2p_leaf": 1.230e9, "translate_dmma": 11.943e9}     # config 5, l_max 6, p 12 (profiles/r1_03_launches_split_m2l.md)
 
 
 def workload_name(c):
@@ -271,13 +271,13 @@ def run_gpu(args):
         k = kernels["p2p"]
         roof = dict(kernel="p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", bound="alu", achieved=k["tflops"],
                     peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", frac=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
-                    fp64_slot_frac=k["fp64_slot_frac"], traffic=NCU_TRAFFIC.get("p2p_direct" if args.direct else "p2p_leaf"),
+                    fp64_slot_frac=k["fp64_slot_frac"], traffic=NCU_TRAFFIC.get("p2p_direct" if args.direct else "p2p_leaf") if args.config == 5 else None,
                     algorithmic="26 flop (17 FP64 instructions) per pair x %d pairs" % stats["p2p_pairs"], ms=tm["p2p"],
                     share_of_step=tm["p2p"] / tm["total"], **common)
     else:
         k = kernels["m2l"]
         roof = dict(kernel="translate_dmma", bound="tensor", achieved=k["executed_tflops"], peak=dmma / 1e3, unit="TFLOP/s",
-                    frac=k["frac_of_measured_dmma_peak"], traffic=NCU_TRAFFIC.get("translate_dmma"),
+                    frac=k["frac_of_measured_dmma_peak"], traffic=NCU_TRAFFIC.get("translate_dmma") if args.config == 5 else None,
                     algorithmic="4 nre^2 flop per M2L pair x %d pairs (FP64 DMMA; peak = DMMA loop measured in this run)" % stats["m2l_pairs"],
                     ms=tm["m2l"], share_of_step=tm["m2l"] / tm["total"], **common)
     breakdown = {k: round(v, 4) for k, v in tm.items()}
