@@ -111,6 +111,7 @@ struct Stage {
     dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
     dvec<Tile> tiles;
     int ntiles = 0;
+    int ntiles_split = 0;           // the first ntiles_split tiles are M2L tiles (matrix ids < MAT_L2L come first)
 };
 
 }  // namespace bem

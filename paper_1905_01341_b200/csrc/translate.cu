@@ -341,6 +341,69 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
     }
 }
 
+// M2L tiles only (block-diagonal matrix): the lean version of the kernel above.  A warp holds ONE half of its
+// A operand at a time -- the rotated real parts while it runs the real-part columns, then (rows gathered again,
+// L2 hits) the rotated imaginary parts for the imaginary-part columns: 2 KSH instead of 4 KSH registers for A,
+// so three CTAs (24 warps) fit an SM instead of two and the row gather of one CTA hides behind the DMMAs of the
+// others (ncu on the two-CTA version: tensor pipe 65% active, 30% of the samples in the gather prologue).
+template <int KSH>
+__global__ void __launch_bounds__(DM_THREADS, (KSH <= 20 ? 3 : 2))
+translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
+                     const double *__restrict__ Mexp, const double *__restrict__ mats,
+                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, double *__restrict__ scratch)
+{
+    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
+    __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
+    constexpr int NRE = 4 * KSH, NST = 2 * NRE;
+    constexpr int NTH = KSH / 2;                               // n-tiles (8 columns) of one block
+    constexpr int CPB = (NTH + DM_NT - 1) / DM_NT;             // chunks per block
+    constexpr int CW = (NTH + CPB - 1) / CPB;                  // chunk width in n-tiles
+    const Tile tile = tiles[blockIdx.x];
+    double *Bs0 = dm_smem, *Bs1 = dm_smem + NRE * DM_S;
+    const double *B = mats + (size_t)tile.mat * NST * NST;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lr = lane >> 2, lk = lane & 3;
+    const int row = warp * 8 + lr;
+    const bool rvalid = row < tile.nrows;
+
+    auto issue = [&](int ch, double *dst) {
+        const int blk = ch >= CPB, cl = blk ? ch - CPB : ch;
+        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
+        const int c0 = 8 * t0, per_row = 4 * nt, k0 = blk * NRE;
+        for (int i = threadIdx.x; i < NRE * per_row; i += DM_THREADS) {
+            const int k = i / per_row, j = (i % per_row) * 2;
+            cp_async16(dst + k * DM_S + j, B + (size_t)(k0 + k) * NST + c0 + j);
+        }
+        cp_async_commit();
+    };
+    issue(0, Bs0);
+    for (int k = threadIdx.x; k < NRE; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
+    const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
+    const double2 *ap = reinterpret_cast<const double2 *>(Mexp + (size_t)(arow < 0 ? 0 : arow) * NST) + lk;
+    double *orow = scratch + (size_t)(tile.row0 + row) * NST + 2 * lk;
+    double a[KSH];
+
+    for (int ch = 0; ch < 2 * CPB; ++ch) {
+        double *cur = (ch & 1) ? Bs1 : Bs0;
+        const int blk = ch >= CPB, cl = blk ? ch - CPB : ch;
+        cp_async_wait<0>();
+        __syncthreads();                                        // chunk ch landed; everyone left chunk ch-1; cs_k visible
+        if (ch + 1 < 2 * CPB) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
+        if (cl == 0) {                                          // first chunk of a block: this block's half of A
+#pragma unroll
+            for (int j = 0; j < KSH / 2; ++j) {
+                double2 re = make_double2(0.0, 0.0), im = re;
+                if (arow >= 0) { re = ap[4 * j]; im = ap[4 * j + NRE / 2]; }
+                const double2 c0 = cs_k[8 * j + 2 * lk], c1 = cs_k[8 * j + 2 * lk + 1];
+                if (blk == 0) { a[2 * j] = fma(c0.x, re.x, -c0.y * im.x); a[2 * j + 1] = fma(c1.x, re.y, -c1.y * im.y); }
+                else { a[2 * j] = fma(c0.x, im.x, c0.y * re.x); a[2 * j + 1] = fma(c1.x, im.y, c1.y * re.y); }
+            }
+        }
+        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
+        dm_chunk<KSH, 0, KSH, 0>(a, cur, nt, lr, lk, rvalid, orow + 8 * t0);
+    }
+}
+
 template <int KSH>
 static void launch_dmma(bem_ctx *c, const Stage &st)
 {
@@ -348,10 +411,16 @@ static void launch_dmma(bem_ctx *c, const Stage &st)
     static bool attr_set = false;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    translate_dmma<KSH><<<st.ntiles, DM_THREADS, smem, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                                   c->mats.get(), c->kinfo.get(), c->rot.get(), c->scratch.get());
+    if (st.ntiles_split > 0)
+        translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
+                                                                                   c->mats.get(), c->kinfo.get(), c->rot.get(), c->scratch.get());
+    if (st.ntiles > st.ntiles_split)
+        translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, c->stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
+                                                                                         c->Mexp.get(), c->Lexp.get(), c->mats.get(),
+                                                                                         c->kinfo.get(), c->rot.get(), c->scratch.get());
 }
 
 // out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[pos[k]][:]   (fixed order; a_k = azimuth of

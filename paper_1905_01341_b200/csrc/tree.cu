@@ -247,6 +247,8 @@ static void finish_stage(Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cuda
     }
     st.mat_t = std::move(mat);
     st.ntiles = (int)tiles.size();
+    st.ntiles_split = 0;
+    for (const Tile &t : tiles) st.ntiles_split += (t.flags & 2) ? 1 : 0;
     st.tiles.alloc(tiles.size());
     if (!tiles.empty()) CUDA_TRY(cudaMemcpy(st.tiles.get(), tiles.data(), tiles.size() * sizeof(Tile), cudaMemcpyHostToDevice));
 }
