@@ -22,6 +22,8 @@ void build_lists(bem_ctx *c);
 // translate.cu
 void build_matrices(bem_ctx *c);
 void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce);
+void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stream);
+void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream);
 void launch_p2m(bem_ctx *c);
 void launch_l2p(bem_ctx *c, const int32_t *leaf_of);
 // p2p.cu
@@ -137,11 +139,32 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
         launch_p2m(c);
         mark(c, BEM_T_P2M);
         for (int l = lmax - 1; l >= 2; --l) launch_stage(c, c->m2m[l], BEM_T_M2M, BEM_T_M2M);
-        for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l], BEM_T_M2L, BEM_T_L2L_REDUCE);
-        launch_l2p(c, c->tb.leaf_of.get());
-        mark(c, BEM_T_L2P);
-        launch_p2p_leaves(c);
-        mark(c, BEM_T_P2P);
+        if (c->timing || !c->side) {
+            // one stream, class by class (option "timing": the per-class event times add up to the total)
+            for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l], BEM_T_M2L, BEM_T_L2L_REDUCE);
+            launch_l2p(c, c->tb.leaf_of.get());
+            mark(c, BEM_T_L2P);
+            launch_p2p_leaves(c);
+            mark(c, BEM_T_P2P);
+        } else {
+            // The M2L tiles of every level only read multipole expansions: issue them all, then fork.  The reduce
+            // passes (HBM-bound), the L2L tiles and L2P go down the levels on a high-priority side stream while the
+            // near field (P2P: FP64-bound, no HBM traffic) runs on the main stream; they meet before the SpMV.
+            cudaStream_t main = c->stream;
+            for (int l = 2; l <= lmax; ++l) launch_stage_gemm(c, c->m2l[l], TILES_SPLIT, main);
+            CUDA_TRY(cudaEventRecord(c->ev_fork, main));
+            CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+            for (int l = 2; l <= lmax; ++l) {
+                launch_stage_gemm(c, c->m2l[l], TILES_DENSE, c->side);
+                launch_stage_reduce(c, c->m2l[l], c->side);
+            }
+            c->stream = c->side;
+            launch_l2p(c, c->tb.leaf_of.get());
+            c->stream = main;
+            CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
+            launch_p2p_leaves(c);
+            CUDA_TRY(cudaStreamWaitEvent(main, c->ev_join, 0));
+        }
     }
     launch_spmv_combine(c, q, phi, y);
     mark(c, BEM_T_SPMV);
@@ -214,11 +237,18 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         c->Mexp.alloc((size_t)c->sb.total() * c->nst);
         c->Lexp.alloc((size_t)c->tb.total() * c->nst);
         build_lists(c);
-        c->nsplit = 1;
-        c->ypart.alloc(N);
+        c->nsplit = 2;                                  // far field (L2P) and near field (P2P) partial sums
+        c->ypart.alloc(2 * N);
+        if (!c->side) {
+            int lo = 0, hi = 0;
+            CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+            CUDA_TRY(cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, hi));
+            CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+            CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+        }
         int launches = 2 /*lift, p2m*/ + 3 /*l2p, p2p, spmv*/;
         for (int l = lmax - 1; l >= 2; --l) launches += 2;
-        for (int l = 2; l <= lmax; ++l) launches += 2;
+        for (int l = 2; l <= lmax; ++l) launches += l > 2 ? 3 : 2;     // M2L tiles, L2L tiles, reduce
         c->launches_per_apply = launches;
     }
 
@@ -496,6 +526,9 @@ void bem_destroy(bem_ctx *c)
     if (!c) return;
     cudaSetDevice(c->device);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->side) cudaStreamDestroy(c->side);
     delete c;
 }
 

@@ -100,8 +100,10 @@ struct BoxSet {                     // the non-empty boxes of one point set on l
 // One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
 // executed as (tiles of a dense GEMM per matrix) -> scratch rows -> fixed-order row sums.
 struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split)
+constexpr int TILES_ALL = 0, TILES_SPLIT = 1, TILES_DENSE = 2;
 struct Stage {
     int64_t npairs = 0;
+    int64_t scratch_off = 0;        // first scratch row of the stage (every M2L level has its own region; M2M stages alias row 0)
     int ntgt = 0;
     int out_base = 0;               // global index of the first target box
     bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
@@ -164,13 +166,16 @@ struct bem_ctx {
     bem::dvec<double2> rot;         // [N_MATS * ROT_M] (cos m a, sin m a): azimuth a of the M2L offset, identity for M2M / L2L
     bem::dvec<int32_t> kinfo;       // [nst] order m of every stored dof (0 for padding)
     bem::dvec<double> Mexp, Lexp;   // [total boxes * nst]
-    bem::dvec<double> scratch;      // [max pairs of a stage * nst]
+    bem::dvec<double> scratch;      // [pairs of all M2L (+ L2L) stages * nst]: one region per level, so that the tiles of all
+                                    // levels can be issued before the first reduce pass
+    cudaStream_t side = nullptr;    // high-priority stream: reduce passes + L2P run here while P2P runs on `stream`
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     std::vector<bem::Stage> m2m;    // leaf-1 .. 2
     std::vector<bem::Stage> m2l;    // 2 .. lmax (M2L + L2L of the level)
     int64_t m2l_pairs = 0, p2p_pairs = 0;
 
     // partial sums of the point engine, combined by the SpMV kernel
-    bem::dvec<double> ypart;        // [nsplit * N]
+    bem::dvec<double> ypart;        // [nsplit * N]  (FMM mode: slot 0 = far field (L2P), slot 1 = near field (P2P))
     int nsplit = 1;
 
     // near-field correction (a3) / V1 diagonal (a3')

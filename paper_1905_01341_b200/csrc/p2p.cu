@@ -131,7 +131,7 @@ void launch_p2p_direct(bem_ctx *c)
 // rounds; one transposed butterfly (31 shuffle steps) at the end leaves the sum of acc[t] over the
 // lanes in lane t, and the 4 warps are added through shared memory -- a fixed order, no atomics, so
 // two runs agree bit for bit.  Work is ~ (targets) x ceil(S/128) x 128 pairs whatever the leaf sizes.
-// y (engine order) already holds the far field (L2P).
+// The near field goes to its own slot of ypart (the far field, L2P, may still be running on the side stream).
 constexpr int P2P_WARPS = P2P_THREADS / 32;
 constexpr int P2P_NT = 16;           // targets per pass (register accumulators per lane); 8, 16 or 32
 
@@ -265,7 +265,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
             double sum = red[0][threadIdx.x];
 #pragma unroll
             for (int w = 1; w < P2P_WARPS; ++w) sum += red[w][threadIdx.x];
-            y[t0 + c0 + threadIdx.x] += sum;
+            y[t0 + c0 + threadIdx.x] = sum;
         }
     }
 }
@@ -275,10 +275,10 @@ void launch_p2p_leaves(bem_ctx *c)
     const int nleaf = c->tb.nbox[c->tb.lmax];
     if (c->has_dipole)
         p2p_leaf_kernel<true><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
-                                                                    c->src_pos.get(), c->src_str.get(), c->ypart.get());
+                                                                    c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N);
     else
         p2p_leaf_kernel<false><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
-                                                                     c->src_pos.get(), c->src_str.get(), c->ypart.get());
+                                                                     c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N);
     KERNEL_CHECK();
 }
 

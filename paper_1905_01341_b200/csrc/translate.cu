@@ -405,7 +405,7 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
 }
 
 template <int KSH>
-static void launch_dmma(bem_ctx *c, const Stage &st)
+static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t stream, double *scratch)
 {
     const size_t smem = (size_t)2 * 4 * KSH * DM_S * sizeof(double);
     static bool attr_set = false;
@@ -414,13 +414,13 @@ static void launch_dmma(bem_ctx *c, const Stage &st)
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    if (st.ntiles_split > 0)
-        translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                   c->mats.get(), c->kinfo.get(), c->rot.get(), c->scratch.get());
-    if (st.ntiles > st.ntiles_split)
-        translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, c->stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
-                                                                                         c->Mexp.get(), c->Lexp.get(), c->mats.get(),
-                                                                                         c->kinfo.get(), c->rot.get(), c->scratch.get());
+    if (which != TILES_DENSE && st.ntiles_split > 0)
+        translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
+                                                                                c->mats.get(), c->kinfo.get(), c->rot.get(), scratch);
+    if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
+        translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
+                                                                                      c->Mexp.get(), c->Lexp.get(), c->mats.get(),
+                                                                                      c->kinfo.get(), c->rot.get(), scratch);
 }
 
 // out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[pos[k]][:]   (fixed order; a_k = azimuth of
@@ -454,30 +454,46 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ po
     }
 }
 
+// the tiles of a stage (which = all, only the M2L tiles, only the dense M2M / L2L tiles) on `stream`
+void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stream)
+{
+    const int first = which == TILES_DENSE ? st.ntiles_split : 0;
+    const int last = which == TILES_SPLIT ? st.ntiles_split : st.ntiles;
+    if (st.ntgt == 0 || last <= first) return;
+    double *scratch = c->scratch.get() + (size_t)st.scratch_off * c->nst;
+    const int pl = c->pl;
+    if (c->gemm_path == 1 || pl > 16) {                         // plain-FMA tiles: p > 16, or forced (option "gemm_path")
+        dim3 grid(last - first, cdiv(c->nst, GEMM_TN));
+        translate_gemm<<<grid, GEMM_THREADS, 0, stream>>>(st.tiles.get() + first, st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
+                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, scratch);
+    }
+    else if (pl == 4) launch_dmma<4>(c, st, which, stream, scratch);     // nre / 4 of the layout for pl = 4, 6, .., 16
+    else if (pl == 6) launch_dmma<6>(c, st, which, stream, scratch);
+    else if (pl == 8) launch_dmma<10>(c, st, which, stream, scratch);
+    else if (pl == 10) launch_dmma<14>(c, st, which, stream, scratch);
+    else if (pl == 12) launch_dmma<20>(c, st, which, stream, scratch);
+    else if (pl == 14) launch_dmma<28>(c, st, which, stream, scratch);
+    else launch_dmma<34>(c, st, which, stream, scratch);
+    KERNEL_CHECK();
+}
+
+void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream)
+{
+    if (st.ntgt == 0) return;
+    double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
+    translate_reduce<<<st.ntgt, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
+        st.ptr.get(), st.pos.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
+        c->kinfo.get(), c->rot.get(), c->nre, out);
+    KERNEL_CHECK();
+}
+
+// one stage start to end on the context's stream
 void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
 {
     if (st.ntgt == 0) return;
-    if (st.ntiles > 0) {
-        const int pl = c->pl;
-        if (c->gemm_path == 1 || pl > 16) {                     // plain-FMA tiles: p > 16, or forced (option "gemm_path")
-            dim3 grid(st.ntiles, cdiv(c->nst, GEMM_TN));
-            translate_gemm<<<grid, GEMM_THREADS, 0, c->stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                                 c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, c->scratch.get());
-        }
-        else if (pl == 4) launch_dmma<4>(c, st);                // nre / 4 of the layout for pl = 4, 6, .., 16
-        else if (pl == 6) launch_dmma<6>(c, st);
-        else if (pl == 8) launch_dmma<10>(c, st);
-        else if (pl == 10) launch_dmma<14>(c, st);
-        else if (pl == 12) launch_dmma<20>(c, st);
-        else if (pl == 14) launch_dmma<28>(c, st);
-        else launch_dmma<34>(c, st);
-        KERNEL_CHECK();
-        mark(c, cls_gemm);
-    }
-    double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
-    translate_reduce<<<st.ntgt, std::min(160, ((c->nre + 31) / 32) * 32), 0, c->stream>>>(st.ptr.get(), st.pos.get(), st.mat_t.get(), c->scratch.get(),
-                                                     c->kinfo.get(), c->rot.get(), c->nre, out);
-    KERNEL_CHECK();
+    launch_stage_gemm(c, st, TILES_ALL, c->stream);
+    if (st.ntiles > 0) mark(c, cls_gemm);
+    launch_stage_reduce(c, st, c->stream);
     mark(c, cls_reduce);
 }
 

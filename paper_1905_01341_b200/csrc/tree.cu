@@ -302,7 +302,8 @@ void build_lists(bem_ctx *c)
         KERNEL_CHECK();
         finish_stage(st, src, mat, s);
         c->m2l_pairs += total - (l > 2 ? nt : 0);
-        max_pairs = std::max<int64_t>(max_pairs, total);
+        st.scratch_off = max_pairs;                           // regions of the levels one after the other
+        max_pairs += total;
     }
     // M2M stages: parents on level l = lmax-1 .. 2
     c->m2m.clear();
@@ -322,6 +323,7 @@ void build_lists(bem_ctx *c)
         m2m_pairs<<<cdiv(nc, 256), 256, 0, s>>>(sb.bkey[l + 1].get(), nc, sb.base[l + 1], src.get(), mat.get());
         KERNEL_CHECK();
         finish_stage(st, src, mat, s);
+        st.scratch_off = 0;                                   // M2M runs before any M2L tile: aliases the first region
         max_pairs = std::max<int64_t>(max_pairs, nc);
     }
     c->scratch.alloc((size_t)max_pairs * c->nst);
