@@ -409,6 +409,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
     else if (!strcmp(key, "lmax")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->force_lmax = v; c->ready = false; }
     else if (!strcmp(key, "timing")) { c->timing = v != 0; }
+    else if (!strcmp(key, "m2l_rows16")) { c->m2l_rows16 = v != 0; }
     else if (!strcmp(key, "precond")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->precond = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }

@@ -404,6 +404,107 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
     }
 }
 
+// Same, 4 warps x 16 rows: every B fragment read from shared memory feeds TWO DMMAs (the two 8-row groups of the
+// warp).  ncu on the 8 x 8-row version: LSU wavefronts 55% with the tensor pipe at 65% -- the fragment loads
+// (2 wavefronts per DMMA), the cp.async fills, the row gather and the stores share one pipe.
+constexpr int DM16_THREADS = 128;
+template <int KSH, int NT>
+__device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KSH], const double (&a1)[KSH], const double *cur, int lr, int lk,
+                                              bool v0, bool v1, double *o0, double *o1)
+{
+    const double *bp = cur + 2 * lk * DM_S + lr;
+    double c0[NT][2], c1[NT][2];
+#pragma unroll
+    for (int j = 0; j < NT; ++j) c0[j][0] = c0[j][1] = c1[j][0] = c1[j][1] = 0.0;
+#pragma unroll
+    for (int s = 0; s < KSH; ++s) {
+        const double *b = bp + (8 * (s >> 1) + (s & 1)) * DM_S;
+#pragma unroll
+        for (int j = 0; j < NT; ++j) {
+            const double bv = b[8 * j];
+            dmma884(c0[j][0], c0[j][1], a0[s], bv);
+            dmma884(c1[j][0], c1[j][1], a1[s], bv);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < NT; ++j) {
+        if (v0) *reinterpret_cast<double2 *>(o0 + 8 * j) = make_double2(c0[j][0], c0[j][1]);
+        if (v1) *reinterpret_cast<double2 *>(o1 + 8 * j) = make_double2(c1[j][0], c1[j][1]);
+    }
+}
+
+template <int KSH>
+__global__ void __launch_bounds__(DM16_THREADS, 3)
+translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
+                       const double *__restrict__ Mexp, const double *__restrict__ mats,
+                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, double *__restrict__ scratch)
+{
+    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
+    __shared__ double2 cs_k[4 * KSH];
+    constexpr int NRE = 4 * KSH, NST = 2 * NRE;
+    constexpr int NTH = KSH / 2;
+    constexpr int CPB = (NTH + DM_NT - 1) / DM_NT;
+    constexpr int CW = (NTH + CPB - 1) / CPB;
+    const Tile tile = tiles[blockIdx.x];
+    double *Bs0 = dm_smem, *Bs1 = dm_smem + NRE * DM_S;
+    const double *B = mats + (size_t)tile.mat * NST * NST;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int lr = lane >> 2, lk = lane & 3;
+    const int row0 = warp * 16 + lr, row1 = row0 + 8;
+    const bool v0 = row0 < tile.nrows, v1 = row1 < tile.nrows;
+
+    auto issue = [&](int ch, double *dst) {
+        const int blk = ch >= CPB, cl = blk ? ch - CPB : ch;
+        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
+        const int c0 = 8 * t0, per_row = 4 * nt, k0 = blk * NRE;
+        for (int i = threadIdx.x; i < NRE * per_row; i += DM16_THREADS) {
+            const int k = i / per_row, j = (i % per_row) * 2;
+            cp_async16(dst + k * DM_S + j, B + (size_t)(k0 + k) * NST + c0 + j);
+        }
+        cp_async_commit();
+    };
+    issue(0, Bs0);
+    for (int k = threadIdx.x; k < NRE; k += DM16_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
+    const int ar0 = v0 ? src_sorted[tile.row0 + row0] : -1, ar1 = v1 ? src_sorted[tile.row0 + row1] : -1;
+    const double2 *ap0 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar0 < 0 ? 0 : ar0) * NST) + lk;
+    const double2 *ap1 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar1 < 0 ? 0 : ar1) * NST) + lk;
+    double *o0 = scratch + (size_t)(tile.row0 + row0) * NST + 2 * lk;
+    double *o1 = scratch + (size_t)(tile.row0 + row1) * NST + 2 * lk;
+    double a0[KSH], a1[KSH];
+
+    for (int ch = 0; ch < 2 * CPB; ++ch) {
+        double *cur = (ch & 1) ? Bs1 : Bs0;
+        const int blk = ch >= CPB, cl = blk ? ch - CPB : ch;
+        cp_async_wait<0>();
+        __syncthreads();
+        if (ch + 1 < 2 * CPB) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
+        if (cl == 0) {
+#pragma unroll
+            for (int j = 0; j < KSH / 2; ++j) {
+                const double2 z = make_double2(0.0, 0.0);
+                const double2 re0 = ar0 >= 0 ? ap0[4 * j] : z, im0 = ar0 >= 0 ? ap0[4 * j + NRE / 2] : z;
+                const double2 re1 = ar1 >= 0 ? ap1[4 * j] : z, im1 = ar1 >= 0 ? ap1[4 * j + NRE / 2] : z;
+                const double2 c0 = cs_k[8 * j + 2 * lk], c1 = cs_k[8 * j + 2 * lk + 1];
+                if (blk == 0) {
+                    a0[2 * j] = fma(c0.x, re0.x, -c0.y * im0.x); a0[2 * j + 1] = fma(c1.x, re0.y, -c1.y * im0.y);
+                    a1[2 * j] = fma(c0.x, re1.x, -c0.y * im1.x); a1[2 * j + 1] = fma(c1.x, re1.y, -c1.y * im1.y);
+                } else {
+                    a0[2 * j] = fma(c0.x, im0.x, c0.y * re0.x); a0[2 * j + 1] = fma(c1.x, im0.y, c1.y * re0.y);
+                    a1[2 * j] = fma(c0.x, im1.x, c0.y * re1.x); a1[2 * j + 1] = fma(c1.x, im1.y, c1.y * re1.y);
+                }
+            }
+        }
+        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
+        switch (nt) {
+        case 5: dm16_chunk_nt<KSH, 5>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
+        case 4: dm16_chunk_nt<KSH, 4>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
+        case 3: dm16_chunk_nt<KSH, 3>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
+        case 2: dm16_chunk_nt<KSH, 2>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
+        default: dm16_chunk_nt<KSH, 1>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
+        }
+    }
+}
+
 template <int KSH>
 static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t stream, double *scratch)
 {
@@ -412,11 +513,17 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (KSH == 20) CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split16<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set = true;
     }
-    if (which != TILES_DENSE && st.ntiles_split > 0)
-        translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                c->mats.get(), c->kinfo.get(), c->rot.get(), scratch);
+    if (which != TILES_DENSE && st.ntiles_split > 0) {
+        if (KSH == 20 && c->m2l_rows16)                          // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
+            translate_dmma_split16<(KSH == 20 ? KSH : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
+                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->kinfo.get(), c->rot.get(), scratch);
+        else
+            translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
+                                                                                    c->mats.get(), c->kinfo.get(), c->rot.get(), scratch);
+    }
     if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
         translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
                                                                                       c->Mexp.get(), c->Lexp.get(), c->mats.get(),
