@@ -102,6 +102,9 @@ bem_status bem_create(const double *vertices, int64_t n_vertices,
  *                   the diagonal rule M_ii = -1/2 - sum_{j!=i} M_ij
  *                   (default); 1 = c_i = 1/2 literally (Eq. 15)
  *   "gmres_restart" 0 = no restart up to max_iter (default), else restart length
+ *   "reduce_ctas"   bem_apply sums the translated M2L rows per target on a side stream while the near field runs;
+ *                   that pass is a persistent grid of this many CTAs per SM (1..32; 0 = chosen in bem_setup from
+ *                   the pair counts so that it ends just before the near field does; default).  Tuning only.
  *   "m2l_rows16"    M2L tiles at p = 11, 12: 1 = 4 warps x 16 rows per CTA (default), 0 = 8 warps x 8 rows.
  *                   A tuning switch: both compute the same tiles.  May be changed between products.
  *   "precond"       bem_solve: 0 = unpreconditioned GMRES, as in the paper (default); 1 = right

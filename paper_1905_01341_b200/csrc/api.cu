@@ -23,7 +23,7 @@ void build_lists(bem_ctx *c);
 void build_matrices(bem_ctx *c);
 void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce);
 void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stream);
-void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream);
+void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int ctas_per_sm);
 void launch_p2m(bem_ctx *c);
 void launch_l2p(bem_ctx *c, const int32_t *leaf_of);
 // p2p.cu
@@ -142,28 +142,26 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
         if (c->timing || !c->side) {
             // one stream, class by class (option "timing": the per-class event times add up to the total)
             for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l], BEM_T_M2L, BEM_T_L2L_REDUCE);
+            for (int l = 3; l <= lmax; ++l) launch_stage(c, c->l2l[l], BEM_T_L2L_REDUCE, BEM_T_L2L_REDUCE);
             launch_l2p(c, c->tb.leaf_of.get());
             mark(c, BEM_T_L2P);
             launch_p2p_leaves(c);
             mark(c, BEM_T_P2P);
         } else {
-            // The M2L tiles of every level only read multipole expansions: issue them all, then fork.  The reduce
-            // passes (HBM-bound), the L2L tiles and L2P go down the levels on a high-priority side stream while the
-            // near field (P2P: FP64-bound, no HBM traffic) runs on the main stream; they meet before the SpMV.
+            // The M2L tiles of every level only read multipole expansions: issue them all, then fork.  The per-level
+            // sums of the translated rows (HBM-bound, independent of each other) run on a high-priority side stream
+            // while the near field (P2P: FP64-bound, no HBM traffic) runs on the main stream; after the join the short
+            // downward pass L(l) += L2L L(l-1) and L2P follow on the main stream.
             cudaStream_t main = c->stream;
-            for (int l = 2; l <= lmax; ++l) launch_stage_gemm(c, c->m2l[l], TILES_SPLIT, main);
+            for (int l = 2; l <= lmax; ++l) launch_stage_gemm(c, c->m2l[l], TILES_ALL, main);
             CUDA_TRY(cudaEventRecord(c->ev_fork, main));
             CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-            for (int l = 2; l <= lmax; ++l) {
-                launch_stage_gemm(c, c->m2l[l], TILES_DENSE, c->side);
-                launch_stage_reduce(c, c->m2l[l], c->side);
-            }
-            c->stream = c->side;
-            launch_l2p(c, c->tb.leaf_of.get());
-            c->stream = main;
+            for (int l = lmax; l >= 2; --l) launch_stage_reduce(c, c->m2l[l], c->side, c->reduce_ctas_eff);
             CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
             launch_p2p_leaves(c);
             CUDA_TRY(cudaStreamWaitEvent(main, c->ev_join, 0));
+            for (int l = 3; l <= lmax; ++l) launch_stage(c, c->l2l[l], BEM_T_L2L_REDUCE, BEM_T_L2L_REDUCE);
+            launch_l2p(c, c->tb.leaf_of.get());
         }
     }
     launch_spmv_combine(c, q, phi, y);
@@ -240,15 +238,25 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         c->nsplit = 2;                                  // far field (L2P) and near field (P2P) partial sums
         c->ypart.alloc(2 * N);
         if (!c->side) {
+            CUDA_TRY(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device));
             int lo = 0, hi = 0;
             CUDA_TRY(cudaDeviceGetStreamPriorityRange(&lo, &hi));
             CUDA_TRY(cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, hi));
             CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
             CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
         }
+        {
+            // CTAs per SM of the persistent side-stream sums: enough for them to end just before P2P does.  Model:
+            // P2P at 700 Gpairs/s; the sums at 4 TB/s with >= 16 CTAs per SM, in proportion below that (measured on
+            // configs 4 and 5: the best values were 12 and 4).
+            const double t_p2p = (double)c->p2p_pairs / 700e9;
+            const double t_sum = (double)c->m2l_pairs * 8.0 * c->nst / 4e12;
+            int k = (int)std::ceil(16.0 * 1.3 * t_sum / std::max(t_p2p, 1e-9));
+            c->reduce_ctas_eff = c->reduce_ctas > 0 ? c->reduce_ctas : std::max(3, std::min(k, 16));
+        }
         int launches = 2 /*lift, p2m*/ + 3 /*l2p, p2p, spmv*/;
         for (int l = lmax - 1; l >= 2; --l) launches += 2;
-        for (int l = 2; l <= lmax; ++l) launches += l > 2 ? 3 : 2;     // M2L tiles, L2L tiles, reduce
+        for (int l = 2; l <= lmax; ++l) launches += l > 2 ? 4 : 2;     // M2L tiles + sum; L2L tiles + sum
         c->launches_per_apply = launches;
     }
 
@@ -409,6 +417,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
     else if (!strcmp(key, "lmax")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->force_lmax = v; c->ready = false; }
     else if (!strcmp(key, "timing")) { c->timing = v != 0; }
+    else if (!strcmp(key, "reduce_ctas")) { if (v < 0 || v > 32) return BEM_ERR_INVALID_ARG; c->reduce_ctas = v; c->ready = false; }
     else if (!strcmp(key, "m2l_rows16")) { c->m2l_rows16 = v != 0; }
     else if (!strcmp(key, "precond")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->precond = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }

@@ -107,6 +107,7 @@ struct Stage {
     int ntgt = 0;
     int out_base = 0;               // global index of the first target box
     bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
+    bool accumulate = false;        // the reduce pass adds to the output instead of overwriting it (L2L)
     dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
     dvec<int32_t> pos;              // [npairs] scratch row of pair k (target-major order)
     dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order): the reduce pass rotates back by its azimuth
@@ -134,6 +135,9 @@ struct bem_ctx {
     // options
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
     int precond = 0;                // bem_solve: 0 = unpreconditioned (the paper), 1 = right diagonal scaling by S_ii
+    int reduce_ctas = 0;            // option "reduce_ctas": CTAs per SM of the persistent side-stream sums, 0 = from the cost model
+    int reduce_ctas_eff = 6;
+    int n_sm = 148;
     int m2l_rows16 = 1;             // M2L tiles: 1 = 4 warps x 16 rows (B fragments feed two DMMAs), 0 = 8 warps x 8 rows
     int gemm_path = 0;              // translations: 0 = FP64 tensor path (DMMA) where p <= 16, 1 = plain-FMA tiles
 
@@ -172,7 +176,8 @@ struct bem_ctx {
     cudaStream_t side = nullptr;    // high-priority stream: reduce passes + L2P run here while P2P runs on `stream`
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     std::vector<bem::Stage> m2m;    // leaf-1 .. 2
-    std::vector<bem::Stage> m2l;    // 2 .. lmax (M2L + L2L of the level)
+    std::vector<bem::Stage> m2l;    // 2 .. lmax: L_own(l) = sum of the M2L rows of the level
+    std::vector<bem::Stage> l2l;    // 3 .. lmax: L(l) = L_own(l) + L2L L(l-1)
     int64_t m2l_pairs = 0, p2p_pairs = 0;
 
     // partial sums of the point engine, combined by the SpMV kernel

@@ -536,28 +536,32 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
 __global__ void __launch_bounds__(160)
 translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ pos, const int32_t *__restrict__ mat_t,
                  const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-                 int nre, double *__restrict__ out)
+                 int nre, int accumulate, int ntgt, double *__restrict__ out)
 {
-    const int t = blockIdx.x;
-    const int b = ptr[t], e = ptr[t + 1];
     const int nst = 2 * nre;
-    double *o = out + (size_t)t * nst;
-    for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
-        const int m = kinfo[cc];
-        double sr = 0.0, si = 0.0;
-        if (m == 0) {
-            for (int k = b; k < e; ++k) sr += scratch[(size_t)pos[k] * nst + cc];
-        } else {
-            for (int k = b; k < e; ++k) {
-                const double *row = scratch + (size_t)pos[k] * nst + cc;
-                double vr = row[0], vi = row[nre];
-                azimuth(__ldg(rot + (size_t)mat_t[k] * ROT_M + m), vr, vi);
-                sr += vr;
-                si += vi;
+    for (int t = blockIdx.x; t < ntgt; t += gridDim.x) {            // grid < ntgt: a persistent pass (see launch_stage_reduce)
+        const int b = ptr[t], e = ptr[t + 1];
+        double *o = out + (size_t)t * nst;
+        for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
+            const int m = kinfo[cc];
+            double sr = 0.0, si = 0.0;
+            if (m == 0) {
+#pragma unroll 4
+                for (int k = b; k < e; ++k) sr += scratch[(size_t)pos[k] * nst + cc];
+            } else {
+#pragma unroll 4
+                for (int k = b; k < e; ++k) {
+                    const double *row = scratch + (size_t)pos[k] * nst + cc;
+                    double vr = row[0], vi = row[nre];
+                    azimuth(__ldg(rot + (size_t)mat_t[k] * ROT_M + m), vr, vi);
+                    sr += vr;
+                    si += vi;
+                }
             }
+            if (accumulate) { sr += o[cc]; si += o[cc + nre]; }
+            o[cc] = sr;
+            o[cc + nre] = si;
         }
-        o[cc] = sr;
-        o[cc + nre] = si;
     }
 }
 
@@ -584,13 +588,18 @@ void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stre
     KERNEL_CHECK();
 }
 
-void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream)
+// ctas_per_sm > 0: a PERSISTENT pass of at most that many CTAs per SM looping over the targets.  The hardware does
+// not backfill an SM with blocks of a lower-priority grid while a higher-priority grid still has blocks waiting, and
+// serves equal priorities in arrival order; only a grid whose blocks are ALL resident at once leaves the rest of the
+// machine to the kernel of the other stream (measured: DESIGN.md section 6).
+void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int ctas_per_sm)
 {
     if (st.ntgt == 0) return;
     double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
-    translate_reduce<<<st.ntgt, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
+    const int grid = ctas_per_sm > 0 ? std::min(st.ntgt, c->n_sm * ctas_per_sm) : st.ntgt;
+    translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
         st.ptr.get(), st.pos.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
-        c->kinfo.get(), c->rot.get(), c->nre, out);
+        c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : 0, st.ntgt, out);
     KERNEL_CHECK();
 }
 
@@ -600,7 +609,7 @@ void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
     if (st.ntgt == 0) return;
     launch_stage_gemm(c, st, TILES_ALL, c->stream);
     if (st.ntiles > 0) mark(c, cls_gemm);
-    launch_stage_reduce(c, st, c->stream);
+    launch_stage_reduce(c, st, c->stream, 0);
     mark(c, cls_reduce);
 }
 

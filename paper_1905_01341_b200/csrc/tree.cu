@@ -145,7 +145,7 @@ __global__ void neighbour_lists(const uint64_t *tkey, int ntb, const uint64_t *s
 }
 
 // Interaction (V) list of target box t at `level`: source boxes that are children of the
-// parent's neighbours and not adjacent to t.  Plus, for level > 2, one L2L pair from the parent.
+// parent's neighbours and not adjacent to t.
 // count pass (src == nullptr) or fill pass.
 __global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
                                   const uint64_t *skey_parent, int nsb_parent, const int32_t *schild_parent,
@@ -176,11 +176,18 @@ __global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
                     ++cnt;
                 }
             }
-    if (level > 2) {
-        if (src) { src[w] = tbase_parent + tparent[t]; mat[w] = MAT_L2L + (int)(tkey[t] & 7ull); ++w; }
-        ++cnt;
-    }
     if (count) count[t] = cnt;
+}
+
+// L2L: one pair per target box: its parent's local expansion through the matrix of its octant
+__global__ void l2l_pairs(const uint64_t *tkey, const int32_t *tparent, int nt, int tbase_parent, int32_t *src, int32_t *mat, int32_t *ptr)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j > nt) return;
+    ptr[j] = j;
+    if (j == nt) return;
+    src[j] = tbase_parent + tparent[j];
+    mat[j] = MAT_L2L + (int)(tkey[j] & 7ull);
 }
 
 __global__ void m2m_pairs(const uint64_t *ckey, int nc, int cbase, int32_t *src, int32_t *mat)
@@ -271,7 +278,7 @@ void build_lists(bem_ctx *c)
     CUDA_TRY(cudaMemcpy(&hp, pc.get(), sizeof hp, cudaMemcpyDeviceToHost));
     c->p2p_pairs = (int64_t)hp;
 
-    // M2L (+ L2L) stages, levels 2..lmax
+    // M2L stages, levels 2..lmax
     c->m2l.clear();
     c->m2l.resize(lmax + 1);
     c->m2l_pairs = 0;
@@ -301,7 +308,7 @@ void build_lists(bem_ctx *c)
                                                         l > 2 ? tb.base[l - 1] : 0, nullptr, st.ptr.get(), src.get(), mat.get());
         KERNEL_CHECK();
         finish_stage(st, src, mat, s);
-        c->m2l_pairs += total - (l > 2 ? nt : 0);
+        c->m2l_pairs += total;
         st.scratch_off = max_pairs;                           // regions of the levels one after the other
         max_pairs += total;
     }
@@ -325,6 +332,27 @@ void build_lists(bem_ctx *c)
         finish_stage(st, src, mat, s);
         st.scratch_off = 0;                                   // M2M runs before any M2L tile: aliases the first region
         max_pairs = std::max<int64_t>(max_pairs, nc);
+    }
+    // L2L stages: children on level l = 3 .. lmax (run after every M2L row has been summed: alias the first region)
+    c->l2l.clear();
+    c->l2l.resize(lmax + 1);
+    for (int l = 3; l <= lmax; ++l) {
+        Stage &st = c->l2l[l];
+        const int nt = tb.nbox[l];
+        st.ntgt = nt;
+        st.out_base = tb.base[l];
+        st.out_is_local = true;
+        st.accumulate = true;
+        st.npairs = nt;
+        st.ptr.alloc(nt + 1);
+        dvec<int32_t> src, mat;
+        src.alloc(nt);
+        mat.alloc(nt);
+        l2l_pairs<<<cdiv(nt + 1, 256), 256, 0, s>>>(tb.bkey[l].get(), tb.parent[l].get(), nt, tb.base[l - 1], src.get(), mat.get(), st.ptr.get());
+        KERNEL_CHECK();
+        finish_stage(st, src, mat, s);
+        st.scratch_off = 0;
+        max_pairs = std::max<int64_t>(max_pairs, nt);
     }
     c->scratch.alloc((size_t)max_pairs * c->nst);
 }
