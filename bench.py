@@ -48,6 +48,19 @@ def workload_name(c):
     return c["name"]
 
 
+def cloud_config(n, seed=190501341 + 6):
+    """Config 6 (not in BASELINE.json): the paper's own Tables 1-2 workload -- n monopoles placed
+    randomly and uniformly in the unit cube, sources = receivers, intensities U(-1, 1), p = 12."""
+    from bem_inputs.configs import random_cube_points
+    pts, m = random_cube_points(n, seed)
+    return dict(V=pts, F=np.zeros((0, 3), np.int32), bubble_id=None, q=2.0 * m - 1.0, phi=None, p=12, leaf_size=256, eta=2.5,
+                cfg=6, cloud=True, name=f"cfg6: {n:,} uniform random monopoles in the unit cube (paper Tables 1-2)")
+
+
+def get_config(args):
+    return cloud_config(args.cloud_points) if args.config == 6 else make_config(args.config)
+
+
 def oracle_sample(c, seconds_target=15.0):
     """Time the oracle, as it stands, on a bounded sample of target rows; extrapolate to all rows
     (rows are independent: the paper extrapolates its CPU brute-force reference the same way)."""
@@ -55,19 +68,25 @@ def oracle_sample(c, seconds_target=15.0):
     V, F, q, phi = c["V"], c["F"], c["q"], c["phi"]
     N = V.shape[0]
     cores = oracle.num_threads()
+    if c.get("cloud"):
+        nsrc = N
+        run = lambda rows: oracle.monopole_sum(V, q, V[rows])
+    else:
+        nsrc = 3 * F.shape[0]
+        run = lambda rows: oracle.g3_apply(V, F, q, phi, eta=c["eta"], rows=rows)
     probe = sample_rows(c["cfg"], N, min(N, 4 * cores))
     t0 = time.perf_counter()
-    oracle.g3_apply(V, F, q, phi, eta=c["eta"], rows=probe)
+    run(probe)
     dt = max(time.perf_counter() - t0, 1e-4)
     nrows = int(min(N, max(len(probe), seconds_target / dt * len(probe))))
     rows = sample_rows(c["cfg"], N, nrows)
     t0 = time.perf_counter()
-    y = oracle.g3_apply(V, F, q, phi, eta=c["eta"], rows=rows)
+    y = run(rows)
     dt = time.perf_counter() - t0
     ms_full = dt * 1e3 * N / len(rows)
     return dict(value=ms_full, unit=UNIT, cores=cores, kind="oracle",
-                sample=f"{len(rows)} of {N} target rows x all {3 * F.shape[0]} sources in {dt:.2f} s, scaled by N/rows",
-                ns_per_pair=dt * 1e9 / (len(rows) * 3.0 * F.shape[0])), rows, y
+                sample=f"{len(rows)} of {N} target rows x all {nsrc} sources in {dt:.2f} s, scaled by N/rows",
+                ns_per_pair=dt * 1e9 / (len(rows) * float(nsrc))), rows, y
 
 
 def run_reference(args):
@@ -75,7 +94,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    c = make_config(args.config)
+    c = get_config(args)
     per_step = []
     info = None
     for i in range(args.warmup + args.steps):
@@ -152,14 +171,14 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    c = make_config(args.config)
+    c = get_config(args)
     V, F = c["V"], c["F"]
     N, T = V.shape[0], F.shape[0]
     p = args.p or c["p"]
     stream = torch.cuda.current_stream()
 
     t0 = time.perf_counter()
-    ctx = bem.bem_create(V, F, c["bubble_id"])
+    ctx = bem.bem_create_points(V, V) if c.get("cloud") else bem.bem_create(V, F, c["bubble_id"])
     ctx.bem_set_stream(stream.cuda_stream)
     ctx.bem_set_option("mode", 1 if args.direct else 0)
     if args.lmax:
@@ -169,9 +188,10 @@ def run_gpu(args):
     setup_wall_ms = (time.perf_counter() - t0) * 1e3
     stats = ctx.bem_get_stats()
 
-    qd = torch.tensor(c["q"], device="cuda"); pd = torch.tensor(c["phi"], device="cuda")
+    cloud = bool(c.get("cloud"))
+    qd = torch.tensor(c["q"], device="cuda"); pd = None if cloud else torch.tensor(c["phi"], device="cuda")
     yd = torch.empty_like(qd)
-    qh = torch.tensor(c["q"]).pin_memory(); ph = torch.tensor(c["phi"]).pin_memory()
+    qh = torch.tensor(c["q"]).pin_memory(); ph = None if cloud else torch.tensor(c["phi"]).pin_memory()
     yh = torch.empty(N, dtype=torch.float64).pin_memory()
 
     # L2 policy: the working set of one apply (sources, expansions, lists, CSR) is far above the 126 MB L2 for
@@ -288,7 +308,7 @@ def run_gpu(args):
     parity = float(np.linalg.norm(y[rows] - yo) / np.linalg.norm(yo))
 
     solve = None
-    if args.solve_iters > 0:
+    if args.solve_iters > 0 and not cloud:
         solve = {}
         for name, pre in (("unpreconditioned (paper)", 0), ("diagonal S_ii (option precond)", 1)):
             ctx.bem_set_option("precond", pre)
@@ -310,12 +330,14 @@ def run_gpu(args):
                             parallelism="replicas only" if world > 1 else "1 gpu",
                             l2="flushed between iterations (512 MB write)" if flush else "working set larger than L2",
                             device_bytes=int(stats["device_bytes"])),
-                e2e=dict(value=e2e, unit=UNIT, h2d_bytes_per_step=16 * N, d2h_bytes_per_step=8 * N),
+                e2e=dict(value=e2e, unit=UNIT, h2d_bytes_per_step=(8 if cloud else 16) * N, d2h_bytes_per_step=8 * N),
                 gpu_launches=int(stats["kernel_launches_per_apply"]) * args.steps,
                 clocks=clocks, roofline=roof, cpu_baseline=cpu, parity_rel_l2_vs_oracle=parity,
                 breakdown_ms=breakdown, kernels=kernels, setup_ms=stats["setup_ms"], setup_wall_ms=setup_wall_ms,
                 m2l_pairs=int(stats["m2l_pairs"]), solve=solve,
-                paper_context="paper Table 3 (PAPER.md:606): 1 MVP = 4.0 s at N=2,629,632, p=12, double, Xeon 5660 x12 cores + Tesla K20")
+                paper_context=("paper Table 2 (PAPER.md:479-490): at N=1,048,576, p=12 the FMM+GPU (double) product is 2309x faster than the CPU "
+                               "brute force and the brute-force GPU (double) 33x, Xeon 5660 + Tesla K20" if cloud else
+                               "paper Table 3 (PAPER.md:606): 1 MVP = 4.0 s at N=2,629,632, p=12, double, Xeon 5660 x12 cores + Tesla K20"))
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -327,7 +349,8 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: 2.57M nodes)")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: 2.57M nodes); 6 = point cloud (paper Tables 1-2)")
+    ap.add_argument("--cloud-points", type=int, default=1048576, help="config 6: number of points")
     ap.add_argument("--p", type=int, default=0)
     ap.add_argument("--leaf-size", type=int, default=0)
     ap.add_argument("--lmax", type=int, default=0)

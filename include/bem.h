@@ -94,6 +94,16 @@ bem_status bem_create(const double *vertices, int64_t n_vertices,
                       const int32_t *triangles, int64_t n_triangles,
                       const int32_t *bubble_id, bem_ctx **out);
 
+/* bem_create_points -- the same engine on a POINT CLOUD: the workload of the paper's Tables 1-2 (PAPER.md:456-490:
+ * "N sources and N receivers distributed randomly and uniformly inside a cube", monopoles).
+ *   sources  [n_sources x 3] fp64 source positions, targets [n_targets x 3] evaluation points (may be the same array).
+ * bem_apply(ctx, q, NULL, y) then computes  y_i = sum_j q_j G(x_i, y_j) = sum_j q_j / (4 pi |x_i - y_j|)  over all
+ * sources with x_i != y_j:  q is [n_sources], y is [n_targets]; phi must be NULL.  There is no mesh, no correction
+ * matrix and no bem_solve in this mode; options "mode", "lmax", "timing", "gemm_path" and bem_setup(p, leaf_size, -)
+ * work as for a mesh (near_radius is ignored).  Arrays are copied; host or device pointers. */
+bem_status bem_create_points(const double *sources, int64_t n_sources, const double *targets, int64_t n_targets,
+                             bem_ctx **out);
+
 /* bem_set_option -- must be called before bem_setup to take effect.
  *   "quadrature"    0 = G3 (default), 1 = V1 (paper's Eq. 17 + Eqs. 19-21)
  *   "mode"          0 = FMM (default), 1 = direct all-pairs sum (the paper's

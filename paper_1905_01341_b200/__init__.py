@@ -29,7 +29,7 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
               "kernel_launches_per_apply"]
 
 # every symbol include/bem.h declares
-EXPORTS = ["bem_create", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
+EXPORTS = ["bem_create", "bem_create_points", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
            "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy"]
 
 
@@ -53,6 +53,7 @@ def load_library() -> ctypes.CDLL:
     lib = ctypes.CDLL(LIB_PATH)
     vp, i64, i32, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
     lib.bem_create.argtypes = [vp, i64, vp, i64, vp, ctypes.POINTER(vp)]
+    lib.bem_create_points.argtypes = [vp, i64, vp, i64, ctypes.POINTER(vp)]
     lib.bem_set_option.argtypes = [vp, ctypes.c_char_p, dbl]
     lib.bem_set_stream.argtypes = [vp, vp]
     lib.bem_setup.argtypes = [vp, i32, i32, dbl]
@@ -93,9 +94,20 @@ def _ptr(a):
 class Bem:
     """One mesh + its setup: the object the C calls operate on (an owned `bem_ctx *`)."""
 
-    def __init__(self, vertices, triangles, bubble_id=None):
+    def __init__(self, vertices, triangles, bubble_id=None, _points=None):
         self._lib = load_library()
         self._ctx = ctypes.c_void_p(0)
+        if _points is not None:                      # bem_create_points(sources, targets)
+            S = np.ascontiguousarray(_points[0], dtype=np.float64)
+            T = np.ascontiguousarray(_points[1], dtype=np.float64)
+            if S.ndim != 2 or S.shape[1] != 3 or T.ndim != 2 or T.shape[1] != 3:
+                raise ValueError("sources and targets must be [n,3]")
+            self.n_vertices, self.n_triangles, self.n_sources = T.shape[0], 0, S.shape[0]
+            st = self._lib.bem_create_points(S.ctypes.data, S.shape[0], T.ctypes.data, T.shape[0], ctypes.byref(self._ctx))
+            if st != BEM_OK:
+                self._ctx = ctypes.c_void_p(0)
+                raise BemError(st, "bem_create_points failed (a CUDA device is required)")
+            return
         V = np.ascontiguousarray(vertices, dtype=np.float64)
         F = np.ascontiguousarray(triangles, dtype=np.int32)
         if V.ndim != 2 or V.shape[1] != 3 or F.ndim != 2 or F.shape[1] != 3:
@@ -176,3 +188,8 @@ class Bem:
 
 def bem_create(vertices, triangles, bubble_id=None) -> Bem:
     return Bem(vertices, triangles, bubble_id)
+
+
+def bem_create_points(sources, targets) -> Bem:
+    """Point-cloud mode (include/bem.h): bem_apply(q[n_sources], None, y[n_targets])."""
+    return Bem(None, None, None, _points=(sources, targets))

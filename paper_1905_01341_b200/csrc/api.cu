@@ -182,9 +182,9 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     c->nst = lay_nst(c->pl);
     c->leaf_size = leaf_size;
     c->eta = eta;
-    compute_geometry(c);
+    if (c->quadrature != 2) compute_geometry(c);
     const int64_t N = c->N;
-    c->ns = c->quadrature == 0 ? 3 * c->T : N;
+    c->ns = c->quadrature == 0 ? 3 * c->T : (c->quadrature == 2 ? c->np : N);
 
     {
         // unit-cube scaling (reading R11): cube centred on the bounding box, side = largest extent (1 + 1e-9)
@@ -193,6 +193,12 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         bbox3(c->V.get(), N, bb.get(), s);
         double hb[6];
         CUDA_TRY(cudaMemcpy(hb, bb.get(), sizeof hb, cudaMemcpyDeviceToHost));
+        if (c->quadrature == 2) {                           // the cube holds sources and targets
+            double hs[6];
+            bbox3(c->P.get(), c->np, bb.get(), s);
+            CUDA_TRY(cudaMemcpy(hs, bb.get(), sizeof hs, cudaMemcpyDeviceToHost));
+            for (int d = 0; d < 3; ++d) { hb[d] = std::min(hb[d], hs[d]); hb[3 + d] = std::max(hb[3 + d], hs[3 + d]); }
+        }
         double side = 0;
         for (int d = 0; d < 3; ++d) side = std::max(side, hb[3 + d] - hb[d]);
         side *= (1.0 + 1e-9);
@@ -263,6 +269,11 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     if (c->quadrature == 0) build_correction(c);
     else build_empty_correction(c);
     c->ready = true;
+    if (c->quadrature == 2) {                               // point cloud: no free term, no solve
+        CUDA_TRY(cudaStreamSynchronize(s));
+        c->setup_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+        return;
+    }
 
     dvec<double> ones, y0;
     ones.alloc(N);
@@ -407,11 +418,37 @@ bem_status bem_create(const double *vertices, int64_t n_vertices, const int32_t 
     return BEM_OK;
 }
 
+bem_status bem_create_points(const double *sources, int64_t n_sources, const double *targets, int64_t n_targets, bem_ctx **out)
+{
+    if (!out) return BEM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!sources || !targets || n_sources < 1 || n_targets < 1 || n_sources > 2000000000ll || n_targets > 2000000000ll)
+        return BEM_ERR_INVALID_ARG;
+    bem_ctx *c = new (std::nothrow) bem_ctx();
+    if (!c) return BEM_ERR_OOM;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { delete c; cudaGetLastError(); return BEM_ERR_CUDA; }
+    cudaGetDevice(&c->device);
+    c->N = n_targets;
+    c->T = 0;
+    c->np = n_sources;
+    c->quadrature = 2;
+    bem_status st = guarded(c, [&]() {
+        c->V.alloc(3 * c->N);
+        c->P.alloc(3 * c->np);
+        CUDA_TRY(cudaMemcpy(c->V.get(), targets, 3 * c->N * sizeof(double), cudaMemcpyDefault));
+        CUDA_TRY(cudaMemcpy(c->P.get(), sources, 3 * c->np * sizeof(double), cudaMemcpyDefault));
+    });
+    if (st != BEM_OK) { delete c; return st; }
+    *out = c;
+    return BEM_OK;
+}
+
 bem_status bem_set_option(bem_ctx *c, const char *key, double value)
 {
     if (!c || !key) return BEM_ERR_INVALID_ARG;
     const int v = (int)value;
-    if (!strcmp(key, "quadrature")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->quadrature = v; c->ready = false; }
+    if (!strcmp(key, "quadrature")) { if ((v != 0 && v != 1) || c->quadrature == 2) return BEM_ERR_INVALID_ARG; c->quadrature = v; c->ready = false; }
     else if (!strcmp(key, "mode")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->mode = v; c->ready = false; }
     else if (!strcmp(key, "free_term")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->free_term = v; c->ready = false; }
     else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
@@ -447,12 +484,14 @@ bem_status bem_apply(bem_ctx *c, const double *q, const double *phi, double *y)
     if (!c || !y) return BEM_ERR_INVALID_ARG;
     if (!c->ready) { c->err = "bem_apply before bem_setup"; return BEM_ERR_NOT_SETUP; }
     if (y == q || y == phi) { c->err = "bem_apply: y aliases an input"; return BEM_ERR_INVALID_ARG; }
+    if (c->quadrature == 2 && phi) { c->err = "bem_apply: a point cloud carries monopoles only (phi must be NULL)"; return BEM_ERR_INVALID_ARG; }
     return guarded(c, [&]() {
         const size_t bytes = c->N * sizeof(double);
+        const size_t qbytes = (c->quadrature == 2 ? c->np : c->N) * sizeof(double);
         const bool hq = !is_device_ptr(q), hp = !is_device_ptr(phi), hy = !is_device_ptr(y);
         const double *dq = q, *dp = phi;
         double *dy = y;
-        if (hq) { if (!c->stage_q.p) c->stage_q.alloc(c->N); CUDA_TRY(cudaMemcpyAsync(c->stage_q.get(), q, bytes, cudaMemcpyHostToDevice, c->stream)); dq = c->stage_q.get(); }
+        if (hq) { if (!c->stage_q.p) c->stage_q.alloc(qbytes / sizeof(double)); CUDA_TRY(cudaMemcpyAsync(c->stage_q.get(), q, qbytes, cudaMemcpyHostToDevice, c->stream)); dq = c->stage_q.get(); }
         if (hp) { if (!c->stage_phi.p) c->stage_phi.alloc(c->N); CUDA_TRY(cudaMemcpyAsync(c->stage_phi.get(), phi, bytes, cudaMemcpyHostToDevice, c->stream)); dp = c->stage_phi.get(); }
         if (hy) { if (!c->stage_y.p) c->stage_y.alloc(c->N); dy = c->stage_y.get(); }
         apply_device(c, dq, dp, dy);

@@ -131,6 +131,8 @@ struct bem_ctx {
     bem::dvec<double> V;            // [N*3]
     bem::dvec<int32_t> F;           // [T*3]
     bem::dvec<int32_t> bid;         // [N]
+    bem::dvec<double> P;            // point-cloud mode (quadrature == 2): [np*3] source points; V holds the targets
+    int64_t np = 0;
 
     // options
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;

@@ -195,11 +195,22 @@ __global__ void build_sources_v1(const double *V, const double *A, const double 
     lv[e] = make_int4((int)j, (int)j, (int)j, 0);
 }
 
+// point cloud: unit weight, no normal; strength j is the j-th entry of q
+__global__ void build_sources_points(const double *P, const uint32_t *order, int64_t n, double4 *pos, double4 *lw, int4 *lv)
+{
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int64_t j = order ? order[e] : e;
+    pos[e] = make_double4(P[3 * j], P[3 * j + 1], P[3 * j + 2], 0.0);
+    lw[e] = make_double4(1.0, 0.0, 0.0, 0.0);
+    lv[e] = make_int4((int)j, (int)j, (int)j, 0);
+}
+
 // Build src_pos / lift_w / lift_vid in engine order (order == nullptr: natural order).
 void build_sources(bem_ctx *c, const uint32_t *order)
 {
     cudaStream_t s = c->stream;
-    c->ns = c->quadrature == 0 ? 3 * c->T : c->N;
+    c->ns = c->quadrature == 0 ? 3 * c->T : (c->quadrature == 2 ? c->np : c->N);
     c->src_pos.alloc(c->ns);
     c->lift_w.alloc(c->ns);
     c->lift_vid.alloc(c->ns);
@@ -207,6 +218,9 @@ void build_sources(bem_ctx *c, const uint32_t *order)
     if (c->quadrature == 0) {
         build_sources_g3<<<cdiv(c->ns, 256), 256, 0, s>>>(c->V.get(), c->F.get(), c->triA.get(), c->triN.get(), order,
                                                           c->ns, c->src_pos.get(), c->lift_w.get(), c->lift_vid.get());
+        KERNEL_CHECK();
+    } else if (c->quadrature == 2) {
+        build_sources_points<<<cdiv(c->ns, 256), 256, 0, s>>>(c->P.get(), order, c->ns, c->src_pos.get(), c->lift_w.get(), c->lift_vid.get());
         KERNEL_CHECK();
     } else {
         const int64_t nc = 3 * c->T;
@@ -243,6 +257,9 @@ void source_points(bem_ctx *c, dvec<double> &xyz)
         xyz.alloc(9 * c->T);
         source_points_g3<<<cdiv(3 * c->T, 256), 256, 0, c->stream>>>(c->V.get(), c->F.get(), c->T, xyz.get());
         KERNEL_CHECK();
+    } else if (c->quadrature == 2) {
+        xyz.alloc(3 * c->np);
+        CUDA_TRY(cudaMemcpyAsync(xyz.get(), c->P.get(), 3 * c->np * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
     } else {
         xyz.alloc(3 * c->N);
         CUDA_TRY(cudaMemcpyAsync(xyz.get(), c->V.get(), 3 * c->N * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));

@@ -265,6 +265,7 @@ extern "C" bem_status bem_solve(bem_ctx *c, const double *phi, double *q, int us
                                 int *iters_out, double *relres_out)
 {
     if (!c || !phi || !q || !(tol > 0.0) || max_iter < 0) return BEM_ERR_INVALID_ARG;
+    if (c->quadrature == 2) { c->err = "bem_solve: not available for a point cloud"; return BEM_ERR_INVALID_ARG; }
     if (!c->ready || !c->have_cfree) { c->err = "bem_solve before bem_setup"; return BEM_ERR_NOT_SETUP; }
     try {
         cudaSetDevice(c->device);
