@@ -126,7 +126,16 @@ bem_status bem_create_points(const double *sources, int64_t n_sources, const dou
  *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply
  *   "gemm_path"     batched translations (M2M, M2L, L2L): 0 = FP64 tensor-core tiles (DMMA; p <= 16,
  *                   default -- measured faster), 1 = plain FP64 FMA tiles (any p).
- *                   May be changed between products. */
+ *                   May be changed between products.
+ *   "p2p_precision" near field A^(sparse) X in FMM mode: 0 = fp64 pairs (default; the measured mode, the only one
+ *                   that meets the 1e-8 tolerance at high p); 1 = the paper's "single precision on GPU" option
+ *                   (Table 1): every pair 1/r, d.(x-y)/r^3 in fp32 on positions taken relative to
+ *                   the leaf centres (in leaf edges), at most 8 pairs per target summed in fp32, all further sums
+ *                   in fp64 in a fixed order.  The far field, the correction matrix and the direct-sum mode stay
+ *                   fp64.  Error floor ~1e-7 (monopoles) .. 1e-6 (dipoles on surfaces) relative L2: at the
+ *                   configs' p (<= 12) the product's error is unchanged.  May be changed between products.
+ *   "p2p_ctas"      fp32 near field: CTAs per SM of its persistent grid while the row sums share the SMs
+ *                   (1..16; 0 = 4, default).  Tuning only. */
 bem_status bem_set_option(bem_ctx *ctx, const char *key, double value);
 
 /* bem_set_stream -- cuda_stream is a cudaStream_t (NULL = default stream).  All

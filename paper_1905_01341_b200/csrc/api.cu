@@ -31,6 +31,9 @@ void launch_lift(bem_ctx *c, const double *q, const double *phi);
 void launch_p2p_direct(bem_ctx *c);
 void launch_p2p_leaves(bem_ctx *c);
 void launch_spmv_combine(bem_ctx *c, const double *q, const double *phi, double *y);
+// p2p_f32.cu
+void launch_p2p_leaves_f32(bem_ctx *c, cudaStream_t stream, int ctas_per_sm, int leaf0, int leaf1, int part);
+void ensure_p2p_f32(bem_ctx *c);
 
 bool is_device_ptr(const void *p)
 {
@@ -128,6 +131,7 @@ void mark(bem_ctx *c, int cls)
 void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
 {
     c->ev_n = 0;
+    if (c->mode == 0 && c->p2p_precision == 1) ensure_p2p_f32(c);
     mark(c, -1);
     launch_lift(c, q, phi);
     mark(c, BEM_T_LIFT);
@@ -145,7 +149,8 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
             for (int l = 3; l <= lmax; ++l) launch_stage(c, c->l2l[l], BEM_T_L2L_REDUCE, BEM_T_L2L_REDUCE);
             launch_l2p(c, c->tb.leaf_of.get());
             mark(c, BEM_T_L2P);
-            launch_p2p_leaves(c);
+            if (c->p2p_precision == 1) launch_p2p_leaves_f32(c, c->stream, 8, 0, c->tb.nbox[lmax], 0);
+            else launch_p2p_leaves(c);
             mark(c, BEM_T_P2P);
         } else {
             // The M2L tiles of every level only read multipole expansions: issue them all, then fork.  The per-level
@@ -158,7 +163,9 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
             CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
             for (int l = lmax; l >= 2; --l) launch_stage_reduce(c, c->m2l[l], c->side, c->reduce_ctas_eff);
             CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
-            launch_p2p_leaves(c);
+            // fp32 pairs: a persistent grid of a few CTAs per SM (80 registers each) so that the CTAs of the sums still fit
+            if (c->p2p_precision == 1) launch_p2p_leaves_f32(c, main, c->p2p_ctas > 0 ? c->p2p_ctas : 4, 0, c->tb.nbox[lmax], 0);
+            else launch_p2p_leaves(c);
             CUDA_TRY(cudaStreamWaitEvent(main, c->ev_join, 0));
             for (int l = 3; l <= lmax; ++l) launch_stage(c, c->l2l[l], BEM_T_L2L_REDUCE, BEM_T_L2L_REDUCE);
             launch_l2p(c, c->tb.leaf_of.get());
@@ -251,6 +258,9 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
             CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
             CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
         }
+        c->p2p_counter.alloc(2);
+        c->src_pos_f.free();
+        c->src_str_f.free();
         {
             // CTAs per SM of the persistent side-stream sums: enough for them to end just before P2P does.  Model:
             // P2P at 700 Gpairs/s; the sums at 4 TB/s with >= 16 CTAs per SM, in proportion below that (measured on
@@ -457,6 +467,8 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "reduce_ctas")) { if (v < 0 || v > 32) return BEM_ERR_INVALID_ARG; c->reduce_ctas = v; c->ready = false; }
     else if (!strcmp(key, "m2l_rows16")) { c->m2l_rows16 = v != 0; }
     else if (!strcmp(key, "precond")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->precond = v; }
+    else if (!strcmp(key, "p2p_precision")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->p2p_precision = v; }
+    else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
     return BEM_OK;

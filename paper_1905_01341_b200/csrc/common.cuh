@@ -142,6 +142,8 @@ struct bem_ctx {
     int n_sm = 148;
     int m2l_rows16 = 1;             // M2L tiles: 1 = 4 warps x 16 rows (B fragments feed two DMMAs), 0 = 8 warps x 8 rows
     int gemm_path = 0;              // translations: 0 = FP64 tensor path (DMMA) where p <= 16, 1 = plain-FMA tiles
+    int p2p_precision = 0;          // near field: 0 = fp64 pairs (default), 1 = fp32 pair arithmetic, fp64 accumulation (p2p_f32.cu)
+    int p2p_ctas = 0;               // fp32 near field: CTAs per SM of its persistent grid beside the row sums, 0 = default (4)
 
     // setup state
     bool ready = false;
@@ -177,6 +179,9 @@ struct bem_ctx {
                                     // levels can be issued before the first reduce pass
     cudaStream_t side = nullptr;    // high-priority stream: reduce passes + L2P run here while P2P runs on `stream`
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    bem::dvec<int> p2p_counter;     // leaf counter of the persistent fp32 near-field grid
+    bem::dvec<float4> src_pos_f;    // [ns] fp32 near field: position relative to the own leaf centre, in leaf edges (built at first use)
+    bem::dvec<float4> src_str_f;    // [ns] fp32 near field: (m/h, d/h^2), rewritten by every apply
     std::vector<bem::Stage> m2m;    // leaf-1 .. 2
     std::vector<bem::Stage> m2l;    // 2 .. lmax: L_own(l) = sum of the M2L rows of the level
     std::vector<bem::Stage> l2l;    // 3 .. lmax: L(l) = L_own(l) + L2L L(l-1)

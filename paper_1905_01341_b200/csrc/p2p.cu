@@ -16,7 +16,7 @@ constexpr double INV_4PI = 0.079577471545947667884441881686257;
 // (P1 interpolation at the Gauss point; in V1 v0 = v1 = v2 = j, w = s_j, N = n_j: Eq. 17)
 __global__ void lift_kernel(const double *__restrict__ q, const double *__restrict__ phi,
                             const double4 *__restrict__ lw, const int4 *__restrict__ lv, int64_t ns,
-                            double4 *__restrict__ str)
+                            double4 *__restrict__ str, float4 *__restrict__ strf, double ih)
 {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= ns) return;
@@ -27,12 +27,17 @@ __global__ void lift_kernel(const double *__restrict__ q, const double *__restri
     if (q) qq = a * q[v.x] + b * q[v.y] + b * q[v.z];
     if (phi) ff = a * phi[v.x] + b * phi[v.y] + b * phi[v.z];
     str[s] = make_double4(w.x * qq, w.y * ff, w.z * ff, w.w * ff);
+    // fp32 near field (p2p_f32.cu): strengths in leaf-edge units, m/h and d/h^2, rounded once
+    if (strf) strf[s] = make_float4((float)(w.x * qq * ih), (float)(w.y * ff * ih * ih), (float)(w.z * ff * ih * ih), (float)(w.w * ff * ih * ih));
 }
 
 void launch_lift(bem_ctx *c, const double *q, const double *phi)
 {
     c->has_dipole = phi != nullptr;                 // the pair and P2M kernels skip the dipole terms otherwise
-    lift_kernel<<<cdiv(c->ns, 256), 256, 0, c->stream>>>(q, phi, c->lift_w.get(), c->lift_vid.get(), c->ns, c->src_str.get());
+    const bool f32 = c->mode == 0 && c->p2p_precision == 1;
+    const double ih = f32 ? (double)(1u << c->sb.lmax) / c->cube_side : 0.0;
+    lift_kernel<<<cdiv(c->ns, 256), 256, 0, c->stream>>>(q, phi, c->lift_w.get(), c->lift_vid.get(), c->ns, c->src_str.get(),
+                                                         f32 ? c->src_str_f.get() : nullptr, ih);
     KERNEL_CHECK();
 }
 

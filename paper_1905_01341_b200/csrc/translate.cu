@@ -546,10 +546,10 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ po
             const int m = kinfo[cc];
             double sr = 0.0, si = 0.0;
             if (m == 0) {
-#pragma unroll 4
+#pragma unroll 8
                 for (int k = b; k < e; ++k) sr += scratch[(size_t)pos[k] * nst + cc];
             } else {
-#pragma unroll 4
+#pragma unroll 8
                 for (int k = b; k < e; ++k) {
                     const double *row = scratch + (size_t)pos[k] * nst + cc;
                     double vr = row[0], vi = row[nre];
