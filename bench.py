@@ -266,13 +266,20 @@ def run_gpu(args):
     # P2P: 17 FP64 instructions per pair (9 DFMA + 5 DMUL + 3 DADD = 26 flop; SASS count).
     P2P_INSTR, P2P_FLOP = 17.0, 26.0
     slot_peak = FP64_NOMINAL_GFLOPS / 2e3                      # T instr/s
+    f32 = args.p2p_precision == 32 and not args.direct
+    if f32:
+        # fp32 pairs (p2p_f32.cu): 12 FP32-pipe instructions (6 FFMA + 3 FMUL + 3 FADD = 18 flop) + 1 MUFU.RSQ per pair;
+        # FP32 pipes: 148 SMs x 128 lanes x 1.965 GHz = 37.2 T instr/s
+        P2P_INSTR, P2P_FLOP = 12.0, 18.0
+        slot_peak = 2.0 * FP64_NOMINAL_GFLOPS / 2e3
     nre = stats["exp_stride"] / 2.0
     kernels = {}
     p2p_s = tm["p2p"] * 1e-3
     kernels["p2p"] = dict(ms=tm["p2p"], pairs=stats["p2p_pairs"], gpairs_per_s=stats["p2p_pairs"] / p2p_s / 1e9 if p2p_s > 0 else None,
                           tflops=stats["p2p_pairs"] * P2P_FLOP / p2p_s / 1e12 if p2p_s > 0 else None,
                           fp64_slot_frac=stats["p2p_pairs"] * P2P_INSTR / p2p_s / 1e12 / slot_peak if p2p_s > 0 else None,
-                          note="17 FP64 instr / 26 flop per pair; slot_frac = share of the FP64 pipe's issue slots (nominal 18.6 T instr/s)")
+                          note=("12 FP32 instr (18 flop) + 1 MUFU.RSQ per pair; fp64_slot_frac here = share of the FP32 pipes' issue slots (nominal 37.2 T instr/s)"
+                                if f32 else "17 FP64 instr / 26 flop per pair; slot_frac = share of the FP64 pipe's issue slots (nominal 18.6 T instr/s)"))
     if not args.direct:
         m2l_s = tm["m2l"] * 1e-3
         exec_flop = stats["m2l_pairs"] * 4.0 * nre * nre          # two nre x nre blocks, 2 flop per MAC (azimuth split)
@@ -293,7 +300,14 @@ def run_gpu(args):
     common = dict(peak_source="derived: 148 SMs x 64 FP64 lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry); "
                               "measured in this run: DFMA loop %.1f, DMMA loop %.1f TFLOP/s" % (dfma / 1e3, dmma / 1e3),
                   measured_dfma_tflops=dfma / 1e3, measured_dmma_tflops=dmma / 1e3)
-    if args.direct or tm["p2p"] >= tm["m2l"]:
+    if f32 and tm["p2p"] >= tm["m2l"]:
+        k = kernels["p2p"]
+        peak32 = 2.0 * FP64_NOMINAL_GFLOPS / 1e3
+        roof = dict(kernel="p2p_leaf_kernel_f32", bound="alu", achieved=k["tflops"], peak=peak32, unit="TFLOP/s", frac=k["tflops"] / peak32,
+                    fp32_slot_frac=k["fp64_slot_frac"], traffic=None, algorithmic="18 flop (12 FP32 instructions) + 1 MUFU per pair x %d pairs" % stats["p2p_pairs"],
+                    ms=tm["p2p"], share_of_step=tm["p2p"] / tm["total"],
+                    peak_source="derived: 148 SMs x 128 FP32 lanes/clk x 2 flop x 1.965 GHz")
+    elif args.direct or tm["p2p"] >= tm["m2l"]:
         k = kernels["p2p"]
         roof = dict(kernel="p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", bound="alu", achieved=k["tflops"],
                     peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", frac=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
@@ -313,6 +327,25 @@ def run_gpu(args):
     y = yd.cpu().numpy()
     parity = float(np.linalg.norm(y[rows] - yo) / np.linalg.norm(yo))
 
+    # the paper's "single precision on GPU" option for A^(sparse) X, measured beside the fp64 default
+    mixed = None
+    if not args.direct and not f32:
+        ctx.bem_set_option("p2p_precision", 1)
+        for _ in range(3):
+            ctx.bem_apply(qd, pd, yd)
+        torch.cuda.synchronize()
+        mixed_ms = timed(lambda: ctx.bem_apply(qd, pd, yd), args.steps) / args.steps
+        ym = yd.cpu().numpy()
+        ctx.bem_set_option("timing", 1)
+        ctx.bem_apply(qd, pd, yd)
+        tmix = ctx.bem_get_timings()
+        ctx.bem_set_option("timing", 0)
+        ctx.bem_set_option("p2p_precision", 0)
+        mixed = dict(option="p2p_precision = 1: near-field pairs in fp32 (leaf-relative positions), sums in fp64; far field and correction fp64",
+                     value=mixed_ms, unit=UNIT, p2p_ms=tmix["p2p"], p2p_gpairs_per_s=stats["p2p_pairs"] / (tmix["p2p"] * 1e-3) / 1e9,
+                     parity_rel_l2_vs_oracle=float(np.linalg.norm(ym[rows] - yo) / np.linalg.norm(yo)),
+                     rel_l2_vs_fp64_path=float(np.linalg.norm(ym - y) / np.linalg.norm(y)))
+
     solve = None
     if args.solve_iters > 0 and not cloud:
         solve = {}
@@ -329,8 +362,9 @@ def run_gpu(args):
         ctx.bem_set_option("precond", 0)
 
     line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
-                higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=workload_name(c), mode="direct" if args.direct else "fmm", p=p, n_nodes=N, n_triangles=T,
+                higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64 (near-field pairs f32)" if f32 else "f64", data="synthetic",
+                config=dict(workload=workload_name(c), mode="direct" if args.direct else "fmm", p=p,
+                            p2p_precision="fp32 pairs, fp64 sums" if f32 else "fp64", n_nodes=N, n_triangles=T,
                             n_sources=int(stats["n_sources"]), leaf_size=args.leaf_size or c["leaf_size"], eta=c["eta"],
                             lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]), n_tgt_leaves=int(stats["n_tgt_leaves"]),
                             parallelism="replicas only" if world > 1 else "1 gpu",
@@ -340,7 +374,7 @@ def run_gpu(args):
                 gpu_launches=int(stats["kernel_launches_per_apply"]) * args.steps,
                 clocks=clocks, roofline=roof, cpu_baseline=cpu, parity_rel_l2_vs_oracle=parity,
                 breakdown_ms=breakdown, kernels=kernels, setup_ms=stats["setup_ms"], setup_wall_ms=setup_wall_ms,
-                m2l_pairs=int(stats["m2l_pairs"]), solve=solve,
+                m2l_pairs=int(stats["m2l_pairs"]), solve=solve, mixed_precision_option=mixed,
                 paper_context=("paper Table 2 (PAPER.md:479-490): at N=1,048,576, p=12 the FMM+GPU (double) product is 2309x faster than the CPU "
                                "brute force and the brute-force GPU (double) 33x, Xeon 5660 + Tesla K20" if cloud else
                                "paper Table 3 (PAPER.md:606): 1 MVP = 4.0 s at N=2,629,632, p=12, double, Xeon 5660 x12 cores + Tesla K20"))
