@@ -185,6 +185,8 @@ def run_gpu(args):
         ctx.bem_set_option("lmax", args.lmax)
     if args.p2p_precision == 32:
         ctx.bem_set_option("p2p_precision", 1)
+    if args.direct_pairs is not None:
+        ctx.bem_set_option("direct_pairs", args.direct_pairs)
     if args.p2p_ctas:
         ctx.bem_set_option("p2p_ctas", args.p2p_ctas)
     if args.reduce_ctas:
@@ -397,6 +399,8 @@ def main():
     ap.add_argument("--direct", action="store_true", help="direct-sum mode (configs 1-3)")
     ap.add_argument("--p2p-precision", type=int, default=64, choices=[64, 32],
                     help="near-field pair arithmetic: 64 = fp64 (default, the measured mode), 32 = fp32 pairs with fp64 accumulation (PAPER.md:456-473)")
+    ap.add_argument("--direct-pairs", type=int, default=None,
+                    help="leaf-level far pairs with nt x ns <= this are summed directly instead of translated (default: library cost model; 0: off)")
     ap.add_argument("--p2p-ctas", type=int, default=0, help="fp32 near field: CTAs per SM of its persistent grid (0: library default)")
     ap.add_argument("--reduce-ctas", type=int, default=0, help="CTAs per SM of the persistent row-sum passes (0: library cost model)")
     ap.add_argument("--solve-iters", type=int, default=30, help="also run bem_solve with this max_iter (0: skip)")

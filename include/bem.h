@@ -134,6 +134,12 @@ bem_status bem_create_points(const double *sources, int64_t n_sources, const dou
  *                   in fp64 in a fixed order.  The far field, the correction matrix and the direct-sum mode stay
  *                   fp64.  Error floor ~1e-7 (monopoles) .. 1e-6 (dipoles on surfaces) relative L2: at the
  *                   configs' p (<= 12) the product's error is unchanged.  May be changed between products.
+ *   "direct_pairs"  leaf-level far-field (M2L) pairs whose boxes hold nt targets and ns sources with nt x ns <= this
+ *                   value are summed directly in the near-field kernel instead of being translated: a translation
+ *                   costs 4 nre^2 flop whatever the boxes hold, and on surface meshes a third of the leaf-level pairs
+ *                   join sparsely filled boxes (the balance of A^(dense) and A^(sparse), per pair).
+ *                   -1 = 800 (nre / 80)^2 from the measured costs (default), 0 = off (the uniform lists of
+ *                   PAPER.md:440).  Direct pairs are exact, so the error can only fall.
  *   "p2p_ctas"      fp32 near field: CTAs per SM of its persistent grid while the row sums share the SMs
  *                   (1..16; 0 = 4, default).  Tuning only. */
 bem_status bem_set_option(bem_ctx *ctx, const char *key, double value);

@@ -247,6 +247,14 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         build_matrices(c);
         c->Mexp.alloc((size_t)c->sb.total() * c->nst);
         c->Lexp.alloc((size_t)c->tb.total() * c->nst);
+        {
+            // leaf-level far pairs that cost less summed directly than translated (option "direct_pairs").  One M2L pair +
+            // its row sum costs ~1.35 us at p = 12 (nre = 80) whatever the boxes hold, one point pair ~1.4 ns in a full
+            // leaf and several times that in the sparsely filled leaves these pairs come from; measured optimum on configs
+            // 4 and 5: nt x ns <= 800 (nre / 80)^2 (flat between half and 1.5x that)
+            const double w = 800.0 * (double)c->nre * (double)c->nre / 6400.0;
+            c->direct_max_eff = c->direct_max >= 0 ? c->direct_max : (int64_t)w;
+        }
         build_lists(c);
         c->nsplit = 2;                                  // far field (L2P) and near field (P2P) partial sums
         c->ypart.alloc(2 * N);
@@ -468,6 +476,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "m2l_rows16")) { c->m2l_rows16 = v != 0; }
     else if (!strcmp(key, "precond")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->precond = v; }
     else if (!strcmp(key, "p2p_precision")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->p2p_precision = v; }
+    else if (!strcmp(key, "direct_pairs")) { if (value < -1 || value > 1e9) return BEM_ERR_INVALID_ARG; c->direct_max = (int64_t)value; c->ready = false; }
     else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }

@@ -54,6 +54,12 @@ struct dvec {
     T *get() const { return p; }
 };
 
+// Preferred shared-memory carve-out (percent of the SM's L1/shared array) of the kernels that bem_apply runs side by side
+// on one SM (the near-field pair kernels and the row sums of the M2L stages).  An SM can only hold CTAs whose kernels
+// agree on the carve-out: with the driver's per-kernel default, a few KB more static shared memory in one of them was
+// enough to serialise the two (measured: config 5, fp32 pairs beside the sums, 21.3 -> 26.5 ms).
+constexpr int CORUN_CARVEOUT = 14;     // 32 KB of 228
+
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 }  // namespace bem
 struct bem_ctx;
@@ -171,6 +177,11 @@ struct bem_ctx {
     // octree + lists (FMM mode)
     bem::BoxSet sb, tb;
     bem::dvec<int32_t> nbr;         // [n_tgt_leaves * 27] source leaves adjacent to a target leaf, -1 padded
+    bem::dvec<int32_t> xdir_ptr;    // [n_tgt_leaves + 1] CSR of the leaf-level far pairs that are summed directly (option direct_pairs)
+    bem::dvec<int32_t> xdir_src;    // [xdir_pairs] their source leaves
+    int64_t xdir_pairs = 0;
+    int64_t direct_max = -1;        // option "direct_pairs": nt x ns threshold, -1 = from the cost model, 0 = off
+    int64_t direct_max_eff = 0;
     bem::dvec<double> mats;         // [N_MATS * nst * nst] real translation matrices, row = input dof k, col = output dof
     bem::dvec<double2> rot;         // [N_MATS * ROT_M] (cos m a, sin m a): azimuth a of the M2L offset, identity for M2M / L2L
     bem::dvec<int32_t> kinfo;       // [nst] order m of every stored dof (0 for padding)

@@ -6,6 +6,7 @@
 // This is the paper's A^(sparse) X, the part it runs on the GPU,
 // and, over all pairs, its brute-force product.
 #include "common.cuh"
+#include "segments.cuh"
 
 namespace bem {
 
@@ -150,39 +151,26 @@ __device__ __forceinline__ void lds_point(unsigned addr, double &x, double &y, d
 template <bool DIP>
 __global__ void __launch_bounds__(P2P_THREADS, 5)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
+                const int32_t *__restrict__ xptr, const int32_t *__restrict__ xsrc,
                 const int32_t *__restrict__ sbegin, const double4 *__restrict__ spos, const double4 *__restrict__ sstr,
                 double *__restrict__ y)
 {
     __shared__ double4 tg[P2P_NT];
     __shared__ double red[P2P_WARPS][P2P_NT];
-    __shared__ int seg_s0[32], seg_pre[33];
+    __shared__ int seg_s0[SEG_MAX], seg_pre[SEG_MAX + 1], seg_n;
     const int leaf = blockIdx.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int t0 = tbegin[leaf], nt = tbegin[leaf + 1] - t0;
-    if (warp == 0) {
-        const int b = lane < 27 ? nbr[(int64_t)leaf * 27 + lane] : -1;
-        int s0 = 0, cnt = 0;
-        if (b >= 0) { s0 = sbegin[b]; cnt = sbegin[b + 1] - s0; }
-        int inc = cnt;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-        seg_s0[lane] = s0;
-        seg_pre[lane + 1] = inc;
-        if (lane == 0) seg_pre[0] = 0;
-    }
+    if (warp == 0) build_segments(lane, leaf, nbr, xptr, xsrc, sbegin, seg_s0, seg_pre, &seg_n, [](int, int) {});
     __syncthreads();
-    const int S = seg_pre[32];
+    const int S = seg_pre[SEG_MAX], nseg = seg_n;
     const int rounds = (S + P2P_THREADS - 1) / P2P_THREADS;
     const unsigned tg_base = (unsigned)__cvta_generic_to_shared(tg);
 
     // source g of the concatenated list; beyond the end a far-away point of zero strength (adds exactly 0)
     auto load_source = [&](int g, double4 &p, double4 &q) {
         if (g < S) {
-            int k = seg_pre[16] <= g ? 16 : 0;                         // last k with seg_pre[k] <= g
-            if (seg_pre[k + 8] <= g) k += 8;
-            if (seg_pre[k + 4] <= g) k += 4;
-            if (seg_pre[k + 2] <= g) k += 2;
-            if (seg_pre[k + 1] <= g) k += 1;
+            const int k = find_segment(seg_pre, nseg, g);
             const int idx = seg_s0[k] + (g - seg_pre[k]);
             p = spos[idx];
             q = sstr[idx];
@@ -278,11 +266,17 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
 void launch_p2p_leaves(bem_ctx *c)
 {
     const int nleaf = c->tb.nbox[c->tb.lmax];
+    static bool attr_set = false;
+    if (!attr_set) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        attr_set = true;
+    }
     if (c->has_dipole)
-        p2p_leaf_kernel<true><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
+        p2p_leaf_kernel<true><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, c->sb.begin.get(),
                                                                     c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N);
     else
-        p2p_leaf_kernel<false><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->sb.begin.get(),
+        p2p_leaf_kernel<false><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, c->sb.begin.get(),
                                                                      c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N);
     KERNEL_CHECK();
 }

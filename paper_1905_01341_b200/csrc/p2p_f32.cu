@@ -22,6 +22,7 @@
 // beside the whole far-field pass.
 #include "common.cuh"
 #include "morton.cuh"
+#include "segments.cuh"
 #include <algorithm>
 
 namespace bem {
@@ -116,15 +117,16 @@ __device__ __forceinline__ void round_f32(float (&facc)[F_NT], unsigned tg_base,
 template <bool DIP, bool SELF>
 __global__ void __launch_bounds__(F_THREADS, F_MINB)
 p2p_leaf_kernel_f32(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const uint64_t *__restrict__ tkey,
-                    const int32_t *__restrict__ nbr, const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey,
+                    const int32_t *__restrict__ nbr, const int32_t *__restrict__ xptr, const int32_t *__restrict__ xsrc,
+                    const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey,
                     const float4 *__restrict__ spos, const float4 *__restrict__ sstr,
                     double cx0, double cy0, double cz0, double h, int leaf0, int nleaf, int *__restrict__ counter,
                     double *__restrict__ y)
 {
     __shared__ float4 tg[F_NT];
     __shared__ double red[F_WARPS][F_NT];
-    __shared__ float4 seg_off[32];
-    __shared__ int seg_s0[32], seg_pre[33];
+    __shared__ int seg_off[SEG_MAX];                                   // (ox + 4) | (oy + 4) << 4 | (oz + 4) << 8
+    __shared__ int seg_s0[SEG_MAX], seg_pre[SEG_MAX + 1], seg_n;
     __shared__ int cur_leaf;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const double inv_h = 1.0 / h;
@@ -140,32 +142,24 @@ p2p_leaf_kernel_f32(const double *__restrict__ tgt, const int32_t *__restrict__ 
         uint32_t ix, iy, iz;
         morton_decode(tkey[leaf], &ix, &iy, &iz);
         const double cx = cx0 + (ix + 0.5) * h, cy = cy0 + (iy + 0.5) * h, cz = cz0 + (iz + 0.5) * h;
-        if (warp == 0) {
-            const int b = lane < 27 ? nbr[(int64_t)leaf * 27 + lane] : -1;
-            int s0 = 0, cnt = 0;
-            float4 off = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-            if (b >= 0) {
-                s0 = sbegin[b]; cnt = sbegin[b + 1] - s0;
-                uint32_t jx, jy, jz;
-                morton_decode(skey[b], &jx, &jy, &jz);
-                off = make_float4((float)((int)jx - (int)ix), (float)((int)jy - (int)iy), (float)((int)jz - (int)iz), 0.0f);
-            }
-            int inc = cnt;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
-            seg_s0[lane] = s0;
-            seg_off[lane] = off;
-            seg_pre[lane + 1] = inc;
-            if (lane == 0) seg_pre[0] = 0;
-        }
+        if (warp == 0)
+            build_segments(lane, leaf, nbr, xptr, xsrc, sbegin, seg_s0, seg_pre, &seg_n, [&](int k, int b) {
+                int off = 0x444;                                       // source leaf - target leaf, in leaf edges (|.| <= 3)
+                if (b >= 0) {
+                    uint32_t jx, jy, jz;
+                    morton_decode(skey[b], &jx, &jy, &jz);
+                    off = ((int)jx - (int)ix + 4) | ((int)jy - (int)iy + 4) << 4 | ((int)jz - (int)iz + 4) << 8;
+                }
+                seg_off[k] = off;
+            });
         __syncthreads();
-        const int S = seg_pre[32];
+        const int S = seg_pre[SEG_MAX];
         const int rounds = (S + F_THREADS * F_SPL - 1) / (F_THREADS * F_SPL);
 
         // source g of the concatenated neighbour list, moved into the frame of the target leaf
         // (g only grows from one round to the next: the segment index k of a lane's source moves forward)
         // (the offset of the segment is returned, not added: an add here would wait for the load it prefetches)
-        auto load_source = [&](int g, int &k, float4 &p, float4 &q, float4 &o) {
+        auto load_source = [&](int g, int &k, float4 &p, float4 &q, int &o) {
             if (g < S) {
                 while (seg_pre[k + 1] <= g) ++k;                       // last k with seg_pre[k] <= g
                 const int idx = seg_s0[k] + (g - seg_pre[k]);
@@ -173,7 +167,7 @@ p2p_leaf_kernel_f32(const double *__restrict__ tgt, const int32_t *__restrict__ 
                 p = spos[idx];
                 q = sstr[idx];
             } else {                                                   // far away, zero strength: adds exactly 0
-                o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                o = 0x444;
                 p = make_float4(1e5f, 0.0f, 0.0f, 0.0f);
                 q = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
             }
@@ -196,7 +190,8 @@ p2p_leaf_kernel_f32(const double *__restrict__ tgt, const int32_t *__restrict__ 
 #pragma unroll
             for (int t = 0; t < F_NT; ++t) facc[t] = 0.0f;
             double dsum = 0.0;                                         // lane L: running fp64 sum of target L over the warp's lanes
-            float4 sp[F_SPL], ss[F_SPL], pn[F_SPL], qn[F_SPL], on[F_SPL];
+            float4 sp[F_SPL], ss[F_SPL], pn[F_SPL], qn[F_SPL];
+            int on[F_SPL];
             int seg[F_SPL];
 #pragma unroll
             for (int j = 0; j < F_SPL; ++j) { seg[j] = 0; load_source(j * F_THREADS + threadIdx.x, seg[j], pn[j], qn[j], on[j]); }
@@ -204,7 +199,7 @@ p2p_leaf_kernel_f32(const double *__restrict__ tgt, const int32_t *__restrict__ 
             for (int r = 0; r < rounds; ++r) {
 #pragma unroll
                 for (int j = 0; j < F_SPL; ++j) {
-                    sp[j] = make_float4(pn[j].x + on[j].x, pn[j].y + on[j].y, pn[j].z + on[j].z, 0.0f);
+                    sp[j] = make_float4(pn[j].x + (float)((on[j] & 15) - 4), pn[j].y + (float)((on[j] >> 4 & 15) - 4), pn[j].z + (float)((on[j] >> 8) - 4), 0.0f);
                     ss[j] = qn[j];
                 }
                 if (r + 1 < rounds) {                                  // prefetch the next round
@@ -277,7 +272,16 @@ void launch_p2p_leaves_f32(bem_ctx *c, cudaStream_t stream, int ctas_per_sm, int
     const int grid = std::max(1, std::min(leaf1 - leaf0, ctas_per_sm * c->n_sm));
     CUDA_TRY(cudaMemsetAsync(c->p2p_counter.get() + part, 0, sizeof(int), stream));
     const bool self = c->quadrature != 0;
-#define BEM_F32_ARGS c->tgt_pos.get(), c->tb.begin.get(), c->tb.bkey[lmax].get(), c->nbr.get(), c->sb.begin.get(), \
+    static bool attr_set = false;
+    if (!attr_set) {
+        // same shared-memory carve-out as the row sums it runs beside (common.cuh): an SM only holds CTAs of one carve-out
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        attr_set = true;
+    }
+#define BEM_F32_ARGS c->tgt_pos.get(), c->tb.begin.get(), c->tb.bkey[lmax].get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, c->sb.begin.get(), \
                      c->sb.bkey[lmax].get(), c->src_pos_f.get(), c->src_str_f.get(), c->cube_min[0], c->cube_min[1], \
                      c->cube_min[2], h, leaf0, nleaf, c->p2p_counter.get() + part, c->ypart.get() + c->N
     if (c->has_dipole) {

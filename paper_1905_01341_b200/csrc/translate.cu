@@ -597,6 +597,11 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
     if (st.ntgt == 0) return;
     double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
     const int grid = ctas_per_sm > 0 ? std::min(st.ntgt, c->n_sm * ctas_per_sm) : st.ntgt;
+    static bool attr_set = false;
+    if (!attr_set) {                                                   // same carve-out as the pair kernels it runs beside (common.cuh)
+        CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        attr_set = true;
+    }
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
         st.ptr.get(), st.pos.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
         c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : 0, st.ntgt, out);

@@ -150,7 +150,9 @@ __global__ void neighbour_lists(const uint64_t *tkey, int ntb, const uint64_t *s
 __global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
                                   const uint64_t *skey_parent, int nsb_parent, const int32_t *schild_parent,
                                   const uint64_t *skey, const int32_t *tparent, int sbase, int tbase_parent,
-                                  int32_t *count, const int32_t *ptr, int32_t *src, int32_t *mat)
+                                  int32_t *count, const int32_t *ptr, int32_t *src, int32_t *mat,
+                                  const int32_t *tbegin, const int32_t *sbegin, int64_t direct_max,
+                                  int32_t *xcount, const int32_t *xptr, int32_t *xsrc, unsigned long long *xpairs)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= ntb) return;
@@ -160,6 +162,11 @@ __global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
     const int lim = 1 << (level - 1);
     int cnt = 0;
     int w = ptr ? ptr[t] : 0;
+    // leaf level, direct_max > 0: a pair whose boxes hold nt x ns <= direct_max point pairs costs less summed directly
+    // than translated (one M2L = 4 nre^2 flop whatever the boxes hold): it goes to the near field (list xsrc) instead
+    const int64_t ntp = direct_max > 0 ? tbegin[t + 1] - tbegin[t] : 0;
+    int xc = 0, xw = xptr ? xptr[t] : 0;
+    unsigned long long xp = 0;
     for (int dz = -1; dz <= 1; ++dz)
         for (int dy = -1; dy <= 1; ++dy)
             for (int dx = -1; dx <= 1; ++dx) {
@@ -172,11 +179,21 @@ __global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
                     morton_decode(skey[c], &cx, &cy, &cz);
                     const int ox = (int)ix - (int)cx, oy = (int)iy - (int)cy, oz = (int)iz - (int)cz;   // target - source
                     if (max(max(abs(ox), abs(oy)), abs(oz)) < 2) continue;                           // adjacent: near field
+                    if (direct_max > 0) {
+                        const int64_t nsp = sbegin[c + 1] - sbegin[c];
+                        if (ntp * nsp <= direct_max) {
+                            if (xsrc) xsrc[xw++] = c;
+                            ++xc;
+                            xp += (unsigned long long)(ntp * nsp);
+                            continue;
+                        }
+                    }
                     if (src) { src[w] = sbase + c; mat[w] = MAT_M2L + (ox + 3) + 7 * (oy + 3) + 49 * (oz + 3); ++w; }
                     ++cnt;
                 }
             }
     if (count) count[t] = cnt;
+    if (xcount) { xcount[t] = xc; if (xp) atomicAdd(xpairs, xp); }
 }
 
 // L2L: one pair per target box: its parent's local expansion through the matrix of its octant
@@ -277,6 +294,9 @@ void build_lists(bem_ctx *c)
     unsigned long long hp = 0;
     CUDA_TRY(cudaMemcpy(&hp, pc.get(), sizeof hp, cudaMemcpyDeviceToHost));
     c->p2p_pairs = (int64_t)hp;
+    c->xdir_pairs = 0;
+    c->xdir_ptr.free();
+    c->xdir_src.free();
 
     // M2L stages, levels 2..lmax
     c->m2l.clear();
@@ -289,13 +309,26 @@ void build_lists(bem_ctx *c)
         st.ntgt = nt;
         st.out_base = tb.base[l];
         st.out_is_local = true;
-        dvec<int32_t> cnt;
+        dvec<int32_t> cnt, xcnt;
         cnt.alloc(nt);
         st.ptr.alloc(nt + 1);
+        const int64_t dmax = l == lmax ? c->direct_max_eff : 0;
+        if (dmax > 0) { xcnt.alloc(nt); c->xdir_ptr.alloc(nt + 1); pc.zero(s); }
         interaction_lists<<<cdiv(nt, 128), 128, 0, s>>>(tb.bkey[l].get(), nt, l, sb.bkey[l - 1].get(), sb.nbox[l - 1], sb.child[l - 1].get(),
                                                         sb.bkey[l].get(), l > 2 ? tb.parent[l].get() : nullptr, sb.base[l],
-                                                        l > 2 ? tb.base[l - 1] : 0, cnt.get(), nullptr, nullptr, nullptr);
+                                                        l > 2 ? tb.base[l - 1] : 0, cnt.get(), nullptr, nullptr, nullptr,
+                                                        tb.begin.get(), sb.begin.get(), dmax, dmax > 0 ? xcnt.get() : nullptr, nullptr, nullptr, pc.get());
         KERNEL_CHECK();
+        if (dmax > 0) {
+            scan_exclusive_i32(xcnt.get(), c->xdir_ptr.get(), nt, s);
+            int xt = 0;
+            CUDA_TRY(cudaMemcpy(&xt, c->xdir_ptr.get() + nt, sizeof(int), cudaMemcpyDeviceToHost));
+            unsigned long long xp = 0;
+            CUDA_TRY(cudaMemcpy(&xp, pc.get(), sizeof xp, cudaMemcpyDeviceToHost));
+            c->xdir_pairs = xt;
+            c->p2p_pairs += (int64_t)xp;
+            c->xdir_src.alloc(xt);
+        }
         scan_exclusive_i32(cnt.get(), st.ptr.get(), nt, s);
         int total = 0;
         CUDA_TRY(cudaMemcpy(&total, st.ptr.get() + nt, sizeof(int), cudaMemcpyDeviceToHost));
@@ -305,7 +338,9 @@ void build_lists(bem_ctx *c)
         mat.alloc(total);
         interaction_lists<<<cdiv(nt, 128), 128, 0, s>>>(tb.bkey[l].get(), nt, l, sb.bkey[l - 1].get(), sb.nbox[l - 1], sb.child[l - 1].get(),
                                                         sb.bkey[l].get(), l > 2 ? tb.parent[l].get() : nullptr, sb.base[l],
-                                                        l > 2 ? tb.base[l - 1] : 0, nullptr, st.ptr.get(), src.get(), mat.get());
+                                                        l > 2 ? tb.base[l - 1] : 0, nullptr, st.ptr.get(), src.get(), mat.get(),
+                                                        tb.begin.get(), sb.begin.get(), dmax, nullptr, dmax > 0 ? c->xdir_ptr.get() : nullptr,
+                                                        dmax > 0 ? c->xdir_src.get() : nullptr, pc.get());
         KERNEL_CHECK();
         finish_stage(st, src, mat, s);
         c->m2l_pairs += total;

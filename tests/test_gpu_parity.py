@@ -234,8 +234,8 @@ def test_fmm_every_truncation_number_cfg1():
     yo = oracle_rows(c, rows, 0, "q", None)
     errs = {}
     for p in (1, 2, 3, 4, 5, 7, 9, 11, 13, 15, 16, 17, 19):
-        ctx = _ctx(c, p=p, lmax=3)
-        errs[p] = _rel(_apply(ctx, c["q"], None), yo)
+        ctx = _ctx(c, p=p, lmax=3, direct_pairs=0)             # uniform lists: the truncation error alone (the direct-pair
+        errs[p] = _rel(_apply(ctx, c["q"], None), yo)           # threshold moves with the layout size of p)
         ctx.bem_destroy()
     print({p: f"{e:.2e}" for p, e in errs.items()})
     ps = sorted(errs)
@@ -383,3 +383,28 @@ def test_mixed_precision_point_cloud_reproduces_table1_single_column():
         assert TABLE1_SINGLE[p] / 4.0 <= errs[p] <= 4.0 * hi, (p, errs[p])
     for p in (16, 20):
         assert TABLE1[p] < errs[p] <= 4.0 * TABLE1_SINGLE[p], (p, errs[p])
+
+
+# ------------------------------------------------------------------ sparse far pairs summed directly (option direct_pairs)
+@pytest.mark.parametrize("n,nb,prec", [(2, None, 0), (5, 150, 0), (5, 150, 1), (4, 60, 0)])
+def test_direct_pairs_thresholds(n, nb, prec):
+    """Leaf-level M2L pairs with nt x ns <= threshold move to the near-field kernel (tree.cu): threshold 0 = the uniform
+    lists of PAPER.md:440, -1 = cost model, 1e9 = every leaf-level far pair direct (up to 27 + 189 source segments per
+    target leaf).  All three meet the FMM tolerance; the pair counts move as stated; the all-direct product is the most
+    accurate (direct pairs are exact)."""
+    c = cfg(n) if nb is None else cfg(n, n_bubbles=nb)
+    N = c["V"].shape[0]
+    rows = sample_rows(n, N, 1500)
+    yo = oracle_rows(c, rows)
+    res = {}
+    for d in (0, -1, 10 ** 9):
+        ctx = _ctx(c, direct_pairs=d, p2p_precision=prec)
+        y = _apply(ctx, c["q"], c["phi"])
+        st = ctx.bem_get_stats()
+        ctx.bem_destroy()
+        res[d] = (_rel(y[rows], yo), st["m2l_pairs"], st["p2p_pairs"])
+        print(f"cfg{n} direct_pairs {d} prec {prec}: S-D {res[d][0]:.2e}, m2l pairs {res[d][1]:.0f}, point pairs {res[d][2]:.3e}")
+    for d in res:
+        assert res[d][0] <= TOL_FULL[c["p"]]
+    assert res[0][1] > res[-1][1] > res[10 ** 9][1] and res[0][2] < res[-1][2] < res[10 ** 9][2]
+    assert res[10 ** 9][0] <= res[0][0] * 1.05
