@@ -163,14 +163,15 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
     const int t0 = tbegin[leaf], nt = tbegin[leaf + 1] - t0;
     if (warp == 0) build_segments(lane, leaf, nbr, xptr, xsrc, sbegin, seg_s0, seg_pre, &seg_n, [](int, int) {});
     __syncthreads();
-    const int S = seg_pre[SEG_MAX], nseg = seg_n;
+    const int S = seg_pre[SEG_MAX];
     const int rounds = (S + P2P_THREADS - 1) / P2P_THREADS;
     const unsigned tg_base = (unsigned)__cvta_generic_to_shared(tg);
 
     // source g of the concatenated list; beyond the end a far-away point of zero strength (adds exactly 0)
-    auto load_source = [&](int g, double4 &p, double4 &q) {
+    // (g only grows from one round to the next: the segment index k of the lane's source moves forward)
+    auto load_source = [&](int g, int &k, double4 &p, double4 &q) {
         if (g < S) {
-            const int k = find_segment(seg_pre, nseg, g);
+            while (seg_pre[k + 1] <= g) ++k;                           // last k with seg_pre[k] <= g
             const int idx = seg_s0[k] + (g - seg_pre[k]);
             p = spos[idx];
             q = sstr[idx];
@@ -193,11 +194,12 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
 #pragma unroll
         for (int t = 0; t < P2P_NT; ++t) acc[t] = 0.0;
         double4 p, q, pn, qn;
-        load_source(threadIdx.x, pn, qn);
+        int seg = 0;
+        load_source(threadIdx.x, seg, pn, qn);
 #pragma unroll 1
         for (int r = 0; r < rounds; ++r) {
             p = pn; q = qn;
-            if (r + 1 < rounds) load_source((r + 1) * P2P_THREADS + threadIdx.x, pn, qn);   // prefetch the next round
+            if (r + 1 < rounds) load_source((r + 1) * P2P_THREADS + threadIdx.x, seg, pn, qn);   // prefetch the next round
 #pragma unroll
             for (int tb = 0; tb < P2P_NT; tb += 8) {                    // 8 independent chains at a time
                 if (tb + 8 <= ntc) {                                    // warp-uniform
