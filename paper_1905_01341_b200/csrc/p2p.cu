@@ -47,11 +47,13 @@ void launch_lift(bem_ctx *c, const double *q, const double *phi)
 // followed by ONE third-order step  y1 = y0 (1 + e/2 + 3 e^2/8),  e = 1 - x y0^2, whose residual is
 // 5 e^3/16 ~ 2.5 d^3 < 1e-19 -- 5 FP64 instructions instead of the two Newton steps and the
 // slow-path branch of the library rsqrt (P2P).
+// SELF = false: the caller guarantees x > 0 (G3: a Gauss point never coincides with a vertex) and the test is left out
+template <bool SELF>
 __device__ __forceinline__ double rsqrt_pos(double x)
 {
     double y0;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
-    y0 = __double2hiint(x) > 0 ? y0 : 0.0;        // x >= 0 here; x == 0 (and subnormal x) -> 0, an integer test off the FP64 pipe
+    if (SELF) y0 = __double2hiint(x) > 0 ? y0 : 0.0;   // x >= 0 here; x == 0 (and subnormal x) -> 0, an integer test off the FP64 pipe
     const double e = fma(-x, y0 * y0, 1.0);
     const double pe = fma(0.375, e, 0.5) * e;
     return fma(y0, pe, y0);
@@ -60,12 +62,12 @@ __device__ __forceinline__ double rsqrt_pos(double x)
 // one (target, source) interaction; r2 == 0 (V1: source j = target i; "i != j") adds nothing
 // acc += that interaction (the last multiply and the accumulation are one FMA)
 // DIP = false: monopole sources only (phi == NULL, every product of a GMRES iteration): 12 FP64 instructions instead of 17
-template <bool DIP>
+template <bool DIP, bool SELF>
 __device__ __forceinline__ double pair_acc(double acc, double tx, double ty, double tz, const double4 &sp, const double4 &ss)
 {
     const double dx = tx - sp.x, dy = ty - sp.y, dz = tz - sp.z;
     const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    const double inv = rsqrt_pos(r2);
+    const double inv = rsqrt_pos<SELF>(r2);
     if (!DIP) return fma(inv, ss.x, acc);
     const double dd = fma(ss.y, dx, fma(ss.z, dy, ss.w * dz));
     // m/r - (d.dx)/r^3 = inv * (m - dd * inv^2)
@@ -80,7 +82,7 @@ constexpr int P2P_TPT = 4;            // direct mode: targets per thread
 // grid = (target blocks, source splits); thread = FOUR targets, so one shared-memory source read
 // (4 x LDS.128, a broadcast) feeds four pairs -- measured with ncu, one target per thread is bound by
 // the shared-memory pipe (88% LSU wavefronts at 48% FP64), not by FP64; sources staged in tiles of 256
-template <bool DIP>
+template <bool DIP, bool SELF>
 __global__ void __launch_bounds__(P2P_THREADS)
 p2p_direct_kernel(const double *__restrict__ tgt, int64_t nt, const double4 *__restrict__ spos,
                   const double4 *__restrict__ sstr, int64_t ns, int64_t chunk, double *__restrict__ ypart)
@@ -105,7 +107,7 @@ p2p_direct_kernel(const double *__restrict__ tgt, int64_t nt, const double4 *__r
         for (int j = 0; j < n; ++j) {
             const double4 p = sp[j], q = ss[j];
 #pragma unroll
-            for (int k = 0; k < P2P_TPT; ++k) acc[k] = pair_acc<DIP>(acc[k], tx[k], ty[k], tz[k], p, q);
+            for (int k = 0; k < P2P_TPT; ++k) acc[k] = pair_acc<DIP, SELF>(acc[k], tx[k], ty[k], tz[k], p, q);
         }
     }
 #pragma unroll
@@ -119,12 +121,12 @@ void launch_p2p_direct(bem_ctx *c)
 {
     const int64_t chunk = (c->ns + c->nsplit - 1) / c->nsplit;
     dim3 grid(cdiv(c->N, P2P_TPT * P2P_THREADS), c->nsplit);
-    if (c->has_dipole)
-        p2p_direct_kernel<true><<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
-                                                                     c->ns, chunk, c->ypart.get());
-    else
-        p2p_direct_kernel<false><<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), c->src_str.get(),
-                                                                      c->ns, chunk, c->ypart.get());
+    const bool self = c->quadrature != 0;                       // V1 (j = i) and point clouds may have r = 0; G3 cannot
+#define BEM_DIRECT(D, S) p2p_direct_kernel<D, S><<<grid, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->src_pos.get(), \
+                                                                                      c->src_str.get(), c->ns, chunk, c->ypart.get())
+    if (c->has_dipole) { if (self) BEM_DIRECT(true, true); else BEM_DIRECT(true, false); }
+    else { if (self) BEM_DIRECT(false, true); else BEM_DIRECT(false, false); }
+#undef BEM_DIRECT
     KERNEL_CHECK();
 }
 
@@ -148,7 +150,7 @@ __device__ __forceinline__ void lds_point(unsigned addr, double &x, double &y, d
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%3];\n\tld.shared.f64 %2, [%3+16];" : "=d"(x), "=d"(y), "=d"(z) : "r"(addr));
 }
 
-template <bool DIP>
+template <bool DIP, bool SELF>
 __global__ void __launch_bounds__(P2P_THREADS, 5)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
                 const int32_t *__restrict__ xptr, const int32_t *__restrict__ xsrc,
@@ -207,7 +209,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                     for (int t = tb; t < tb + 8; ++t) {
                         double Tx, Ty, Tz;
                         lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                        acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
+                        acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
                     }
                 } else if (tb < ntc) {                                  // the last 1..7 targets: 4 + singles
                     if (tb + 4 <= ntc) {
@@ -215,14 +217,14 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                         for (int t = tb; t < tb + 4; ++t) {
                             double Tx, Ty, Tz;
                             lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                            acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
+                            acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
                         }
 #pragma unroll
                         for (int t = tb + 4; t < tb + 7; ++t) {
                             if (t < ntc) {
                                 double Tx, Ty, Tz;
                                 lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                                acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
+                                acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
                             }
                         }
                     } else {
@@ -231,7 +233,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                             if (t < ntc) {
                                 double Tx, Ty, Tz;
                                 lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                                acc[t] = pair_acc<DIP>(acc[t], Tx, Ty, Tz, p, q);
+                                acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
                             }
                         }
                     }
@@ -270,16 +272,18 @@ void launch_p2p_leaves(bem_ctx *c)
     const int nleaf = c->tb.nbox[c->tb.lmax];
     static bool attr_set = false;
     if (!attr_set) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
-        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         attr_set = true;
     }
-    if (c->has_dipole)
-        p2p_leaf_kernel<true><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, c->sb.begin.get(),
-                                                                    c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N);
-    else
-        p2p_leaf_kernel<false><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, c->sb.begin.get(),
-                                                                     c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N);
+    const bool self = c->quadrature != 0;                       // V1 (j = i) and point clouds may have r = 0; G3 cannot
+#define BEM_LEAF(D, S) p2p_leaf_kernel<D, S><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, \
+                           c->xdir_src.p, c->sb.begin.get(), c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N)
+    if (c->has_dipole) { if (self) BEM_LEAF(true, true); else BEM_LEAF(true, false); }
+    else { if (self) BEM_LEAF(false, true); else BEM_LEAF(false, false); }
+#undef BEM_LEAF
     KERNEL_CHECK();
 }
 
