@@ -266,7 +266,7 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
             CUDA_TRY(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
             CUDA_TRY(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
         }
-        c->p2p_counter.alloc(2);
+        c->p2p_counter.alloc(4);                         // [0], [1] fp32 pair kernel, [2] P2M: leaf counters of the persistent grids
         c->src_pos_f.free();
         c->src_str_f.free();
         {

@@ -190,7 +190,7 @@ struct bem_ctx {
                                     // levels can be issued before the first reduce pass
     cudaStream_t side = nullptr;    // high-priority stream: reduce passes + L2P run here while P2P runs on `stream`
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    bem::dvec<int> p2p_counter;     // leaf counter of the persistent fp32 near-field grid
+    bem::dvec<int> p2p_counter;     // leaf counters of the persistent grids (fp32 pair kernel, P2M)
     bem::dvec<float4> src_pos_f;    // [ns] fp32 near field: position relative to the own leaf centre, in leaf edges (built at first use)
     bem::dvec<float4> src_str_f;    // [ns] fp32 near field: (m/h, d/h^2), rewritten by every apply
     std::vector<bem::Stage> m2m;    // leaf-1 .. 2

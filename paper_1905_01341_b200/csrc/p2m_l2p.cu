@@ -10,6 +10,7 @@
 #include "common.cuh"
 #include "harmonics.cuh"
 #include "morton.cuh"
+#include <algorithm>
 
 namespace bem {
 
@@ -55,20 +56,29 @@ __device__ __forceinline__ void next_row(int l, double ax, double ay, double az,
 // One warp per source leaf, lane = source (32 at a time).  Each lane's p^2 values go through a
 // [64][33] shared-memory table, group of rows by group; lane k then sums value k over the 32
 // sources in a fixed order (no atomics) into a register accumulator.
+#ifndef P2M_MINB
+#define P2M_MINB 3
+#endif
 constexpr int P2M_WARPS = 4;
 constexpr int P2M_TBL = 64 * 33;
 
 template <int P, bool DIP>
-__global__ void __launch_bounds__(P2M_WARPS * 32)
+__global__ void __launch_bounds__(P2M_WARPS * 32, P2M_MINB)
 p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf,
              double cmx, double cmy, double cmz, double h,
-             const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nst, double *__restrict__ Mout)
+             const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nst, double *__restrict__ Mout,
+             int *__restrict__ counter)
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int leaf = blockIdx.x * P2M_WARPS + warp;
-    if (leaf >= nleaf) return;
     double *tbl = sm + (size_t)warp * P2M_TBL;
+    // persistent warps: leaf sizes differ by an order of magnitude on polydisperse clusters, and with one leaf per warp of a
+    // 4-warp CTA the SM ran at 7 of its 12 warps on average (ncu); every warp now takes the next leaf from a counter
+    for (;;) {
+    int leaf = 0;
+    if (lane == 0) leaf = atomicAdd(counter, 1);
+    leaf = __shfl_sync(0xffffffffu, leaf, 0);
+    if (leaf >= nleaf) return;
     uint32_t ix, iy, iz;
     morton_decode(skey[leaf], &ix, &iy, &iz);
     const double cx = cmx + (ix + 0.5) * h, cy = cmy + (iy + 0.5) * h, cz = cmz + (iz + 0.5) * h;
@@ -158,6 +168,8 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
             }
         }
     }
+    __syncwarp();
+    }
 }
 
 template <int P>
@@ -174,9 +186,11 @@ static void p2m_launch(bem_ctx *c)
         attr = true;
     }
     auto kern = c->has_dipole ? p2m_kernel_t<P, true> : p2m_kernel_t<P, false>;
-    kern<<<cdiv(nleaf, P2M_WARPS), P2M_WARPS * 32, smem, c->stream>>>(
+    CUDA_TRY(cudaMemsetAsync(c->p2p_counter.get() + 2, 0, sizeof(int), c->stream));
+    const int grid = std::max(1, std::min(cdiv(nleaf, P2M_WARPS), P2M_MINB * c->n_sm));     // the CTAs that fit an SM (registers, shared memory)
+    kern<<<grid, P2M_WARPS * 32, smem, c->stream>>>(
         sb.begin.get(), sb.bkey[lmax].get(), nleaf, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
-        c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
+        c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst, c->p2p_counter.get() + 2);
     KERNEL_CHECK();
 }
 
