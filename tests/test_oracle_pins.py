@@ -329,3 +329,90 @@ def test_monopole_sum_matches_definition():
     with np.errstate(divide="ignore"):
         k = np.where(d > 0, 1.0 / (4 * np.pi * d), 0.0)
     assert _rel(y, k @ m) < 1e-14
+
+
+# ------------------------------------------------------------------ surface functions and shape filter
+from oracle import surface_oracle as so   # noqa: E402
+
+
+def test_s1_vertex_geometry_on_the_sphere():
+    """Eq. 17: sum s_j = sum A_k exactly; on a sphere n_j -> r_j / R (the worst vertex is first order:
+    the error halves per refinement) and sum s_j -> 4 pi R^2 from below, O(h^2) (drops 4x per refinement)."""
+    R = 1.7
+    errs, area = [], []
+    for lvl in (2, 3, 4):
+        v, f = bi.icosphere(lvl)
+        s, n, A, _ = so.vertex_geometry(R * v, f)
+        assert abs(s.sum() - A.sum()) <= 1e-13 * A.sum()
+        errs.append(np.max(np.linalg.norm(n - v, axis=1)))
+        area.append(1.0 - s.sum() / (4 * np.pi * R * R))
+    assert all(a > 0 for a in area)
+    assert errs[2] < 1.5e-2 and 1.8 < errs[0] / errs[1] < 4.5 and 1.8 < errs[1] / errs[2] < 4.5
+    assert 3.5 < area[0] / area[1] < 4.5 and 3.5 < area[1] / area[2] < 4.5
+
+
+def test_s2_surface_velocity_of_a_linear_potential():
+    """Eqs. 22-27.  For phi = a.r the contour integral of Eq. 26 is exact on every flat triangle,
+    (n x v)_k = N_k x a, so Eq. 27 gives (n x v)_j = (m_j x a) / sum_{k ni j} A_k with m_j of Eq. 17 -- an identity that
+    fixes the orientation and every sign of Eq. 26; with q = n.a the full velocity tends to a, O(h^2), on a sphere."""
+    a = np.array([0.3, -1.1, 0.7])
+    errs = []
+    for lvl in (2, 3, 4):
+        v, f = bi.icosphere(lvl)
+        V = 0.9 * v + np.array([0.2, 0.1, -0.4])
+        s, n, A, Ntri = so.vertex_geometry(V, f)
+        phi = V @ a
+        vel = so.surface_velocity(V, f, phi, n @ a)
+        m = np.zeros_like(V)
+        for c in range(3):
+            np.add.at(m, f[:, c], Ntri * A[:, None])
+        nxv = np.cross(m, a) / (3.0 * s)[:, None]
+        expect = n * (n @ a)[:, None] + np.cross(nxv, n)
+        assert np.max(np.abs(vel - expect)) <= 1e-13
+        errs.append(np.max(np.linalg.norm(vel - a, axis=1)))
+    print(errs)
+    assert errs[2] < 3e-2 and 1.8 < errs[0] / errs[1] < 5.5 and 1.8 < errs[1] / errs[2] < 5.5
+
+
+def test_s3_harmonic_matrix_against_an_independent_implementation():
+    """G of Eq. 39: the m >= 0 cosine columns equal bem_inputs.sph.real_sph_harm (own Legendre recurrence; the scipy call of
+    the oracle could have its angles swapped), and the columns are orthonormal under the lumped quadrature s_j, O(h^2)."""
+    from bem_inputs.sph import real_sph_harm
+    v, f = bi.icosphere(4)
+    th, ph = _angles(v)
+    G = so.harmonic_matrix(th, ph, 6)
+    assert G.shape == (v.shape[0], 36)
+    col = 0
+    for n in range(6):
+        assert np.max(np.abs(G[:, col] - real_sph_harm(n, 0, th, ph))) <= 1e-13
+        col += 1
+        for m in range(1, n + 1):
+            assert np.max(np.abs(G[:, col] - np.sqrt(2.0) * real_sph_harm(n, m, th, ph))) <= 1e-13
+            col += 2
+    s, _, _, _ = so.vertex_geometry(v, f)
+    gram = G.T @ (G * s[:, None])
+    assert np.max(np.abs(gram - np.eye(36))) < 2e-2
+
+
+def test_s4_shape_filter_is_the_orthogonal_projector_on_the_band():
+    """Eq. 42: F = G (G* G)^-1 G* is the orthogonal projector on span{Y_n^m, n < p_f} sampled at the mesh
+    angles: F^2 = F = F^T, trace = p_f^2, band-limited samples pass unchanged (the unit sphere itself is n = 1; the
+    config-3 shape has coordinates of degree <= 7), anything else shrinks; the scale of the bubble does not matter."""
+    v, f = bi.icosphere(3)
+    th, ph = _angles(v)
+    p_f = 9
+    Fm = so.filter_matrix(th, ph, p_f)
+    assert np.max(np.abs(Fm @ Fm - Fm)) < 1e-12 and np.max(np.abs(Fm - Fm.T)) < 1e-12
+    assert abs(np.trace(Fm) - p_f ** 2) < 1e-10
+    assert np.max(np.abs(so.filter_apply(Fm, v.T) - v.T)) < 1e-12
+    from bem_inputs.sph import real_sph_harm
+    r = 1.0 + 0.3 * real_sph_harm(4, 2, th, ph) + 0.15 * real_sph_harm(6, 3, th, ph)
+    X = (r[:, None] * v).T                                              # degree <= 7 < p_f
+    assert np.max(np.abs(so.filter_apply(Fm, X) - X)) < 1e-11
+    assert np.max(np.abs(so.filter_apply(Fm, 3.7 * X) - 3.7 * X)) < 1e-10
+    hi = real_sph_harm(12, 5, th, ph)
+    assert np.linalg.norm(so.filter_apply(Fm, hi[None, :])) < 0.5 * np.linalg.norm(hi)
+    rng = np.random.default_rng(5)
+    noise = rng.standard_normal((3, v.shape[0]))
+    out = so.filter_apply(Fm, X + 1e-3 * noise) - X
+    assert np.linalg.norm(out) < 0.5 * np.linalg.norm(1e-3 * noise)     # ~ sqrt(81 / 642) of the noise survives
