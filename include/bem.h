@@ -208,6 +208,46 @@ const char *bem_last_error(const bem_ctx *ctx);
 /* Free every device allocation of the context.  NULL is allowed. */
 void bem_destroy(bem_ctx *ctx);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * The steps either side of the solve in one time step ("Surface" functions and filters, ~10% of an
+ * FMM call).  They need the mesh only, not bem_setup.
+ *
+ * bem_surface_velocity -- per vertex j (Eq. 17; Eqs. 22-27):
+ *     s_j = 1/3 sum_{k ni j} A_k,   n_j = m_j / |m_j|,   m_j = sum_{k ni j} N_k A_k                       (Eq. 17)
+ *     (n x v)_k A_k = 1/2 [ (r_k2 - r_k3) phi_k1 + (r_k3 - r_k1) phi_k2 + (r_k1 - r_k2) phi_k3 ]         (Eq. 26: the
+ *         contour integral of the linearly interpolated phi around triangle k, by Stokes' theorem, Eq. 23)
+ *     (n x v)_j = 1/(3 s_j) sum_{k ni j} (n x v)_k A_k,   v_j = n_j q_j + (n x v)_j x n_j                 (Eqs. 27, 22)
+ *   phi, q  [n_vertices] potential and its normal derivative (q may be NULL: tangential part only; phi may be NULL
+ *           when v is NULL)
+ *   v            [n_vertices x 3] row-major, or NULL
+ *   normals_out  [n_vertices x 3] n_j, or NULL;  areas_out [n_vertices] s_j, or NULL  (at least one output)
+ * Host or device pointers (host: staged and synchronised).  The sums over the triangles of a vertex run in mesh
+ * order (bit-reproducible).  BEM_ERR_INVALID_ARG for a point-cloud context. */
+bem_status bem_surface_velocity(bem_ctx *ctx, const double *phi, const double *q, double *v, double *normals_out,
+                                double *areas_out);
+
+/* Shape filter of bandwidth p_f (Eqs. 34-43): every bubble surface is a map of the unit sphere, the
+ * mesh points keep their spherical angles (theta_i, phi_i) for all times, and a surface function sampled at them is
+ * replaced by its least-squares fit with the spherical harmonics of degree n < p_f,
+ *     xhat = F x,   F = G (G* G)^-1 G*,   G_ij = Y_j(theta_i, phi_i),  j = (n, m), n = 0..p_f-1          (Eqs. 39-42)
+ * -- the orthogonal projector on the band.  One filter serves all bubbles that share the angles of their mesh points
+ * ("only one shape filter is necessary when all bubbles have the same initial shape").  The library keeps
+ * F in its factored form (rank p_f^2 << N_d): xhat = G (G^+ x), G^+ = (G^T G)^-1 G^T by a Cholesky factorisation on
+ * the device, in the real orthonormal harmonic basis (same span as Eq. 37, so the same F).
+ *
+ * bem_filter_create -- theta (polar angle), phi (azimuth): [n_d] angles of the points of ONE bubble, host or device,
+ *   copied.  1 <= p_f <= 16 and p_f^2 < n_d.  BEM_ERR_BAD_MESH when G^T G is singular (the points do not
+ *   resolve the band).
+ * bem_filter_apply -- x, xhat: [n_cols x n_d] row-major; a column c = (surface function, bubble) is the n_d samples of
+ *   that function on that bubble (x, y, z, phi, ... of Eqs. 41, 43), contiguous.  xhat may be x (in place).  Host or
+ *   device pointers; enqueued on cuda_stream (a cudaStream_t, NULL = default stream), synchronised only for host
+ *   pointers. */
+typedef struct bem_filter bem_filter;
+bem_status bem_filter_create(const double *theta, const double *phi, int64_t n_d, int p_f, bem_filter **out);
+bem_status bem_filter_apply(bem_filter *f, const double *x, int64_t n_cols, double *xhat, void *cuda_stream);
+const char *bem_filter_last_error(const bem_filter *f);
+void bem_filter_destroy(bem_filter *f);
+
 #ifdef __cplusplus
 }
 #endif

@@ -30,7 +30,8 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
 
 # every symbol include/bem.h declares
 EXPORTS = ["bem_create", "bem_create_points", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
-           "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy"]
+           "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy",
+           "bem_surface_velocity", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy"]
 
 
 class BemError(RuntimeError):
@@ -68,8 +69,15 @@ def load_library() -> ctypes.CDLL:
     lib.bem_last_error.restype = ctypes.c_char_p
     lib.bem_destroy.argtypes = [vp]
     lib.bem_destroy.restype = None
+    lib.bem_surface_velocity.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.bem_filter_create.argtypes = [vp, vp, i64, i32, ctypes.POINTER(vp)]
+    lib.bem_filter_apply.argtypes = [vp, vp, i64, vp, vp]
+    lib.bem_filter_last_error.argtypes = [vp]
+    lib.bem_filter_last_error.restype = ctypes.c_char_p
+    lib.bem_filter_destroy.argtypes = [vp]
+    lib.bem_filter_destroy.restype = None
     for name in EXPORTS:
-        if name not in ("bem_last_error", "bem_destroy"):
+        if name not in ("bem_last_error", "bem_destroy", "bem_filter_last_error", "bem_filter_destroy"):
             getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -174,6 +182,11 @@ class Bem:
         self._check(self._lib.bem_fp64_tensor_peak(self._ctx, ctypes.byref(g)))
         return g.value
 
+    def bem_surface_velocity(self, phi, q, v=None, normals_out=None, areas_out=None):
+        """v = n q + v_t (Eqs. 22-27), vertex normals and areas (Eq. 17); outputs may be None (at least one given)."""
+        self._check(self._lib.bem_surface_velocity(self._ctx, _ptr(phi), _ptr(q), _ptr(v), _ptr(normals_out), _ptr(areas_out)))
+        return v
+
     def bem_destroy(self):
         if self._ctx:
             self._lib.bem_destroy(self._ctx)
@@ -193,3 +206,41 @@ def bem_create(vertices, triangles, bubble_id=None) -> Bem:
 def bem_create_points(sources, targets) -> Bem:
     """Point-cloud mode (include/bem.h): bem_apply(q[n_sources], None, y[n_targets])."""
     return Bem(None, None, None, _points=(sources, targets))
+
+
+class BemFilter:
+    """Shape filter of bandwidth p_f (an owned `bem_filter *`): bem_filter_create / bem_filter_apply / bem_filter_destroy."""
+
+    def __init__(self, theta, phi, p_f: int):
+        self._lib = load_library()
+        self._f = ctypes.c_void_p(0)
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        ph = np.ascontiguousarray(phi, dtype=np.float64)
+        if th.ndim != 1 or th.shape != ph.shape:
+            raise ValueError("theta and phi must be [n_d]")
+        self.n_d, self.p_f = th.shape[0], int(p_f)
+        st = self._lib.bem_filter_create(th.ctypes.data, ph.ctypes.data, th.shape[0], int(p_f), ctypes.byref(self._f))
+        if st != BEM_OK:
+            self._f = ctypes.c_void_p(0)
+            raise BemError(st, "bem_filter_create failed (need 1 <= p_f <= 16, p_f^2 < n_d, angles that resolve the band, a CUDA device)")
+
+    def bem_filter_apply(self, x, n_cols: int, xhat, stream_handle: int = 0):
+        st = self._lib.bem_filter_apply(self._f, _ptr(x), int(n_cols), _ptr(xhat), ctypes.c_void_p(stream_handle))
+        if st != BEM_OK:
+            raise BemError(st, self._lib.bem_filter_last_error(self._f).decode())
+        return xhat
+
+    def bem_filter_destroy(self):
+        if self._f:
+            self._lib.bem_filter_destroy(self._f)
+            self._f = ctypes.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.bem_filter_destroy()
+        except Exception:
+            pass
+
+
+def bem_filter_create(theta, phi, p_f: int) -> BemFilter:
+    return BemFilter(theta, phi, p_f)

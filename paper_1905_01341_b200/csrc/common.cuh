@@ -140,6 +140,10 @@ struct bem_ctx {
     bem::dvec<double> P;            // point-cloud mode (quadrature == 2): [np*3] source points; V holds the targets
     int64_t np = 0;
 
+    // vertex -> incident triangle corners, sorted by vertex (bem_surface_velocity; built at first use)
+    bem::dvec<int32_t> vc_begin;    // [N+1]
+    bem::dvec<uint32_t> vc_corner;  // [3T] corner index 3 k + a, in mesh order within a vertex
+
     // options
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
     int precond = 0;                // bem_solve: 0 = unpreconditioned (the paper), 1 = right diagonal scaling by S_ii

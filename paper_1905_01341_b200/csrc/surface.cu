@@ -1,0 +1,344 @@
+// The steps either side of the solve in a time step (include/bem.h):
+//   bem_surface_velocity   vertex areas and normals (Eq. 17) and the surface velocity
+//                          v = n q + (n x v) x n with n x v from the contour integrals of phi (Eqs. 22-27)
+//   bem_filter_*           the shape filter F = G (G* G)^-1 G* of bandwidth p_f (Eqs. 37-43), kept in
+//                          the factored form  xhat = G (G^+ x)  (rank p_f^2 << N_d) and applied to all bubbles and all
+//                          surface functions at once
+#include "common.cuh"
+
+#include <algorithm>
+#include <cmath>
+
+namespace bem {
+bool is_device_ptr(const void *p);      // api.cu
+
+// ------------------------------------------------------------------ vertex -> incident corners (fixed summation order)
+__global__ void sv_corner_keys(const int32_t *F, int64_t n, uint64_t *keys)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) keys[i] = (uint64_t)F[i];
+}
+__global__ void sv_vertex_ranges(const uint64_t *keys, int64_t n, int64_t N, int32_t *begin)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i > n) return;
+    const int64_t lo = (i == 0) ? -1 : (int64_t)keys[i - 1];          // begin[v] = first i with keys[i] >= v
+    const int64_t hi = (i == n) ? N : (int64_t)keys[i];
+    for (int64_t v = lo + 1; v <= hi; ++v) begin[v] = (int32_t)i;
+}
+
+static void build_vertex_corners(bem_ctx *c)
+{
+    if (c->vc_begin.p && c->vc_begin.n == (size_t)c->N + 1) return;
+    cudaStream_t s = c->stream;
+    const int64_t nc = 3 * c->T;
+    dvec<uint64_t> keys, keys_tmp;
+    dvec<uint32_t> vals_tmp;
+    keys.alloc(nc); keys_tmp.alloc(nc); vals_tmp.alloc(nc);
+    c->vc_corner.alloc(nc);
+    c->vc_begin.alloc(c->N + 1);
+    sv_corner_keys<<<cdiv(nc, 256), 256, 0, s>>>(c->F.get(), nc, keys.get());
+    KERNEL_CHECK();
+    iota_u32(c->vc_corner.get(), nc, s);
+    radix_sort_pairs(keys.get(), c->vc_corner.get(), keys_tmp.get(), vals_tmp.get(), nc, 0, 32, s);   // stable: corners of a vertex in mesh order
+    sv_vertex_ranges<<<cdiv(nc + 1, 256), 256, 0, s>>>(keys.get(), nc, c->N, c->vc_begin.get());
+    KERNEL_CHECK();
+    CUDA_TRY(cudaStreamSynchronize(s));
+}
+
+// ------------------------------------------------------------------ Eq. 17 and Eqs. 22-27, one thread per vertex
+__global__ void surface_velocity_kernel(const double *__restrict__ V, const int32_t *__restrict__ F, const int32_t *__restrict__ begin,
+                                        const uint32_t *__restrict__ corner, const double *__restrict__ phi, const double *__restrict__ q,
+                                        int64_t N, double *__restrict__ vel, double *__restrict__ nrm, double *__restrict__ area)
+{
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    double s3 = 0.0, mx = 0.0, my = 0.0, mz = 0.0, wx = 0.0, wy = 0.0, wz = 0.0;     // 3 s_j, m_j, sum (n x v)_k A_k
+    for (int i = begin[j]; i < begin[j + 1]; ++i) {
+        const int64_t k = corner[i] / 3;
+        const int v1 = F[3 * k], v2 = F[3 * k + 1], v3 = F[3 * k + 2];
+        const double x1 = V[3 * (int64_t)v1], y1 = V[3 * (int64_t)v1 + 1], z1 = V[3 * (int64_t)v1 + 2];
+        const double x2 = V[3 * (int64_t)v2], y2 = V[3 * (int64_t)v2 + 1], z2 = V[3 * (int64_t)v2 + 2];
+        const double x3 = V[3 * (int64_t)v3], y3 = V[3 * (int64_t)v3 + 1], z3 = V[3 * (int64_t)v3 + 2];
+        const double ax = x2 - x1, ay = y2 - y1, az = z2 - z1, bx = x3 - x1, by = y3 - y1, bz = z3 - z1;
+        const double cx = ay * bz - az * by, cy = az * bx - ax * bz, cz = ax * by - ay * bx;        // N_k 2 A_k
+        s3 += 0.5 * sqrt(cx * cx + cy * cy + cz * cz);
+        mx += 0.5 * cx; my += 0.5 * cy; mz += 0.5 * cz;
+        if (phi) {
+            const double f1 = phi[v1], f2 = phi[v2], f3 = phi[v3];                                  // Eq. 26 times A_k
+            wx += 0.5 * ((x2 - x3) * f1 + (x3 - x1) * f2 + (x1 - x2) * f3);
+            wy += 0.5 * ((y2 - y3) * f1 + (y3 - y1) * f2 + (y1 - y2) * f3);
+            wz += 0.5 * ((z2 - z3) * f1 + (z3 - z1) * f2 + (z1 - z2) * f3);
+        }
+    }
+    const double im = 1.0 / sqrt(mx * mx + my * my + mz * mz);
+    const double nx = mx * im, ny = my * im, nz = mz * im;
+    if (nrm) { nrm[3 * j] = nx; nrm[3 * j + 1] = ny; nrm[3 * j + 2] = nz; }
+    if (area) area[j] = s3 / 3.0;
+    if (vel) {
+        const double ux = wx / s3, uy = wy / s3, uz = wz / s3;                                      // (n x v)_j, Eq. 27
+        const double qq = q ? q[j] : 0.0;
+        vel[3 * j] = nx * qq + (uy * nz - uz * ny);                                                 // Eq. 22
+        vel[3 * j + 1] = ny * qq + (uz * nx - ux * nz);
+        vel[3 * j + 2] = nz * qq + (ux * ny - uy * nx);
+    }
+}
+
+// ------------------------------------------------------------------ shape filter
+}  // namespace bem
+
+struct bem_filter {
+    int device = 0;
+    int64_t nd = 0;
+    int pf = 0, P = 0;
+    bem::dvec<double> GT;       // [P x nd]   GT[j][i] = Y_j(theta_i, phi_i)        (Eq. 39, real orthonormal basis)
+    bem::dvec<double> GpT;      // [nd x P]   GpT[i][j] = ((G^T G)^-1 G^T)[j][i]     (Eq. 40)
+    bem::dvec<double> stage_in, stage_out;
+    std::string err;
+};
+
+namespace bem {
+
+// real orthonormal Y_n^m (Condon-Shortley phase) of one point: column n^2 (m = 0), n^2 + 2m - 1 (cos), n^2 + 2m (sin)
+__global__ void filter_harmonics_kernel(const double *__restrict__ theta, const double *__restrict__ phi, int64_t nd, int pf, int P,
+                                        double *__restrict__ GT)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nd) return;
+    const double ct = cos(theta[i]), st = sin(theta[i]), ph = phi[i];
+    double pmm = 0.28209479177387814347403972578039;                  // sqrt(1 / 4 pi)
+    for (int m = 0; m < pf; ++m) {
+        if (m > 0) pmm *= -sqrt((2.0 * m + 1.0) / (2.0 * m)) * st;
+        const double cm = m == 0 ? 1.0 : 1.4142135623730950488 * cos(m * ph), sm = 1.4142135623730950488 * sin(m * ph);
+        double p2 = 0.0, p1 = pmm;
+        for (int n = m; n < pf; ++n) {
+            double pn;
+            if (n == m) pn = pmm;
+            else {
+                const double a = sqrt((4.0 * n * n - 1.0) / ((double)n * n - (double)m * m));
+                const double b = sqrt((((double)n - 1.0) * (n - 1.0) - (double)m * m) / (4.0 * (n - 1.0) * (n - 1.0) - 1.0));
+                pn = a * (ct * p1 - b * p2);
+            }
+            p2 = p1; p1 = pn;
+            if (m == 0) GT[(size_t)(n * n) * nd + i] = pn;
+            else { GT[(size_t)(n * n + 2 * m - 1) * nd + i] = pn * cm; GT[(size_t)(n * n + 2 * m) * nd + i] = pn * sm; }
+        }
+    }
+}
+
+// A = G^T G, one thread per entry (fixed order)
+__global__ void filter_gram_kernel(const double *__restrict__ GT, int64_t nd, int P, double *__restrict__ A)
+{
+    const int a = blockIdx.x, b = blockIdx.y * blockDim.x + threadIdx.x;
+    if (b >= P) return;
+    const double *ra = GT + (size_t)a * nd, *rb = GT + (size_t)b * nd;
+    double s = 0.0;
+    for (int64_t i = 0; i < nd; ++i) s = fma(ra[i], rb[i], s);
+    A[(size_t)a * P + b] = s;
+}
+
+// in-place Cholesky A = L L^T (lower triangle), one CTA; *ok = 0 if a pivot is not positive
+__global__ void filter_cholesky_kernel(double *A, int P, int *ok)
+{
+    __shared__ double piv;
+    for (int k = 0; k < P; ++k) {
+        if (threadIdx.x == 0) {
+            const double d = A[(size_t)k * P + k];
+            if (!(d > 0.0)) *ok = 0;
+            piv = sqrt(d > 0.0 ? d : 1.0);
+            A[(size_t)k * P + k] = piv;
+        }
+        __syncthreads();
+        for (int i = k + 1 + threadIdx.x; i < P; i += blockDim.x) A[(size_t)i * P + k] /= piv;
+        __syncthreads();
+        for (int i = k + 1 + threadIdx.x; i < P; i += blockDim.x) {
+            const double lik = A[(size_t)i * P + k];
+            for (int j = k + 1; j <= i; ++j) A[(size_t)i * P + j] -= lik * A[(size_t)j * P + k];
+        }
+        __syncthreads();
+    }
+}
+
+// GpT[i][:] = (L L^T)^-1 G[i][:], one thread per mesh point
+__global__ void filter_solve_kernel(const double *__restrict__ L, const double *__restrict__ GT, int64_t nd, int P, double *__restrict__ GpT)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nd) return;
+    double *z = GpT + (size_t)i * P;
+    for (int j = 0; j < P; ++j) {                                      // L w = g
+        double s = GT[(size_t)j * nd + i];
+        for (int k = 0; k < j; ++k) s -= L[(size_t)j * P + k] * z[k];
+        z[j] = s / L[(size_t)j * P + j];
+    }
+    for (int j = P - 1; j >= 0; --j) {                                 // L^T z = w
+        double s = z[j];
+        for (int k = j + 1; k < P; ++k) s -= L[(size_t)k * P + j] * z[k];
+        z[j] = s / L[(size_t)j * P + j];
+    }
+}
+
+// xhat[c][:] = G (G^+ x[c][:]) for FC columns per CTA: x rows staged in shared memory, the P coefficients of every
+// column in shared memory, G^T and G^+T streamed from L2 (coalesced over the thread index in both passes)
+constexpr int FILTER_THREADS = 256;
+__global__ void __launch_bounds__(FILTER_THREADS)
+filter_apply_kernel(const double *__restrict__ x, int64_t ncols, int64_t nd, int P, int fc, const double *__restrict__ GT,
+                    const double *__restrict__ GpT, double *__restrict__ xhat)
+{
+    extern __shared__ double fsm[];
+    double *xs = fsm;                        // [fc][nd]
+    double *cs = fsm + (size_t)fc * nd;      // [fc][P]
+    const int64_t c0 = (int64_t)blockIdx.x * fc;
+    const int nc = (int)min((int64_t)fc, ncols - c0);
+    for (int64_t e = threadIdx.x; e < (int64_t)nc * nd; e += FILTER_THREADS) xs[e] = x[c0 * nd + e];
+    __syncthreads();
+    for (int j = threadIdx.x; j < P; j += FILTER_THREADS) {            // coefficients: C[c][j] = sum_i G^+[j][i] x[c][i]
+        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int64_t i = 0; i < nd; ++i) {
+            const double g = GpT[(size_t)i * P + j];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) if (c < nc) acc[c] = fma(xs[(size_t)c * nd + i], g, acc[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c) if (c < nc) cs[(size_t)c * P + j] = acc[c];
+    }
+    __syncthreads();
+    for (int64_t i = threadIdx.x; i < nd; i += FILTER_THREADS) {       // xhat[c][i] = sum_j G[i][j] C[c][j]
+        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        for (int j = 0; j < P; ++j) {
+            const double g = GT[(size_t)j * nd + i];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) if (c < nc) acc[c] = fma(cs[(size_t)c * P + j], g, acc[c]);
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c) if (c < nc) xhat[(c0 + c) * nd + i] = acc[c];
+    }
+}
+
+}  // namespace bem
+
+using namespace bem;
+
+extern "C" {
+
+bem_status bem_surface_velocity(bem_ctx *c, const double *phi, const double *q, double *v, double *normals_out, double *areas_out)
+{
+    if (!c || (!v && !normals_out && !areas_out)) return BEM_ERR_INVALID_ARG;
+    if (c->quadrature == 2 || c->T == 0) { c->err = "bem_surface_velocity: the context holds a point cloud, not a mesh"; return BEM_ERR_INVALID_ARG; }
+    if (v && !phi) { c->err = "bem_surface_velocity: phi is required for the velocity"; return BEM_ERR_INVALID_ARG; }
+    try {
+        CUDA_TRY(cudaSetDevice(c->device));
+        build_vertex_corners(c);
+        const int64_t N = c->N;
+        cudaStream_t s = c->stream;
+        dvec<double> dphi, dq, dv, dn, da;
+        auto in = [&](const double *h, dvec<double> &d) -> const double * {
+            if (!h || is_device_ptr(h)) return h;
+            d.alloc(N);
+            CUDA_TRY(cudaMemcpyAsync(d.get(), h, N * sizeof(double), cudaMemcpyHostToDevice, s));
+            return d.get();
+        };
+        auto out = [&](double *h, dvec<double> &d, int64_t n) -> double * {
+            if (!h || is_device_ptr(h)) return h;
+            d.alloc(n);
+            return d.get();
+        };
+        const double *pphi = in(phi, dphi), *pq = in(q, dq);
+        double *pv = out(v, dv, 3 * N), *pn = out(normals_out, dn, 3 * N), *pa = out(areas_out, da, N);
+        surface_velocity_kernel<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), c->F.get(), c->vc_begin.get(), c->vc_corner.get(), pphi, pq, N, pv, pn, pa);
+        KERNEL_CHECK();
+        bool sync = false;
+        if (pv != v) { CUDA_TRY(cudaMemcpyAsync(v, pv, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, s)); sync = true; }
+        if (pn != normals_out) { CUDA_TRY(cudaMemcpyAsync(normals_out, pn, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, s)); sync = true; }
+        if (pa != areas_out) { CUDA_TRY(cudaMemcpyAsync(areas_out, pa, N * sizeof(double), cudaMemcpyDeviceToHost, s)); sync = true; }
+        if (sync || dphi.p || dq.p) CUDA_TRY(cudaStreamSynchronize(s));
+        return BEM_OK;
+    } catch (const Error &e) {
+        c->err = e.what();
+        cudaGetLastError();
+        return e.status;
+    }
+}
+
+bem_status bem_filter_create(const double *theta, const double *phi, int64_t n_d, int p_f, bem_filter **out)
+{
+    if (!out) return BEM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!theta || !phi || n_d < 4 || p_f < 1 || p_f > 16 || (int64_t)p_f * p_f >= n_d) return BEM_ERR_INVALID_ARG;   // p_f < sqrt(N_d)
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return BEM_ERR_CUDA; }
+    bem_filter *f = new (std::nothrow) bem_filter();
+    if (!f) return BEM_ERR_OOM;
+    cudaGetDevice(&f->device);
+    f->nd = n_d; f->pf = p_f; f->P = p_f * p_f;
+    try {
+        const int P = f->P;
+        dvec<double> th, ph, A;
+        dvec<int> ok;
+        th.alloc(n_d); ph.alloc(n_d); A.alloc((size_t)P * P); ok.alloc(1);
+        CUDA_TRY(cudaMemcpy(th.get(), theta, n_d * sizeof(double), cudaMemcpyDefault));
+        CUDA_TRY(cudaMemcpy(ph.get(), phi, n_d * sizeof(double), cudaMemcpyDefault));
+        f->GT.alloc((size_t)P * n_d);
+        f->GpT.alloc((size_t)n_d * P);
+        filter_harmonics_kernel<<<cdiv(n_d, 128), 128>>>(th.get(), ph.get(), n_d, p_f, P, f->GT.get());
+        KERNEL_CHECK();
+        filter_gram_kernel<<<dim3(P, cdiv(P, 64)), 64>>>(f->GT.get(), n_d, P, A.get());
+        KERNEL_CHECK();
+        const int one = 1;
+        CUDA_TRY(cudaMemcpy(ok.get(), &one, sizeof(int), cudaMemcpyHostToDevice));
+        filter_cholesky_kernel<<<1, 256>>>(A.get(), P, ok.get());
+        KERNEL_CHECK();
+        filter_solve_kernel<<<cdiv(n_d, 64), 64>>>(A.get(), f->GT.get(), n_d, P, f->GpT.get());
+        KERNEL_CHECK();
+        int h_ok = 0;
+        CUDA_TRY(cudaMemcpy(&h_ok, ok.get(), sizeof(int), cudaMemcpyDeviceToHost));
+        if (!h_ok) { delete f; return BEM_ERR_BAD_MESH; }            // the angles do not resolve the band: G^T G is singular
+    } catch (const Error &e) {
+        cudaGetLastError();
+        const bem_status st = e.status;
+        delete f;
+        return st;
+    }
+    *out = f;
+    return BEM_OK;
+}
+
+bem_status bem_filter_apply(bem_filter *f, const double *x, int64_t n_cols, double *xhat, void *cuda_stream)
+{
+    if (!f || !x || !xhat || n_cols < 0) return BEM_ERR_INVALID_ARG;
+    if (n_cols == 0) return BEM_OK;
+    try {
+        CUDA_TRY(cudaSetDevice(f->device));
+        cudaStream_t s = (cudaStream_t)cuda_stream;
+        const size_t n = (size_t)n_cols * f->nd;
+        const bool hx = !is_device_ptr(x), hy = !is_device_ptr(xhat);
+        const double *dx = x;
+        double *dy = xhat;
+        if (hx) { if (f->stage_in.n < n) f->stage_in.alloc(n); CUDA_TRY(cudaMemcpyAsync(f->stage_in.get(), x, n * sizeof(double), cudaMemcpyHostToDevice, s)); dx = f->stage_in.get(); }
+        if (hy) { if (f->stage_out.n < n) f->stage_out.alloc(n); dy = f->stage_out.get(); }
+        int fc = 8;
+        while (fc > 1 && ((size_t)fc * (f->nd + f->P)) * sizeof(double) > 160 * 1024) fc >>= 1;
+        const size_t smem = ((size_t)fc * (f->nd + f->P)) * sizeof(double);
+        if (smem > 200 * 1024) { f->err = "bem_filter_apply: N_d too large for the shared-memory staging"; return BEM_ERR_INVALID_ARG; }
+        CUDA_TRY(cudaFuncSetAttribute(filter_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        filter_apply_kernel<<<cdiv(n_cols, fc), FILTER_THREADS, smem, s>>>(dx, n_cols, f->nd, f->P, fc, f->GT.get(), f->GpT.get(), dy);
+        KERNEL_CHECK();
+        if (hy) CUDA_TRY(cudaMemcpyAsync(xhat, dy, n * sizeof(double), cudaMemcpyDeviceToHost, s));
+        if (hx || hy) CUDA_TRY(cudaStreamSynchronize(s));
+        return BEM_OK;
+    } catch (const Error &e) {
+        f->err = e.what();
+        cudaGetLastError();
+        return e.status;
+    }
+}
+
+const char *bem_filter_last_error(const bem_filter *f) { return f ? f->err.c_str() : "null filter"; }
+
+void bem_filter_destroy(bem_filter *f)
+{
+    if (!f) return;
+    cudaSetDevice(f->device);
+    delete f;
+}
+
+}  // extern "C"
