@@ -102,8 +102,11 @@ def make_config(cfg: int, n_bubbles: int | None = None):
         name = f"cfg{cfg}: {n} bubbles in cube {side:.3g}, icosphere L3, {V.shape[0]:,} nodes"
     else:
         raise ValueError("cfg must be 1..5")
+    # unit-sphere template whose vertex angles every bubble of the config keeps (the correspondence point index ->
+    # (theta, phi) of the shape filter); the bubbles follow each other in V, template order inside each
+    template = {1: 3, 2: 4, 3: 7, 4: 3, 5: 3}[cfg]
     out = dict(V=np.ascontiguousarray(V), F=np.ascontiguousarray(F, dtype=np.int32),
-               bubble_id=bid, q=q, phi=phi, name=name, cfg=cfg)
+               bubble_id=bid, q=q, phi=phi, name=name, cfg=cfg, template=icosphere(template)[0])
     out.update(CONFIG_PARAMS[cfg])
     return out
 

@@ -348,6 +348,31 @@ def run_gpu(args):
                      parity_rel_l2_vs_oracle=float(np.linalg.norm(ym[rows] - yo) / np.linalg.norm(yo)),
                      rel_l2_vs_fp64_path=float(np.linalg.norm(ym - y) / np.linalg.norm(y)))
 
+    # the steps either side of the solve in a time step: surface velocity, shape filter
+    extras = None
+    if not cloud and not args.direct:
+        vd = torch.empty(N, 3, dtype=torch.float64, device="cuda")
+        ctx.bem_surface_velocity(pd, qd, vd)
+        torch.cuda.synchronize()
+        sv_ms = timed(lambda: ctx.bem_surface_velocity(pd, qd, vd), args.steps) / args.steps
+        extras = dict(surface_velocity_ms=sv_ms, surface_velocity_note="Eq. 17 + Eqs. 22-27, one thread per vertex")
+        tmpl = c.get("template")
+        if tmpl is not None and 81 < tmpl.shape[0] <= 2600:         # all bubbles share the angles of one template mesh
+            th = np.arccos(np.clip(tmpl[:, 2], -1, 1)); ph = np.arctan2(tmpl[:, 1], tmpl[:, 0])
+            nd, p_f = tmpl.shape[0], 9
+            flt = bem.bem_filter_create(th, ph, p_f)
+            nbub = N // nd
+            X = torch.cat([torch.tensor(np.ascontiguousarray(V.T), device="cuda").reshape(3 * nbub, nd), pd.reshape(nbub, nd)]).contiguous()
+            Y = torch.empty_like(X)
+            flt.bem_filter_apply(X, X.shape[0], Y, stream.cuda_stream)
+            torch.cuda.synchronize()
+            f_ms = timed(lambda: flt.bem_filter_apply(X, X.shape[0], Y, stream.cuda_stream), args.steps) / args.steps
+            flop = 4.0 * p_f * p_f * nd * X.shape[0]
+            extras.update(filter_ms=f_ms, filter_columns=int(X.shape[0]), filter_bandwidth=p_f, filter_points_per_bubble=int(nd),
+                          filter_tflops=flop / (f_ms * 1e-3) / 1e12, filter_frac_of_fp64_peak=flop / (f_ms * 1e-3) / 1e9 / FP64_NOMINAL_GFLOPS,
+                          filter_note="xhat = G (G^+ x) on x, y, z, phi of every bubble: 4 p_f^2 N_d flop per column; the paper's dense F x would be 2 N_d^2")
+            flt.bem_filter_destroy()
+
     solve = None
     if args.solve_iters > 0 and not cloud:
         solve = {}
@@ -376,7 +401,7 @@ def run_gpu(args):
                 gpu_launches=int(stats["kernel_launches_per_apply"]) * args.steps,
                 clocks=clocks, roofline=roof, cpu_baseline=cpu, parity_rel_l2_vs_oracle=parity,
                 breakdown_ms=breakdown, kernels=kernels, setup_ms=stats["setup_ms"], setup_wall_ms=setup_wall_ms,
-                m2l_pairs=int(stats["m2l_pairs"]), solve=solve, mixed_precision_option=mixed,
+                m2l_pairs=int(stats["m2l_pairs"]), solve=solve, mixed_precision_option=mixed, time_step_extras=extras,
                 paper_context=("paper Table 2 (PAPER.md:479-490): at N=1,048,576, p=12 the FMM+GPU (double) product is 2309x faster than the CPU "
                                "brute force and the brute-force GPU (double) 33x, Xeon 5660 + Tesla K20" if cloud else
                                "paper Table 3 (PAPER.md:606): 1 MVP = 4.0 s at N=2,629,632, p=12, double, Xeon 5660 x12 cores + Tesla K20"))

@@ -191,15 +191,28 @@ filter_apply_kernel(const double *__restrict__ x, int64_t ncols, int64_t nd, int
     const int nc = (int)min((int64_t)fc, ncols - c0);
     for (int64_t e = threadIdx.x; e < (int64_t)nc * nd; e += FILTER_THREADS) xs[e] = x[c0 * nd + e];
     __syncthreads();
-    for (int j = threadIdx.x; j < P; j += FILTER_THREADS) {            // coefficients: C[c][j] = sum_i G^+[j][i] x[c][i]
-        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        for (int64_t i = 0; i < nd; ++i) {
-            const double g = GpT[(size_t)i * P + j];
+    // coefficients C[c][j] = sum_i G^+[j][i] x[c][i]: thread (j, g) sums the points i = g (mod groups); the partial
+    // sums of the groups are added in a fixed order
+    const int groups = max(1, FILTER_THREADS / P);
+    double *part = cs + (size_t)fc * P;      // [groups][fc][P]
+    {
+        const int j = threadIdx.x % P, g = threadIdx.x / P;
+        if (g < groups) {
+            double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            for (int64_t i = g; i < nd; i += groups) {
+                const double gp = GpT[(size_t)i * P + j];
 #pragma unroll
-            for (int c = 0; c < 8; ++c) if (c < nc) acc[c] = fma(xs[(size_t)c * nd + i], g, acc[c]);
+                for (int c = 0; c < 8; ++c) if (c < nc) acc[c] = fma(xs[(size_t)c * nd + i], gp, acc[c]);
+            }
+#pragma unroll
+            for (int c = 0; c < 8; ++c) if (c < nc) part[((size_t)g * fc + c) * P + j] = acc[c];
         }
-#pragma unroll
-        for (int c = 0; c < 8; ++c) if (c < nc) cs[(size_t)c * P + j] = acc[c];
+    }
+    __syncthreads();
+    for (int e = threadIdx.x; e < nc * P; e += FILTER_THREADS) {
+        double sum = 0.0;
+        for (int g = 0; g < groups; ++g) sum += part[(size_t)g * fc * P + e];
+        cs[e] = sum;
     }
     __syncthreads();
     for (int64_t i = threadIdx.x; i < nd; i += FILTER_THREADS) {       // xhat[c][i] = sum_j G[i][j] C[c][j]
@@ -316,8 +329,10 @@ bem_status bem_filter_apply(bem_filter *f, const double *x, int64_t n_cols, doub
         if (hx) { if (f->stage_in.n < n) f->stage_in.alloc(n); CUDA_TRY(cudaMemcpyAsync(f->stage_in.get(), x, n * sizeof(double), cudaMemcpyHostToDevice, s)); dx = f->stage_in.get(); }
         if (hy) { if (f->stage_out.n < n) f->stage_out.alloc(n); dy = f->stage_out.get(); }
         int fc = 8;
-        while (fc > 1 && ((size_t)fc * (f->nd + f->P)) * sizeof(double) > 160 * 1024) fc >>= 1;
-        const size_t smem = ((size_t)fc * (f->nd + f->P)) * sizeof(double);
+        const int groups = std::max(1, FILTER_THREADS / f->P);
+        auto bytes = [&](int k) { return ((size_t)k * (f->nd + (size_t)(1 + groups) * f->P)) * sizeof(double); };
+        while (fc > 1 && bytes(fc) > 160 * 1024) fc >>= 1;
+        const size_t smem = bytes(fc);
         if (smem > 200 * 1024) { f->err = "bem_filter_apply: N_d too large for the shared-memory staging"; return BEM_ERR_INVALID_ARG; }
         CUDA_TRY(cudaFuncSetAttribute(filter_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         filter_apply_kernel<<<cdiv(n_cols, fc), FILTER_THREADS, smem, s>>>(dx, n_cols, f->nd, f->P, fc, f->GT.get(), f->GpT.get(), dy);
