@@ -83,3 +83,48 @@ def filter_apply(Fm, x):
     """xhat[c, :] = F x[c, :] for every column c = (surface function, bubble): x is [n_cols, N_d] (Eqs. 41, 43)."""
     x = np.asarray(x, dtype=np.float64)
     return x @ Fm.T
+
+
+def one_ring_first_five(F, N):
+    """The five neighbours of every vertex used by the paraboloid fit ("when more than 5 neighbors are
+    available, we use just 5" -- which five is not said; reading R32 of DESIGN.md): walk the triangles that hold the
+    vertex in mesh order (triangle index, then corner index), and of each take the two other vertices in the
+    triangle's cyclic order; keep the first five distinct ones.  Returns [N, 5] (-1 where a vertex has fewer)."""
+    F = np.asarray(F, dtype=np.int64)
+    ring = [[] for _ in range(N)]
+    for k in range(F.shape[0]):
+        for a in range(3):
+            j = int(F[k, a])
+            for b in (F[k, (a + 1) % 3], F[k, (a + 2) % 3]):
+                b = int(b)
+                if b not in ring[j] and len(ring[j]) < 5:
+                    ring[j].append(b)
+    out = -np.ones((N, 5), dtype=np.int64)
+    for j, r in enumerate(ring):
+        out[j, :len(r)] = r
+    return out
+
+
+def mean_curvature(V, F):
+    """H_j = -B_j^(3) - B_j^(5) (Eq. 29) from the paraboloid z = B1 x + B2 y + B3 x^2 + B4 x y + B5 y^2 through five
+    neighbours (Eq. 28), in a frame centred at r_j whose z axis is the vertex normal n_j of Eq. 17.  The sum B3 + B5 does
+    not depend on the choice of the x, y axes.  Positive for a sphere with the normal out of the bubble: H = 1/R."""
+    V = np.asarray(V, dtype=np.float64)
+    N = V.shape[0]
+    _, n, _, _ = vertex_geometry(V, F)
+    ring = one_ring_first_five(F, N)
+    H = np.zeros(N)
+    for j in range(N):
+        if ring[j].min() < 0:
+            H[j] = np.nan
+            continue
+        z = n[j]
+        a = np.array([1.0, 0.0, 0.0]) if abs(z[0]) < 0.9 else np.array([0.0, 1.0, 0.0])
+        ex = np.cross(z, a); ex /= np.linalg.norm(ex)
+        ey = np.cross(z, ex)
+        d = V[ring[j]] - V[j]
+        x, y, zz = d @ ex, d @ ey, d @ z
+        Q = np.stack([x, y, x * x, x * y, y * y], axis=1)            # Eq. 28
+        B = np.linalg.solve(Q, zz)
+        H[j] = -B[2] - B[4]                                           # Eq. 29
+    return H

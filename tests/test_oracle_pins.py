@@ -416,3 +416,30 @@ def test_s4_shape_filter_is_the_orthogonal_projector_on_the_band():
     noise = rng.standard_normal((3, v.shape[0]))
     out = so.filter_apply(Fm, X + 1e-3 * noise) - X
     assert np.linalg.norm(out) < 0.5 * np.linalg.norm(1e-3 * noise)     # ~ sqrt(81 / 642) of the noise survives
+
+
+def test_s5_mean_curvature_paraboloid_fit():
+    """Eqs. 28-29.  (i) A fan of five vertices placed exactly on z = B (x^2 + y^2) around a vertex (by
+    symmetry its Eq.-17 normal is the z axis) returns H = -2 B to rounding.  (ii) The paper's own figure: "for a good
+    quality mesh (N_d > 600) the relative errors in the mean curvature ... do not exceed 1%": icospheres of
+    642 and 2562 vertices, radius R, H = 1/R."""
+    Bq = 0.37                                                          # axisymmetric paraboloid z = Bq (x^2 + y^2): H = -2 Bq
+    ang = 2 * np.pi * np.arange(5) / 5 + 0.3
+    ringp = np.stack([0.1 * np.cos(ang), 0.1 * np.sin(ang), Bq * 0.01 * np.ones(5)], axis=1)
+    Vf = np.vstack([np.zeros((1, 3)), ringp])
+    Ff = np.array([[0, 1 + i, 1 + (i + 1) % 5] for i in range(5)])      # a fan: by symmetry the vertex normal is the z axis
+    Hf = so.mean_curvature(Vf, Ff)
+    assert abs(Hf[0] - (-2 * Bq)) < 1e-12
+    for lvl, R in ((3, 1.0), (4, 2.5)):
+        v, f = bi.icosphere(lvl)
+        H = so.mean_curvature(R * v + np.array([0.3, -0.2, 0.1]), f)
+        assert np.all(np.isfinite(H))
+        assert np.max(np.abs(H * R - 1.0)) < 1e-2, np.max(np.abs(H * R - 1.0))
+    # the in-plane frame does not matter: a rotated copy of the mesh gives the same curvatures
+    v, f = bi.icosphere(2)
+    th, ph = _angles(v)
+    from bem_inputs.sph import real_sph_harm
+    V = (1.0 + 0.2 * real_sph_harm(3, 2, th, ph))[:, None] * v
+    c, s = np.cos(0.7), np.sin(0.7)
+    Rm = np.array([[c, -s, 0], [s, c, 0], [0, 0, 1.0]]) @ np.array([[1, 0, 0], [0, c, -s], [0, s, c]])
+    assert np.max(np.abs(so.mean_curvature(V, f) - so.mean_curvature(V @ Rm.T, f))) < 1e-10
