@@ -226,6 +226,15 @@ void bem_destroy(bem_ctx *ctx);
 bem_status bem_surface_velocity(bem_ctx *ctx, const double *phi, const double *q, double *v, double *normals_out,
                                 double *areas_out);
 
+/* bem_surface_curvature -- mean curvature H_j at every vertex by the fitted paraboloid (Eqs. 28-29):
+ * in the frame centred at r_j whose z axis is n_j (Eq. 17), the paraboloid z = B1 x + B2 y + B3 x^2 + B4 x y + B5 y^2
+ * through FIVE neighbours of the vertex (5 x 5 linear system, Eq. 28), H_j = -B3 - B5 (Eq. 29): 1/R on a sphere whose
+ * normal points out of the bubble.  The paper does not say which five of the neighbours are used: they are the first
+ * five distinct vertices met when walking the triangles that hold vertex j in mesh order (triangle index, then corner),
+ * taking of each triangle its two other vertices in cyclic order.  NaN where a vertex has fewer than five neighbours
+ * or the system is singular.  H: [n_vertices], host or device. */
+bem_status bem_surface_curvature(bem_ctx *ctx, double *H);
+
 /* Shape filter of bandwidth p_f (Eqs. 34-43): every bubble surface is a map of the unit sphere, the
  * mesh points keep their spherical angles (theta_i, phi_i) for all times, and a surface function sampled at them is
  * replaced by its least-squares fit with the spherical harmonics of degree n < p_f,

@@ -31,7 +31,7 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
 # every symbol include/bem.h declares
 EXPORTS = ["bem_create", "bem_create_points", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
            "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy",
-           "bem_surface_velocity", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy"]
+           "bem_surface_velocity", "bem_surface_curvature", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy"]
 
 
 class BemError(RuntimeError):
@@ -70,6 +70,7 @@ def load_library() -> ctypes.CDLL:
     lib.bem_destroy.argtypes = [vp]
     lib.bem_destroy.restype = None
     lib.bem_surface_velocity.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.bem_surface_curvature.argtypes = [vp, vp]
     lib.bem_filter_create.argtypes = [vp, vp, i64, i32, ctypes.POINTER(vp)]
     lib.bem_filter_apply.argtypes = [vp, vp, i64, vp, vp]
     lib.bem_filter_last_error.argtypes = [vp]
@@ -186,6 +187,11 @@ class Bem:
         """v = n q + v_t (Eqs. 22-27), vertex normals and areas (Eq. 17); outputs may be None (at least one given)."""
         self._check(self._lib.bem_surface_velocity(self._ctx, _ptr(phi), _ptr(q), _ptr(v), _ptr(normals_out), _ptr(areas_out)))
         return v
+
+    def bem_surface_curvature(self, H):
+        """Mean curvature by the fitted paraboloid (Eqs. 28-29); H: [n_vertices] output."""
+        self._check(self._lib.bem_surface_curvature(self._ctx, _ptr(H)))
+        return H
 
     def bem_destroy(self):
         if self._ctx:

@@ -84,6 +84,69 @@ __global__ void surface_velocity_kernel(const double *__restrict__ V, const int3
     }
 }
 
+// ------------------------------------------------------------------ Eqs. 28-29: mean curvature by the fitted paraboloid
+// One thread per vertex.  The five neighbours are the first five distinct vertices met when walking the triangles of the
+// vertex in mesh order, taking of each its two other vertices in cyclic order (reading R32).  Frame: z = n_j of
+// Eq. 17, x and y any orthonormal pair (H = -B3 - B5 does not depend on it).  The 5 x 5 system of Eq. 28 is solved by
+// Gaussian elimination with partial pivoting (the paper uses Cramer's rule: the same solution).
+__global__ void surface_curvature_kernel(const double *__restrict__ V, const int32_t *__restrict__ F, const int32_t *__restrict__ begin,
+                                         const uint32_t *__restrict__ corner, int64_t N, double *__restrict__ H)
+{
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    double mx = 0.0, my = 0.0, mz = 0.0;
+    int ring[5], nr = 0;
+    for (int i = begin[j]; i < begin[j + 1]; ++i) {
+        const uint32_t c = corner[i];
+        const int64_t k = c / 3;
+        const int a = (int)(c - 3 * k);
+        const int v1 = F[3 * k], v2 = F[3 * k + 1], v3 = F[3 * k + 2];
+        const double x1 = V[3 * (int64_t)v1], y1 = V[3 * (int64_t)v1 + 1], z1 = V[3 * (int64_t)v1 + 2];
+        const double ax = V[3 * (int64_t)v2] - x1, ay = V[3 * (int64_t)v2 + 1] - y1, az = V[3 * (int64_t)v2 + 2] - z1;
+        const double bx = V[3 * (int64_t)v3] - x1, by = V[3 * (int64_t)v3 + 1] - y1, bz = V[3 * (int64_t)v3 + 2] - z1;
+        mx += 0.5 * (ay * bz - az * by); my += 0.5 * (az * bx - ax * bz); mz += 0.5 * (ax * by - ay * bx);
+        const int cand[2] = {F[3 * k + (a + 1) % 3], F[3 * k + (a + 2) % 3]};
+        for (int t = 0; t < 2; ++t) {
+            bool seen = false;
+            for (int r = 0; r < nr; ++r) seen = seen || ring[r] == cand[t];
+            if (!seen && nr < 5) ring[nr++] = cand[t];
+        }
+    }
+    const double nan = __longlong_as_double(0x7ff8000000000000ll);
+    if (nr < 5) { H[j] = nan; return; }
+    const double im = 1.0 / sqrt(mx * mx + my * my + mz * mz);
+    const double zx = mx * im, zy = my * im, zz = mz * im;
+    double ex, ey, ez;                                                 // e_x = normalised z x a, a = a coordinate axis away from z
+    if (fabs(zx) < 0.9) { ex = 0.0; ey = zz; ez = -zy; } else { ex = -zz; ey = 0.0; ez = zx; }
+    const double ie = 1.0 / sqrt(ex * ex + ey * ey + ez * ez);
+    ex *= ie; ey *= ie; ez *= ie;
+    const double fx = zy * ez - zz * ey, fy = zz * ex - zx * ez, fz = zx * ey - zy * ex;      // e_y = z x e_x
+    double A[5][6];
+    const double px = V[3 * j], py = V[3 * j + 1], pz = V[3 * j + 2];
+    for (int l = 0; l < 5; ++l) {
+        const double dx = V[3 * (int64_t)ring[l]] - px, dy = V[3 * (int64_t)ring[l] + 1] - py, dz = V[3 * (int64_t)ring[l] + 2] - pz;
+        const double x = dx * ex + dy * ey + dz * ez, y = dx * fx + dy * fy + dz * fz, z = dx * zx + dy * zy + dz * zz;
+        A[l][0] = x; A[l][1] = y; A[l][2] = x * x; A[l][3] = x * y; A[l][4] = y * y; A[l][5] = z;       // Eq. 28
+    }
+    for (int col = 0; col < 5; ++col) {
+        int piv = col;
+        for (int r = col + 1; r < 5; ++r) if (fabs(A[r][col]) > fabs(A[piv][col])) piv = r;
+        if (A[piv][col] == 0.0) { H[j] = nan; return; }
+        for (int cc = 0; cc < 6; ++cc) { const double t = A[col][cc]; A[col][cc] = A[piv][cc]; A[piv][cc] = t; }
+        for (int r = col + 1; r < 5; ++r) {
+            const double f = A[r][col] / A[col][col];
+            for (int cc = col; cc < 6; ++cc) A[r][cc] -= f * A[col][cc];
+        }
+    }
+    double B[5];
+    for (int r = 4; r >= 0; --r) {
+        double sum = A[r][5];
+        for (int cc = r + 1; cc < 5; ++cc) sum -= A[r][cc] * B[cc];
+        B[r] = sum / A[r][r];
+    }
+    H[j] = -B[2] - B[4];                                               // Eq. 29
+}
+
 // ------------------------------------------------------------------ shape filter
 }  // namespace bem
 
@@ -264,6 +327,31 @@ bem_status bem_surface_velocity(bem_ctx *c, const double *phi, const double *q, 
         if (pn != normals_out) { CUDA_TRY(cudaMemcpyAsync(normals_out, pn, 3 * N * sizeof(double), cudaMemcpyDeviceToHost, s)); sync = true; }
         if (pa != areas_out) { CUDA_TRY(cudaMemcpyAsync(areas_out, pa, N * sizeof(double), cudaMemcpyDeviceToHost, s)); sync = true; }
         if (sync || dphi.p || dq.p) CUDA_TRY(cudaStreamSynchronize(s));
+        return BEM_OK;
+    } catch (const Error &e) {
+        c->err = e.what();
+        cudaGetLastError();
+        return e.status;
+    }
+}
+
+bem_status bem_surface_curvature(bem_ctx *c, double *H)
+{
+    if (!c || !H) return BEM_ERR_INVALID_ARG;
+    if (c->quadrature == 2 || c->T == 0) { c->err = "bem_surface_curvature: the context holds a point cloud, not a mesh"; return BEM_ERR_INVALID_ARG; }
+    try {
+        CUDA_TRY(cudaSetDevice(c->device));
+        build_vertex_corners(c);
+        const int64_t N = c->N;
+        dvec<double> dh;
+        double *ph = H;
+        if (!is_device_ptr(H)) { dh.alloc(N); ph = dh.get(); }
+        surface_curvature_kernel<<<cdiv(N, 128), 128, 0, c->stream>>>(c->V.get(), c->F.get(), c->vc_begin.get(), c->vc_corner.get(), N, ph);
+        KERNEL_CHECK();
+        if (ph != H) {
+            CUDA_TRY(cudaMemcpyAsync(H, ph, N * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            CUDA_TRY(cudaStreamSynchronize(c->stream));
+        }
         return BEM_OK;
     } catch (const Error &e) {
         c->err = e.what();
