@@ -373,20 +373,30 @@ def run_gpu(args):
                           filter_note="xhat = G (G^+ x) on x, y, z, phi of every bubble: 4 p_f^2 N_d flop per column; the paper's dense F x would be 2 N_d^2")
             flt.bem_filter_destroy()
 
+    # bem_solve: config 4 asks for exactly 30 iterations at tol 1e-6 (BASELINE.json), config 5 for a solve to tol 1e-6;
+    # --solve-iters -1 (default) = 30, or 400 on config 5 (it converges in ~220 / ~150 iterations)
     solve = None
-    if args.solve_iters > 0 and not cloud:
+    max_it = args.solve_iters if args.solve_iters >= 0 else (400 if args.config == 5 else 30)
+    if max_it > 0 and not cloud:
         solve = {}
-        for name, pre in (("unpreconditioned (paper)", 0), ("diagonal S_ii (option precond)", 1)):
+        runs = [("unpreconditioned (paper)", 0, 0), ("diagonal S_ii (option precond)", 1, 0)]
+        if not args.direct and not f32:
+            runs.append(("diagonal S_ii, fp32 pairs (options precond, p2p_precision)", 1, 1))
+        for name, pre, prec in runs:
             ctx.bem_set_option("precond", pre)
+            if not args.direct:
+                ctx.bem_set_option("p2p_precision", 1 if (prec or f32) else 0)
             qs = torch.zeros_like(qd)
             torch.cuda.synchronize()
             t0 = time.perf_counter()
-            st, it, rr = ctx.bem_solve(pd, qs, tol=args.solve_tol, max_iter=args.solve_iters)
+            st, it, rr = ctx.bem_solve(pd, qs, tol=args.solve_tol, max_iter=max_it)
             torch.cuda.synchronize()
             ms_s = (time.perf_counter() - t0) * 1e3
-            solve[name] = dict(ms=ms_s, iterations=it, relres=rr, tol=args.solve_tol, max_iter=args.solve_iters,
+            solve[name] = dict(ms=ms_s, iterations=it, relres=rr, tol=args.solve_tol, max_iter=max_it,
                                status=bem.STATUS_NAMES[st], ms_per_iteration=ms_s / max(it, 1))
         ctx.bem_set_option("precond", 0)
+        if not args.direct:
+            ctx.bem_set_option("p2p_precision", 1 if f32 else 0)
 
     line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
                 higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64 (near-field pairs f32)" if f32 else "f64", data="synthetic",
@@ -428,7 +438,7 @@ def main():
                     help="leaf-level far pairs with nt x ns <= this are summed directly instead of translated (default: library cost model; 0: off)")
     ap.add_argument("--p2p-ctas", type=int, default=0, help="fp32 near field: CTAs per SM of its persistent grid (0: library default)")
     ap.add_argument("--reduce-ctas", type=int, default=0, help="CTAs per SM of the persistent row-sum passes (0: library cost model)")
-    ap.add_argument("--solve-iters", type=int, default=30, help="also run bem_solve with this max_iter (0: skip)")
+    ap.add_argument("--solve-iters", type=int, default=-1, help="also run bem_solve with this max_iter (0: skip; -1: 30, or 400 = to convergence on config 5)")
     ap.add_argument("--solve-tol", type=float, default=1e-6)
     ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU time budget of one oracle sample")
     args = ap.parse_args()
