@@ -408,3 +408,42 @@ def test_direct_pairs_thresholds(n, nb, prec):
         assert res[d][0] <= TOL_FULL[c["p"]]
     assert res[0][1] > res[-1][1] > res[10 ** 9][1] and res[0][2] < res[-1][2] < res[10 ** 9][2]
     assert res[10 ** 9][0] <= res[0][0] * 1.05
+
+
+@pytest.mark.parametrize("quad", [0, 1])
+def test_options_combine_on_v1_and_g3(quad):
+    """fp32 pairs and direct far pairs with both quadratures: V1 has coincident source and target (j = i),
+    which the fp32 kernel and the all-direct lists must skip as the fp64 kernel does."""
+    c = cfg(1)
+    rows = np.arange(c["V"].shape[0], dtype=np.int64)
+    yo = oracle_rows(c, rows, quad)
+    base = None
+    for opts in (dict(), dict(direct_pairs=10 ** 9), dict(p2p_precision=1), dict(p2p_precision=1, direct_pairs=10 ** 9)):
+        ctx = _ctx(c, quad=quad, p=12, lmax=3, **opts)
+        y = _apply(ctx, c["q"], c["phi"])
+        ctx.bem_destroy()
+        e = _rel(y, yo)
+        print(f"quad {quad} {opts}: {e:.2e}")
+        assert e <= 1e-5
+        base = e if base is None else base
+        assert e <= 1.5 * base + 2e-6
+
+
+def test_point_cloud_options_and_coincident_points():
+    """Point clouds where sources and targets are the same points (r = 0 pairs are skipped) with fp32 pairs and with
+    every leaf-level far pair summed directly."""
+    pts, m01, rows = _cloud(30000, 21)
+    m = 2.0 * m01 - 1.0
+    yo = oracle.monopole_sum(pts, m, pts[rows])
+    for opts in (dict(), dict(p2p_precision=1), dict(direct_pairs=10 ** 9), dict(p2p_precision=1, direct_pairs=10 ** 9)):
+        ctx = _bem().bem_create_points(pts, pts)
+        for k, v in opts.items():
+            ctx.bem_set_option(k, v)
+        ctx.bem_setup(12, 64, 2.5)
+        y = np.full(len(pts), np.nan)
+        ctx.bem_apply(m, None, y)
+        ctx.bem_destroy()
+        assert np.isfinite(y).all()
+        e = _rel(y[rows], yo)
+        print(opts, f"{e:.2e}")
+        assert e <= 1e-5
