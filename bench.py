@@ -40,8 +40,8 @@ UNIT = "ms"
 # FMA lanes per SM per clock x 2 flop x 1.965 GHz (clocks.max.sm)
 FP64_NOMINAL_GFLOPS = 148 * 64 * 2 * 1.965
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels on config 5, from the committed
-# ncu --set full capture (profiles/r1_05_launches_and_full_capture.md); None for workloads that were not captured
-NCU_TRAFFIC = {"p2p_leaf": 1.347e9, "translate_dmma": 7.204e9}      # config 5, l_max 6, p 12: P2P launch; M2L tiles of level 6
+# ncu --set full capture (profiles/r1_06_launches_and_full_capture.md); None for workloads that were not captured
+NCU_TRAFFIC = {"p2p_leaf": 1.351e9, "translate_dmma": 7.205e9}      # config 5, l_max 6, p 12: P2P launch; M2L tiles of level 6
 
 
 def workload_name(c):
