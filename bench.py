@@ -57,7 +57,22 @@ def cloud_config(n, seed=190501341 + 6):
                 cfg=6, cloud=True, name=f"cfg6: {n:,} uniform random monopoles in the unit cube (paper Tables 1-2)")
 
 
+def lattice_config(nb, seed=190501341 + 7):
+    """Config 7 (not in BASELINE.json): the paper's own scaling family and the workload of its Table 3 -- nb^3 equal bubbles
+    (icosphere L3, 642 vertices, a0 = 1) on a regular grid with centre spacing 4 a0 (PAPER.md:568-574, 596-606);
+    nb = 12 -> N = 1,109,376, nb = 16 -> N = 2,629,632.  q, phi ~ U(-1, 1)."""
+    from bem_inputs.meshes import lattice_cluster, icosphere
+    V, F, bid = lattice_cluster(3, nb, 4.0, 1.0)
+    rng = np.random.default_rng(seed)
+    N = V.shape[0]
+    return dict(V=np.ascontiguousarray(V), F=np.ascontiguousarray(F, dtype=np.int32), bubble_id=bid, q=rng.uniform(-1, 1, N),
+                phi=rng.uniform(-1, 1, N), p=12, leaf_size=256, eta=2.5, cfg=7, template=icosphere(3)[0],
+                name=f"cfg7: {nb}x{nb}x{nb} regular cluster, spacing 4 a0, icosphere L3, {N:,} nodes (paper Table 3 family)")
+
+
 def get_config(args):
+    if args.config == 7:
+        return lattice_config(args.lattice_nb)
     return cloud_config(args.cloud_points) if args.config == 6 else make_config(args.config)
 
 
@@ -355,7 +370,12 @@ def run_gpu(args):
         ctx.bem_surface_velocity(pd, qd, vd)
         torch.cuda.synchronize()
         sv_ms = timed(lambda: ctx.bem_surface_velocity(pd, qd, vd), args.steps) / args.steps
-        extras = dict(surface_velocity_ms=sv_ms, surface_velocity_note="Eq. 17 + Eqs. 22-27, one thread per vertex")
+        hd = torch.empty(N, dtype=torch.float64, device="cuda")
+        ctx.bem_surface_curvature(hd)
+        torch.cuda.synchronize()
+        cv_ms = timed(lambda: ctx.bem_surface_curvature(hd), args.steps) / args.steps
+        extras = dict(surface_velocity_ms=sv_ms, surface_curvature_ms=cv_ms,
+                      surface_note="normals, areas, velocity (Eq. 17, Eqs. 22-27) and curvature (Eqs. 28-29), one thread per vertex")
         tmpl = c.get("template")
         if tmpl is not None and 81 < tmpl.shape[0] <= 2600:         # all bubbles share the angles of one template mesh
             th = np.arccos(np.clip(tmpl[:, 2], -1, 1)); ph = np.arctan2(tmpl[:, 1], tmpl[:, 0])
@@ -426,8 +446,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: 2.57M nodes); 6 = point cloud (paper Tables 1-2)")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config 1..5 (default 5: 2.57M nodes); 6 = point cloud (paper Tables 1-2); 7 = regular nb^3 cluster (paper Table 3)")
     ap.add_argument("--cloud-points", type=int, default=1048576, help="config 6: number of points")
+    ap.add_argument("--lattice-nb", type=int, default=16, help="config 7: bubbles per edge of the regular cluster (paper: 1..16)")
     ap.add_argument("--p", type=int, default=0)
     ap.add_argument("--leaf-size", type=int, default=0)
     ap.add_argument("--lmax", type=int, default=0)

@@ -128,6 +128,19 @@ void mark(bem_ctx *c, int cls)
     CUDA_TRY(cudaEventRecord(c->ev[c->ev_n++], c->stream));
 }
 
+// CTAs per SM of the persistent side-stream sums: enough for them to end just before the pair kernel does.  Model: fp64
+// pairs at 700 Gpairs/s, fp32 pairs at 1400 (with 4 CTAs per SM of the pair kernel resident, 6 CTAs of the sums still
+// fit); the sums at 4 TB/s with >= 16 CTAs per SM, in proportion below that (measured on configs 4 and 5).
+static int reduce_ctas_for(const bem_ctx *c)
+{
+    if (c->reduce_ctas > 0) return c->reduce_ctas;
+    const bool f32 = c->p2p_precision == 1;
+    const double t_p2p = (double)c->p2p_pairs / (f32 ? 1400e9 : 700e9);
+    const double t_sum = (double)c->m2l_pairs * 8.0 * c->nst / 4e12;
+    const int k = (int)std::ceil(16.0 * 1.3 * t_sum / std::max(t_p2p, 1e-9));
+    return std::max(3, std::min(k, f32 ? 6 : 16));
+}
+
 void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
 {
     c->ev_n = 0;
@@ -161,7 +174,7 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
             for (int l = 2; l <= lmax; ++l) launch_stage_gemm(c, c->m2l[l], TILES_ALL, main);
             CUDA_TRY(cudaEventRecord(c->ev_fork, main));
             CUDA_TRY(cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-            for (int l = lmax; l >= 2; --l) launch_stage_reduce(c, c->m2l[l], c->side, c->reduce_ctas_eff);
+            for (int l = lmax; l >= 2; --l) launch_stage_reduce(c, c->m2l[l], c->side, reduce_ctas_for(c));
             CUDA_TRY(cudaEventRecord(c->ev_join, c->side));
             // fp32 pairs: a persistent grid of a few CTAs per SM (80 registers each) so that the CTAs of the sums still fit
             if (c->p2p_precision == 1) launch_p2p_leaves_f32(c, main, c->p2p_ctas > 0 ? c->p2p_ctas : 4, 0, c->tb.nbox[lmax], 0);
@@ -269,15 +282,6 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         c->p2p_counter.alloc(4);                         // [0], [1] fp32 pair kernel, [2] P2M: leaf counters of the persistent grids
         c->src_pos_f.free();
         c->src_str_f.free();
-        {
-            // CTAs per SM of the persistent side-stream sums: enough for them to end just before P2P does.  Model:
-            // P2P at 700 Gpairs/s; the sums at 4 TB/s with >= 16 CTAs per SM, in proportion below that (measured on
-            // configs 4 and 5: the best values were 12 and 4).
-            const double t_p2p = (double)c->p2p_pairs / 700e9;
-            const double t_sum = (double)c->m2l_pairs * 8.0 * c->nst / 4e12;
-            int k = (int)std::ceil(16.0 * 1.3 * t_sum / std::max(t_p2p, 1e-9));
-            c->reduce_ctas_eff = c->reduce_ctas > 0 ? c->reduce_ctas : std::max(3, std::min(k, 16));
-        }
         int launches = 2 /*lift, p2m*/ + 3 /*l2p, p2p, spmv*/;
         for (int l = lmax - 1; l >= 2; --l) launches += 2;
         for (int l = 2; l <= lmax; ++l) launches += l > 2 ? 4 : 2;     // M2L tiles + sum; L2L tiles + sum
@@ -472,7 +476,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
     else if (!strcmp(key, "lmax")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->force_lmax = v; c->ready = false; }
     else if (!strcmp(key, "timing")) { c->timing = v != 0; }
-    else if (!strcmp(key, "reduce_ctas")) { if (v < 0 || v > 32) return BEM_ERR_INVALID_ARG; c->reduce_ctas = v; c->ready = false; }
+    else if (!strcmp(key, "reduce_ctas")) { if (v < 0 || v > 32) return BEM_ERR_INVALID_ARG; c->reduce_ctas = v; }
     else if (!strcmp(key, "m2l_rows16")) { c->m2l_rows16 = v != 0; }
     else if (!strcmp(key, "precond")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->precond = v; }
     else if (!strcmp(key, "p2p_precision")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->p2p_precision = v; }

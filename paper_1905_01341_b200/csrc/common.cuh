@@ -148,7 +148,6 @@ struct bem_ctx {
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
     int precond = 0;                // bem_solve: 0 = unpreconditioned (the paper), 1 = right diagonal scaling by S_ii
     int reduce_ctas = 0;            // option "reduce_ctas": CTAs per SM of the persistent side-stream sums, 0 = from the cost model
-    int reduce_ctas_eff = 6;
     int n_sm = 148;
     int m2l_rows16 = 1;             // M2L tiles: 1 = 4 warps x 16 rows (B fragments feed two DMMAs), 0 = 8 warps x 8 rows
     int gemm_path = 0;              // translations: 0 = FP64 tensor path (DMMA) where p <= 16, 1 = plain-FMA tiles
