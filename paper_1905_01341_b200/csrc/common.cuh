@@ -104,7 +104,7 @@ struct BoxSet {                     // the non-empty boxes of one point set on l
 };
 
 // One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
-// executed as (tiles of a dense GEMM per matrix) -> scratch rows -> fixed-order row sums.
+// executed as (tiles of a dense GEMM per matrix) -> scratch rows in target-major order -> fixed-order row sums.
 struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split)
 constexpr int TILES_ALL = 0, TILES_SPLIT = 1, TILES_DENSE = 2;
 struct Stage {
@@ -115,7 +115,8 @@ struct Stage {
     bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
     bool accumulate = false;        // the reduce pass adds to the output instead of overwriting it (L2L)
     dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
-    dvec<int32_t> pos;              // [npairs] scratch row of pair k (target-major order)
+    dvec<int32_t> krow;             // [npairs] target-major index k of the pair in tile row r: its scratch row (the rows of a target are
+                                    // contiguous in scratch, so the row sums stream them; the tiles scatter whole 8 nst-byte rows)
     dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order): the reduce pass rotates back by its azimuth
     dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
     dvec<Tile> tiles;

@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(GEMM_THREADS)
 translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
                const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-               int nst, double *__restrict__ scratch)
+               int nst, const int32_t *__restrict__ krow, double *__restrict__ scratch)
 {
     __shared__ double As[GEMM_KC][GEMM_TM + 4];
     __shared__ double Bs[GEMM_KC][GEMM_TN];
@@ -175,7 +175,7 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
     for (int i = 0; i < 4; ++i) {
         const int r = ty * 4 + i;
         if (r >= tile.nrows) continue;
-        double *out = scratch + (size_t)(tile.row0 + r) * nst + n0;
+        double *out = scratch + (size_t)krow[tile.row0 + r] * nst + n0;
 #pragma unroll
         for (int j = 0; j < 4; ++j)
             if (n0 + tx + 16 * j < nst) out[tx + 16 * j] = acc[i][j];
@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(DM_THREADS)
 translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
                const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-               double *__restrict__ scratch)
+               const int32_t *__restrict__ krow, double *__restrict__ scratch)
 {
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S] (dense tiles: [2][2 NRE][DM_S_DENSE])
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
@@ -321,7 +321,7 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
             a[2 * j + 1] = v.y;
         }
     }
-    double *orow = scratch + (size_t)(tile.row0 + row) * NST + 2 * lk;
+    double *orow = scratch + (size_t)(rvalid ? krow[tile.row0 + row] : 0) * NST + 2 * lk;
 
     for (int ch = 0; ch < nchunks; ++ch) {
         double *cur = (ch & 1) ? Bs1 : Bs0;
@@ -350,7 +350,7 @@ template <int KSH>
 __global__ void __launch_bounds__(DM_THREADS, (KSH <= 20 ? 3 : 2))
 translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                      const double *__restrict__ Mexp, const double *__restrict__ mats,
-                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, double *__restrict__ scratch)
+                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
 {
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
@@ -380,7 +380,7 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
     for (int k = threadIdx.x; k < NRE; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
     const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
     const double2 *ap = reinterpret_cast<const double2 *>(Mexp + (size_t)(arow < 0 ? 0 : arow) * NST) + lk;
-    double *orow = scratch + (size_t)(tile.row0 + row) * NST + 2 * lk;
+    double *orow = scratch + (size_t)(rvalid ? krow[tile.row0 + row] : 0) * NST + 2 * lk;
     double a[KSH];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
@@ -437,7 +437,7 @@ template <int KSH>
 __global__ void __launch_bounds__(DM16_THREADS, 3)
 translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                        const double *__restrict__ Mexp, const double *__restrict__ mats,
-                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, double *__restrict__ scratch)
+                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
 {
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];
@@ -468,8 +468,8 @@ translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict
     const int ar0 = v0 ? src_sorted[tile.row0 + row0] : -1, ar1 = v1 ? src_sorted[tile.row0 + row1] : -1;
     const double2 *ap0 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar0 < 0 ? 0 : ar0) * NST) + lk;
     const double2 *ap1 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar1 < 0 ? 0 : ar1) * NST) + lk;
-    double *o0 = scratch + (size_t)(tile.row0 + row0) * NST + 2 * lk;
-    double *o1 = scratch + (size_t)(tile.row0 + row1) * NST + 2 * lk;
+    double *o0 = scratch + (size_t)(v0 ? krow[tile.row0 + row0] : 0) * NST + 2 * lk;
+    double *o1 = scratch + (size_t)(v1 ? krow[tile.row0 + row1] : 0) * NST + 2 * lk;
     double a0[KSH], a1[KSH];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
@@ -519,22 +519,22 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
     if (which != TILES_DENSE && st.ntiles_split > 0) {
         if (KSH == 20 && c->m2l_rows16)                          // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
             translate_dmma_split16<(KSH == 20 ? KSH : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
-                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->kinfo.get(), c->rot.get(), scratch);
+                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
         else
             translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                    c->mats.get(), c->kinfo.get(), c->rot.get(), scratch);
+                                                                                    c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
     }
     if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
         translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
                                                                                       c->Mexp.get(), c->Lexp.get(), c->mats.get(),
-                                                                                      c->kinfo.get(), c->rot.get(), scratch);
+                                                                                      c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
 }
 
-// out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[pos[k]][:]   (fixed order; a_k = azimuth of
+// out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[k][:]   (fixed order; a_k = azimuth of
 // pair k's matrix, the identity for M2M / L2L pairs).  One CTA per target box, one thread per coefficient (l, m):
 // it reads the real and the imaginary part (nre apart) of every row once and writes both.
 __global__ void __launch_bounds__(160)
-translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ pos, const int32_t *__restrict__ mat_t,
+translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t,
                  const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
                  int nre, int accumulate, int ntgt, double *__restrict__ out)
 {
@@ -547,11 +547,11 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ po
             double sr = 0.0, si = 0.0;
             if (m == 0) {
 #pragma unroll 8
-                for (int k = b; k < e; ++k) sr += scratch[(size_t)pos[k] * nst + cc];
+                for (int k = b; k < e; ++k) sr += scratch[(size_t)k * nst + cc];
             } else {
 #pragma unroll 8
                 for (int k = b; k < e; ++k) {
-                    const double *row = scratch + (size_t)pos[k] * nst + cc;
+                    const double *row = scratch + (size_t)k * nst + cc;
                     double vr = row[0], vi = row[nre];
                     azimuth(__ldg(rot + (size_t)mat_t[k] * ROT_M + m), vr, vi);
                     sr += vr;
@@ -576,7 +576,7 @@ void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stre
     if (c->gemm_path == 1 || pl > 16) {                         // plain-FMA tiles: p > 16, or forced (option "gemm_path")
         dim3 grid(last - first, cdiv(c->nst, GEMM_TN));
         translate_gemm<<<grid, GEMM_THREADS, 0, stream>>>(st.tiles.get() + first, st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, scratch);
+                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, st.krow.get(), scratch);
     }
     else if (pl == 4) launch_dmma<4>(c, st, which, stream, scratch);     // nre / 4 of the layout for pl = 4, 6, .., 16
     else if (pl == 6) launch_dmma<6>(c, st, which, stream, scratch);
@@ -603,7 +603,7 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
         attr_set = true;
     }
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
-        st.ptr.get(), st.pos.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
+        st.ptr.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
         c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : 0, st.ntgt, out);
     KERNEL_CHECK();
 }

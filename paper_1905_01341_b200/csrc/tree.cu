@@ -222,13 +222,13 @@ __global__ void mat_keys(const int32_t *mat, int64_t n, uint64_t *keys, int *his
     keys[k] = (uint64_t)mat[k];
     atomicAdd(&hist[mat[k]], 1);
 }
-__global__ void stage_finish(const uint32_t *order, const int32_t *src, int64_t n, int32_t *src_sorted, int32_t *pos)
+__global__ void stage_finish(const uint32_t *order, const int32_t *src, int64_t n, int32_t *src_sorted, int32_t *krow)
 {
     const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n) return;
     const uint32_t k = order[r];
     src_sorted[r] = src[k];
-    pos[k] = (int32_t)r;
+    krow[r] = (int32_t)k;
 }
 
 constexpr int GEMM_TM = 64;   // rows per GEMM tile (translate.cu uses the same constant)
@@ -238,7 +238,7 @@ static void finish_stage(Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cuda
 {
     const int64_t n = st.npairs;
     st.src_sorted.alloc(n);
-    st.pos.alloc(n);
+    st.krow.alloc(n);
     std::vector<int> h(N_MATS, 0);
     if (n > 0) {
         dvec<uint64_t> keys, ktmp;
@@ -251,7 +251,7 @@ static void finish_stage(Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cuda
         KERNEL_CHECK();
         iota_u32(order.get(), n, s);
         radix_sort_pairs(keys.get(), order.get(), ktmp.get(), otmp.get(), n, 0, 16, s);
-        stage_finish<<<cdiv(n, 256), 256, 0, s>>>(order.get(), src.get(), n, st.src_sorted.get(), st.pos.get());
+        stage_finish<<<cdiv(n, 256), 256, 0, s>>>(order.get(), src.get(), n, st.src_sorted.get(), st.krow.get());
         KERNEL_CHECK();
         CUDA_TRY(cudaMemcpyAsync(h.data(), hist.get(), N_MATS * sizeof(int), cudaMemcpyDeviceToHost, s));
         CUDA_TRY(cudaStreamSynchronize(s));
