@@ -272,3 +272,60 @@ def test_solve_diagonal_preconditioner_same_solution_fewer_iterations():
     print("iterations", res[0][1], res[1][1])
     assert _rel(res[1][0], res[0][0]) <= 1e-5          # cond(S) ~ 1e2-1e3 times the residual tolerance
     assert res[1][1] < res[0][1]
+
+
+def test_non_default_stream_and_option_toggles_between_products():
+    """bem_set_stream with a torch side stream: same bits as on the default stream; p2p_precision, reduce_ctas, p2p_ctas
+    and timing may change between products without a new bem_setup (include/bem.h)."""
+    import torch
+    c = make_config(4, n_bubbles=30)
+    ctx = _bem().bem_create(c["V"], c["F"], c["bubble_id"])
+    ctx.bem_setup(c["p"], c["leaf_size"], c["eta"])
+    qd, pd = torch.tensor(c["q"], device="cuda"), torch.tensor(c["phi"], device="cuda")
+    y0 = torch.empty_like(qd)
+    ctx.bem_apply(qd, pd, y0)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    ctx.bem_set_stream(side.cuda_stream)
+    y1 = torch.empty_like(qd)
+    with torch.cuda.stream(side):
+        ctx.bem_apply(qd, pd, y1)
+    side.synchronize()
+    assert torch.equal(y0, y1)
+    outs = {}
+    for prec in (1, 0, 1):
+        ctx.bem_set_option("p2p_precision", prec)
+        for rc, pc, tm in ((0, 0, 0), (3, 2, 0), (16, 6, 0), (0, 0, 1)):
+            ctx.bem_set_option("reduce_ctas", rc); ctx.bem_set_option("p2p_ctas", pc); ctx.bem_set_option("timing", tm)
+            y = torch.empty_like(qd)
+            with torch.cuda.stream(side):
+                ctx.bem_apply(qd, pd, y)
+            side.synchronize()
+            outs.setdefault(prec, []).append(y.clone())
+    ctx.bem_set_stream(0)
+    ctx.bem_destroy()
+    for prec, ys in outs.items():
+        assert all(torch.equal(ys[0], y) for y in ys)               # launch configuration never changes the bits
+    assert torch.equal(outs[0][0], y0)
+    rel = float(torch.linalg.norm(outs[1][0] - y0) / torch.linalg.norm(y0))
+    assert 0 < rel < 5e-6
+
+
+def test_solve_with_single_precision_pairs_reaches_the_same_solution():
+    c = make_config(4, n_bubbles=20)
+    ctx = _bem().bem_create(c["V"], c["F"], c["bubble_id"])
+    ctx.bem_setup(12, c["leaf_size"], c["eta"])
+    ctx.bem_set_option("precond", 1)
+    N = c["V"].shape[0]
+    sols = []
+    for prec in (0, 1):
+        ctx.bem_set_option("p2p_precision", prec)
+        q = np.zeros(N)
+        st, it, rr = ctx.bem_solve(c["phi"], q, tol=1e-6, max_iter=500)
+        print("p2p_precision", prec, "status", st, "iterations", it, "relres", rr)
+        assert st == 0 and rr <= 1e-6
+        sols.append((q, it))
+    ctx.bem_destroy()
+    (q0, it0), (q1, it1) = sols
+    assert abs(it0 - it1) <= 2
+    assert np.linalg.norm(q1 - q0) / np.linalg.norm(q0) < 1e-3    # cond(S) times (tolerance + the 1e-6 perturbation of the operator)
