@@ -190,7 +190,13 @@ def run_gpu(args):
     V, F = c["V"], c["F"]
     N, T = V.shape[0], F.shape[0]
     p = args.p or c["p"]
+    # bem_apply replays a CUDA graph on any stream but the legacy default one (option "graph"): one launch instead of 20-40,
+    # which pays on the launch-bound small meshes (config 1: 0.104 -> 0.079 ms); on the large configs the product is
+    # kernel-bound and measured 1-3% faster launched kernel by kernel on the default stream.  auto = side stream below 200k nodes
     stream = torch.cuda.current_stream()
+    if args.stream == "side" or (args.stream == "auto" and N < 200000):
+        stream = torch.cuda.Stream()
+        torch.cuda.set_stream(stream)
 
     t0 = time.perf_counter()
     ctx = bem.bem_create_points(V, V) if c.get("cloud") else bem.bem_create(V, F, c["bubble_id"])
@@ -198,6 +204,8 @@ def run_gpu(args):
     ctx.bem_set_option("mode", 1 if args.direct else 0)
     if args.lmax:
         ctx.bem_set_option("lmax", args.lmax)
+    if args.no_graph:
+        ctx.bem_set_option("graph", 0)
     if args.p2p_precision == 32:
         ctx.bem_set_option("p2p_precision", 1)
     if args.direct_pairs is not None:
@@ -425,6 +433,7 @@ def run_gpu(args):
                             n_sources=int(stats["n_sources"]), leaf_size=args.leaf_size or c["leaf_size"], eta=c["eta"],
                             lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]), n_tgt_leaves=int(stats["n_tgt_leaves"]),
                             parallelism="replicas only" if world > 1 else "1 gpu",
+                            launch="CUDA graph replay" if (stream.cuda_stream != 0 and not args.no_graph) else "kernel by kernel",
                             l2="flushed between iterations (512 MB write)" if flush else "working set larger than L2",
                             device_bytes=int(stats["device_bytes"])),
                 e2e=dict(value=e2e, unit=UNIT, h2d_bytes_per_step=(8 if cloud else 16) * N, d2h_bytes_per_step=8 * N),
@@ -455,6 +464,9 @@ def main():
     ap.add_argument("--direct", action="store_true", help="direct-sum mode (configs 1-3)")
     ap.add_argument("--p2p-precision", type=int, default=64, choices=[64, 32],
                     help="near-field pair arithmetic: 64 = fp64 (default, the measured mode), 32 = fp32 pairs with fp64 accumulation (PAPER.md:456-473)")
+    ap.add_argument("--stream", default="auto", choices=["auto", "default", "side"],
+                    help="stream of the products: the legacy default stream, or a side stream (CUDA-graph replay); auto = side below 200k nodes")
+    ap.add_argument("--no-graph", action="store_true", help="launch bem_apply kernel by kernel instead of replaying its CUDA graph")
     ap.add_argument("--direct-pairs", type=int, default=None,
                     help="leaf-level far pairs with nt x ns <= this are summed directly instead of translated (default: library cost model; 0: off)")
     ap.add_argument("--p2p-ctas", type=int, default=0, help="fp32 near field: CTAs per SM of its persistent grid (0: library default)")

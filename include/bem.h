@@ -140,6 +140,10 @@ bem_status bem_create_points(const double *sources, int64_t n_sources, const dou
  *                   join sparsely filled boxes (the balance of A^(dense) and A^(sparse), per pair).
  *                   -1 = 800 (nre / 80)^2 from the measured costs (default), 0 = off (the uniform lists of
  *                   PAPER.md:440).  Direct pairs are exact, so the error can only fall.
+ *   "graph"         1 (default): bem_apply with DEVICE pointers q, phi, y on a stream other than the legacy default stream is
+ *                   captured into a CUDA graph the second time the same (q, phi, y) is asked for and replayed from then
+ *                   on -- one launch instead of 20-40 on the launch-bound small meshes.  Any bem_set_option,
+ *                   bem_set_stream or bem_setup drops the captured graphs.  0: always launch kernel by kernel.
  *   "p2p_ctas"      fp32 near field: CTAs per SM of its persistent grid while the row sums share the SMs
  *                   (1..16; 0 = 4, default).  Tuning only. */
 bem_status bem_set_option(bem_ctx *ctx, const char *key, double value);

@@ -189,8 +189,52 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
     c->ev_valid = c->timing != 0;
 }
 
+static void drop_graphs(bem_ctx *c)
+{
+    for (auto &g : c->graphs) if (g.exec) cudaGraphExecDestroy(g.exec);
+    c->graphs.clear();
+}
+
+// bem_apply with device pointers: replay a captured graph when the same product was asked for before
+static void apply_device_cached(bem_ctx *c, const double *q, const double *phi, double *y)
+{
+    // the legacy default stream cannot be captured; option "timing" records events between the kernels
+    if (!c->use_graph || c->timing || c->stream == nullptr || c->stream == cudaStreamLegacy) { apply_device(c, q, phi, y); return; }
+    for (auto &g : c->graphs) {
+        if (g.q != q || g.phi != phi || g.y != y || g.stream != c->stream) continue;
+        if (g.exec) { CUDA_TRY(cudaGraphLaunch(g.exec, c->stream)); return; }
+        if (c->mode == 0 && c->p2p_precision == 1) ensure_p2p_f32(c);       // allocations stay outside the capture
+        c->has_dipole = phi != nullptr;
+        cudaGraph_t graph = nullptr;
+        CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        try {
+            apply_device(c, q, phi, y);
+        } catch (...) {
+            cudaStreamEndCapture(c->stream, &graph);
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            throw;
+        }
+        CUDA_TRY(cudaStreamEndCapture(c->stream, &graph));
+        cudaGraphExec_t exec = nullptr;
+        const cudaError_t e = cudaGraphInstantiate(&exec, graph, 0);
+        cudaGraphDestroy(graph);
+        CUDA_TRY(e);
+        g.exec = exec;
+        CUDA_TRY(cudaGraphLaunch(g.exec, c->stream));
+        return;
+    }
+    if (c->graphs.size() >= 8) {                                             // keep the cache small: drop the oldest entry
+        if (c->graphs.front().exec) cudaGraphExecDestroy(c->graphs.front().exec);
+        c->graphs.erase(c->graphs.begin());
+    }
+    c->graphs.push_back({q, phi, y, c->stream, 1, nullptr});
+    apply_device(c, q, phi, y);
+}
+
 static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
 {
+    drop_graphs(c);
     cudaStream_t s = c->stream;
     const auto t0 = std::chrono::steady_clock::now();
     c->ready = false;
@@ -212,11 +256,11 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         bb.alloc(6);
         bbox3(c->V.get(), N, bb.get(), s);
         double hb[6];
-        CUDA_TRY(cudaMemcpy(hb, bb.get(), sizeof hb, cudaMemcpyDeviceToHost));
+        d2h_sync(hb, bb.get(), sizeof hb, s);
         if (c->quadrature == 2) {                           // the cube holds sources and targets
             double hs[6];
             bbox3(c->P.get(), c->np, bb.get(), s);
-            CUDA_TRY(cudaMemcpy(hs, bb.get(), sizeof hs, cudaMemcpyDeviceToHost));
+            d2h_sync(hs, bb.get(), sizeof hs, s);
             for (int d = 0; d < 3; ++d) { hb[d] = std::min(hb[d], hs[d]); hb[3 + d] = std::max(hb[3 + d], hs[3 + d]); }
         }
         double side = 0;
@@ -470,6 +514,8 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
 {
     if (!c || !key) return BEM_ERR_INVALID_ARG;
     const int v = (int)value;
+    drop_graphs(c);
+    if (!strcmp(key, "graph")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->use_graph = v; return BEM_OK; }
     if (!strcmp(key, "quadrature")) { if ((v != 0 && v != 1) || c->quadrature == 2) return BEM_ERR_INVALID_ARG; c->quadrature = v; c->ready = false; }
     else if (!strcmp(key, "mode")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->mode = v; c->ready = false; }
     else if (!strcmp(key, "free_term")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->free_term = v; c->ready = false; }
@@ -490,6 +536,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
 bem_status bem_set_stream(bem_ctx *c, void *cuda_stream)
 {
     if (!c) return BEM_ERR_INVALID_ARG;
+    drop_graphs(c);
     c->stream = (cudaStream_t)cuda_stream;
     return BEM_OK;
 }
@@ -519,7 +566,8 @@ bem_status bem_apply(bem_ctx *c, const double *q, const double *phi, double *y)
         if (hq) { if (!c->stage_q.p) c->stage_q.alloc(qbytes / sizeof(double)); CUDA_TRY(cudaMemcpyAsync(c->stage_q.get(), q, qbytes, cudaMemcpyHostToDevice, c->stream)); dq = c->stage_q.get(); }
         if (hp) { if (!c->stage_phi.p) c->stage_phi.alloc(c->N); CUDA_TRY(cudaMemcpyAsync(c->stage_phi.get(), phi, bytes, cudaMemcpyHostToDevice, c->stream)); dp = c->stage_phi.get(); }
         if (hy) { if (!c->stage_y.p) c->stage_y.alloc(c->N); dy = c->stage_y.get(); }
-        apply_device(c, dq, dp, dy);
+        if (hq || hp || hy) apply_device(c, dq, dp, dy);
+        else apply_device_cached(c, dq, dp, dy);
         if (hy) CUDA_TRY(cudaMemcpyAsync(y, dy, bytes, cudaMemcpyDeviceToHost, c->stream));
         if (hq || hp || hy) CUDA_TRY(cudaStreamSynchronize(c->stream));
     });
@@ -599,6 +647,7 @@ void bem_destroy(bem_ctx *c)
 {
     if (!c) return;
     cudaSetDevice(c->device);
+    drop_graphs(c);
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);

@@ -60,6 +60,14 @@ struct dvec {
 // enough to serialise the two (measured: config 5, fp32 pairs beside the sums, 21.3 -> 26.5 ms).
 constexpr int CORUN_CARVEOUT = 14;     // 32 KB of 228
 
+// device -> host copy of a result of the work enqueued on stream s.  (A plain cudaMemcpy runs on the legacy default stream,
+// which does not wait for a NON-BLOCKING user stream: bem_setup on such a stream would read counters before their kernels end.)
+inline void d2h_sync(void *dst, const void *src, size_t bytes, cudaStream_t s)
+{
+    CUDA_TRY(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+}
+
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 }  // namespace bem
 struct bem_ctx;
@@ -217,6 +225,13 @@ struct bem_ctx {
 
     bem::dvec<double> cfree;        // [N] free term c_i of bem_solve
     bool have_cfree = false;
+
+    // CUDA graphs of bem_apply with device pointers (option "graph"): a product with the same (q, phi, y, stream) is
+    // captured the second time it is asked for and replayed from then on (the launch-bound small meshes: 20-40 launches of
+    // a few microseconds each); any bem_set_option / bem_setup / bem_set_stream drops the cache
+    struct GraphEntry { const double *q, *phi; double *y; cudaStream_t stream; int seen; cudaGraphExec_t exec; };
+    std::vector<GraphEntry> graphs;
+    int use_graph = 1;
 
     // staging for host-pointer arguments
     bem::dvec<double> stage_q, stage_phi, stage_y;

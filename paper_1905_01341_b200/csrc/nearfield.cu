@@ -275,7 +275,7 @@ void build_correction(bem_ctx *c)
     bb.alloc(6);
     bbox3(c->V.get(), N, bb.get(), s);
     double hb[6];
-    CUDA_TRY(cudaMemcpy(hb, bb.get(), sizeof hb, cudaMemcpyDeviceToHost));
+    d2h_sync(hb, bb.get(), sizeof hb, s);
     Grid g;
     double ext = 0;
     for (int d = 0; d < 3; ++d) { g.mn[d] = hb[d]; ext = std::max(ext, hb[3 + d] - hb[d]); }
@@ -305,7 +305,7 @@ void build_correction(bem_ctx *c)
     KERNEL_CHECK();
     scan_exclusive_i64(cnt.get(), nptr.get(), N, s);
     int64_t nnear = 0;
-    CUDA_TRY(cudaMemcpy(&nnear, nptr.get() + N, sizeof(int64_t), cudaMemcpyDeviceToHost));
+    d2h_sync(&nnear, nptr.get() + N, sizeof(int64_t), s);
     c->near_tris = nnear;
     dvec<int32_t> near;
     near.alloc(nnear);
@@ -316,7 +316,7 @@ void build_correction(bem_ctx *c)
     KERNEL_CHECK();
     c->rowptr.alloc(N + 1);
     scan_exclusive_i64(cnt.get(), c->rowptr.get(), N, s);
-    CUDA_TRY(cudaMemcpy(&c->nnz, c->rowptr.get() + N, sizeof(int64_t), cudaMemcpyDeviceToHost));
+    d2h_sync(&c->nnz, c->rowptr.get() + N, sizeof(int64_t), s);
     c->col.alloc(c->nnz);
     c->val.alloc(c->nnz);
     c->diagS.alloc(N);

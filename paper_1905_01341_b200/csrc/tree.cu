@@ -58,7 +58,7 @@ static int unique_level(const uint64_t *keys, int64_t n, int shift, dvec<uint64_
     KERNEL_CHECK();
     scan_exclusive_i32(flags.get(), excl.get(), n, s);
     int total = 0;
-    CUDA_TRY(cudaMemcpy(&total, excl.get() + n, sizeof(int), cudaMemcpyDeviceToHost));
+    d2h_sync(&total, excl.get() + n, sizeof(int), s);
     if (expect >= 0 && total != expect) throw Error(BEM_ERR_CUDA, "octree: box count mismatch between histogram and scan");
     ukey.alloc(total);
     ubegin.alloc(total + 1);
@@ -292,7 +292,7 @@ void build_lists(bem_ctx *c)
                                                    tb.begin.get(), sb.begin.get(), pc.get());
     KERNEL_CHECK();
     unsigned long long hp = 0;
-    CUDA_TRY(cudaMemcpy(&hp, pc.get(), sizeof hp, cudaMemcpyDeviceToHost));
+    d2h_sync(&hp, pc.get(), sizeof hp, s);
     c->p2p_pairs = (int64_t)hp;
     c->xdir_pairs = 0;
     c->xdir_ptr.free();
@@ -322,16 +322,16 @@ void build_lists(bem_ctx *c)
         if (dmax > 0) {
             scan_exclusive_i32(xcnt.get(), c->xdir_ptr.get(), nt, s);
             int xt = 0;
-            CUDA_TRY(cudaMemcpy(&xt, c->xdir_ptr.get() + nt, sizeof(int), cudaMemcpyDeviceToHost));
+            d2h_sync(&xt, c->xdir_ptr.get() + nt, sizeof(int), s);
             unsigned long long xp = 0;
-            CUDA_TRY(cudaMemcpy(&xp, pc.get(), sizeof xp, cudaMemcpyDeviceToHost));
+            d2h_sync(&xp, pc.get(), sizeof xp, s);
             c->xdir_pairs = xt;
             c->p2p_pairs += (int64_t)xp;
             c->xdir_src.alloc(xt);
         }
         scan_exclusive_i32(cnt.get(), st.ptr.get(), nt, s);
         int total = 0;
-        CUDA_TRY(cudaMemcpy(&total, st.ptr.get() + nt, sizeof(int), cudaMemcpyDeviceToHost));
+        d2h_sync(&total, st.ptr.get() + nt, sizeof(int), s);
         st.npairs = total;
         dvec<int32_t> src, mat;
         src.alloc(total);

@@ -302,6 +302,37 @@ def test_non_default_stream_and_option_toggles_between_products():
                 ctx.bem_apply(qd, pd, y)
             side.synchronize()
             outs.setdefault(prec, []).append(y.clone())
+    # CUDA graph replay (option graph, default on): the third and later products with the same pointers are one launch
+    ctx.bem_set_option("p2p_precision", 0); ctx.bem_set_option("timing", 0); ctx.bem_set_option("reduce_ctas", 0); ctx.bem_set_option("p2p_ctas", 0)
+    yg = torch.empty_like(qd)
+    for prec in (0, 1):
+        ctx.bem_set_option("p2p_precision", prec)
+        for rep in range(5):
+            yg.fill_(float("nan"))
+            with torch.cuda.stream(side):
+                ctx.bem_apply(qd, pd, yg)
+                ctx.bem_apply(qd, None, y1)                         # a second cached product in between
+            side.synchronize()
+            assert torch.equal(yg, outs[prec][0]), (prec, rep)
+    ctx.bem_set_option("graph", 0)
+    with torch.cuda.stream(side):
+        ctx.bem_apply(qd, pd, yg)
+    side.synchronize()
+    assert torch.equal(yg, outs[1][0])
+    # bem_setup itself on the (non-blocking) side stream: same lists, same bits
+    st0 = ctx.bem_get_stats()
+    ctx2 = _bem().bem_create(c["V"], c["F"], c["bubble_id"])
+    ctx2.bem_set_stream(side.cuda_stream)
+    with torch.cuda.stream(side):
+        ctx2.bem_setup(c["p"], c["leaf_size"], c["eta"])
+        y2 = torch.empty_like(qd)
+        ctx2.bem_apply(qd, pd, y2)
+    side.synchronize()
+    st2 = ctx2.bem_get_stats()
+    for k in ("p2p_pairs", "m2l_pairs", "csr_nnz", "lmax", "n_src_leaves", "n_tgt_leaves"):
+        assert st0[k] == st2[k], k
+    assert torch.equal(y2, y0)
+    ctx2.bem_destroy()
     ctx.bem_set_stream(0)
     ctx.bem_destroy()
     for prec, ys in outs.items():
