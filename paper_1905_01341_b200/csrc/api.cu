@@ -200,6 +200,12 @@ static void apply_device_cached(bem_ctx *c, const double *q, const double *phi, 
 {
     // the legacy default stream cannot be captured; option "timing" records events between the kernels
     if (!c->use_graph || c->timing || c->stream == nullptr || c->stream == cudaStreamLegacy) { apply_device(c, q, phi, y); return; }
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(c->stream, &cap) != cudaSuccess || cap != cudaStreamCaptureStatusNone) {
+        cudaGetLastError();
+        apply_device(c, q, phi, y);                                          // the caller is capturing this stream: become part of ITS graph
+        return;
+    }
     for (auto &g : c->graphs) {
         if (g.q != q || g.phi != phi || g.y != y || g.stream != c->stream) continue;
         if (g.exec) { CUDA_TRY(cudaGraphLaunch(g.exec, c->stream)); return; }

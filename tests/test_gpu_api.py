@@ -360,3 +360,31 @@ def test_solve_with_single_precision_pairs_reaches_the_same_solution():
     (q0, it0), (q1, it1) = sols
     assert abs(it0 - it1) <= 2
     assert np.linalg.norm(q1 - q0) / np.linalg.norm(q0) < 1e-3    # cond(S) times (tolerance + the 1e-6 perturbation of the operator)
+
+
+def test_apply_inside_a_callers_cuda_graph():
+    """A caller may capture bem_apply into a CUDA graph of its own (torch.cuda.graph): the library then launches kernel by
+    kernel into that capture instead of starting one of its own."""
+    import torch
+    c = make_config(1)
+    ctx = _bem().bem_create(c["V"], c["F"], c["bubble_id"])
+    ctx.bem_setup(c["p"], c["leaf_size"], c["eta"])
+    qd, pd = torch.tensor(c["q"], device="cuda"), torch.tensor(c["phi"], device="cuda")
+    y0, y1 = torch.empty_like(qd), torch.empty_like(qd)
+    ctx.bem_apply(qd, pd, y0)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    ctx.bem_set_stream(side.cuda_stream)
+    with torch.cuda.stream(side):
+        ctx.bem_apply(qd, pd, y1)                                    # warm: every lazy allocation and attribute is made
+    side.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        ctx.bem_apply(qd, pd, y1)
+    for _ in range(3):
+        y1.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(y0, y1)
+    ctx.bem_set_stream(0)
+    ctx.bem_destroy()
