@@ -175,8 +175,22 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
         converged = true;
     } else {
         const int m = c->gmres_restart > 0 ? std::min(c->gmres_restart, std::max(max_iter, 1)) : std::max(max_iter, 1);
+        // Krylov basis: grown by doubling (64 vectors first) instead of (max_iter + 1) vectors up front -- config 5 with
+        // max_iter = 400 would reserve 8.2 GB for the 148-222 vectors it ends up using
         dvec<double> basis;
-        basis.alloc((size_t)(m + 1) * n);
+        int cap = std::min(m + 1, 64);
+        basis.alloc((size_t)cap * n);
+        auto grow = [&](int need) {
+            if (need <= cap) return;
+            int ncap = cap;
+            while (ncap < need) ncap = std::min(m + 1, 2 * ncap);
+            dvec<double> nb;
+            nb.alloc((size_t)ncap * n);
+            CUDA_TRY(cudaMemcpyAsync(nb.get(), basis.get(), (size_t)cap * n * sizeof(double), cudaMemcpyDeviceToDevice, s));
+            CUDA_TRY(cudaStreamSynchronize(s));
+            basis = std::move(nb);
+            cap = ncap;
+        };
         std::vector<double> H((size_t)(m + 1) * m, 0.0), cs(m), sn(m), g(m + 1), yv(m), hh(2 * (m + 1));
         auto Vk = [&](int k) { return basis.get() + (size_t)k * n; };
         bool x_is_zero = !use_x0;
@@ -208,6 +222,7 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
                 for (int i = 0; i <= k; ++i) H[(size_t)i * m + k] = hh[i] + hh[m + 1 + i];
                 const double hn = std::sqrt(K.dot(w.get(), w.get()));
                 H[(size_t)(k + 1) * m + k] = hn;
+                grow(k + 2);
                 if (hn > 0.0) K.scale(1.0 / hn, w.get(), Vk(k + 1));
                 for (int i = 0; i < k; ++i) {              // previous rotations
                     const double t = cs[i] * H[(size_t)i * m + k] + sn[i] * H[(size_t)(i + 1) * m + k];
