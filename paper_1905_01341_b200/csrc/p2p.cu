@@ -289,8 +289,8 @@ void launch_p2p_leaves(bem_ctx *c)
 
 // ------------------------------------------------------------------ SpMV + combine (a11, a12)
 // y_i = (1/4pi) sum_split ypart[split][map(i)] + sum_j ( C^S_ij q_j - C^D_ij phi_j ) [+ L_ii q_i - M_ii phi_i in V1]
-// 8 lanes per row: consecutive lanes read consecutive (col, val) entries -- coalesced 4 B + 16 B loads.
-constexpr int SPMV_LANES = 8;
+// 4 lanes per row: consecutive lanes read consecutive (col, val) entries -- coalesced 4 B + 16 B loads.
+constexpr int SPMV_LANES = 4;          // measured on config 5 (16 entries per row): 1, 2, 4, 8, 16 lanes -> 0.29, 0.24, 0.24, 0.27, 0.47 ms
 __global__ void __launch_bounds__(256)
 spmv_combine_kernel(const int64_t *__restrict__ rowptr, const int32_t *__restrict__ col, const double2 *__restrict__ val,
                     const double *__restrict__ q, const double *__restrict__ phi,
