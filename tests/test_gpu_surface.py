@@ -107,6 +107,32 @@ def test_filter_matches_oracle(lvl, p_f):
     flt.bem_filter_destroy()
 
 
+def test_filter_large_batch_takes_the_tensor_path():
+    """2048 columns and more run as two DMMA GEMMs (filter_apply_dmma): same tolerance against the oracle, ragged last
+    warp (2051 columns), in place, and equal to the FMA kernel's result on a small batch of the same columns to rounding."""
+    rng = np.random.default_rng(190501341 + 40)
+    v, _ = bi.icosphere(3)
+    th, ph = _angles(v)
+    nd = v.shape[0]
+    for p_f in (9, 4, 10):
+        Fm = so.filter_matrix(th, ph, p_f)
+        X = rng.standard_normal((2051, nd))
+        ref = so.filter_apply(Fm, X)
+        flt = _bem().bem_filter_create(th, ph, p_f)
+        out = np.full_like(X, np.nan)
+        flt.bem_filter_apply(X, X.shape[0], out)
+        assert _maxrel(out, ref) <= 1e-10
+        small = np.full((64, nd), np.nan)
+        flt.bem_filter_apply(np.ascontiguousarray(X[:64]), 64, small)
+        assert _maxrel(small, out[:64]) <= 1e-12
+        import torch
+        xd = torch.tensor(X, device="cuda")
+        flt.bem_filter_apply(xd, X.shape[0], xd)
+        torch.cuda.synchronize()
+        assert np.array_equal(xd.cpu().numpy(), out)
+        flt.bem_filter_destroy()
+
+
 def test_filter_argument_checks():
     bem = _bem()
     v, _ = bi.icosphere(1)                                          # 42 points
