@@ -214,6 +214,9 @@ def run_gpu(args):
         ctx.bem_set_option("p2p_ctas", args.p2p_ctas)
     if args.reduce_ctas:
         ctx.bem_set_option("reduce_ctas", args.reduce_ctas)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        ctx.bem_set_option(k, float(v))
     ctx.bem_setup(p, args.leaf_size or c["leaf_size"], c["eta"])
     torch.cuda.synchronize()
     setup_wall_ms = (time.perf_counter() - t0) * 1e3
@@ -307,13 +310,13 @@ def run_gpu(args):
                                 if f32 else "17 FP64 instr / 26 flop per pair; slot_frac = share of the FP64 pipe's issue slots (nominal 18.6 T instr/s)"))
     if not args.direct:
         m2l_s = tm["m2l"] * 1e-3
-        exec_flop = stats["m2l_pairs"] * 4.0 * nre * nre          # two nre x nre blocks, 2 flop per MAC (azimuth split)
+        exec_flop = stats["m2l_flop"]                             # two blocks of (4 KE)^2 MACs per pair, KE = k-steps of the pair's truncation class
         dense_flop = stats["m2l_pairs"] * 2.0 * p ** 4            # the dense p^2 x p^2 translation of SURVEY.md 8(d)
         kernels["m2l"] = dict(ms=tm["m2l"], pairs=stats["m2l_pairs"], executed_tflops=exec_flop / m2l_s / 1e12,
                               dense_equivalent_tflops=dense_flop / m2l_s / 1e12,
                               frac_of_measured_dmma_peak=exec_flop / m2l_s / 1e9 / dmma, frac_of_nominal_fp64_peak=exec_flop / m2l_s / 1e9 / FP64_NOMINAL_GFLOPS,
                               note="executed = 4 nre^2 flop per pair on the FP64 tensor path (nre = %d); dense-equivalent = 2 p^4" % int(nre))
-        red_bytes = stats["m2l_pairs"] * 8.0 * stats["exp_stride"]
+        red_bytes = stats["m2l_row_bytes"]
         kernels["reduce"] = dict(ms=tm["l2l_reduce"], gbs=red_bytes / (tm["l2l_reduce"] * 1e-3) / 1e9,
                                  frac_hbm=red_bytes / (tm["l2l_reduce"] * 1e-3) / 1e9 / hbm_peak, bytes=red_bytes,
                                  note="reads one translated row (8 nst bytes) per pair; L2L rows not counted")
@@ -471,6 +474,7 @@ def main():
                     help="leaf-level far pairs with nt x ns <= this are summed directly instead of translated (default: library cost model; 0: off)")
     ap.add_argument("--p2p-ctas", type=int, default=0, help="fp32 near field: CTAs per SM of its persistent grid (0: library default)")
     ap.add_argument("--reduce-ctas", type=int, default=0, help="CTAs per SM of the persistent row-sum passes (0: library cost model)")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="any bem_set_option key (repeatable), set before bem_setup")
     ap.add_argument("--solve-iters", type=int, default=-1, help="also run bem_solve with this max_iter (0: skip; -1: 30, or 400 = to convergence on config 5)")
     ap.add_argument("--solve-tol", type=float, default=1e-6)
     ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU time budget of one oracle sample")

@@ -72,7 +72,10 @@ enum {
     BEM_S_N_TARGETS = 0, BEM_S_N_SOURCES, BEM_S_LMAX, BEM_S_N_SRC_LEAVES, BEM_S_N_TGT_LEAVES,
     BEM_S_P2P_PAIRS, BEM_S_M2L_PAIRS, BEM_S_CSR_NNZ, BEM_S_NEAR_TRIANGLES, BEM_S_SETUP_MS,
     BEM_S_N_SRC_BOXES, BEM_S_N_TGT_BOXES, BEM_S_DEVICE_BYTES, BEM_S_EXP_STRIDE,
-    BEM_S_KERNEL_LAUNCHES_PER_APPLY, BEM_S_COUNT
+    BEM_S_KERNEL_LAUNCHES_PER_APPLY,
+    BEM_S_M2L_FLOP,        /* executed flop of the M2L tiles of one product (graded truncation: 4 (4 KE)^2 per pair) */
+    BEM_S_M2L_ROW_BYTES,   /* bytes of translated rows the per-target sums read in one product                     */
+    BEM_S_COUNT
 };
 
 /* bem_create -- take a triangulated bubble-cluster surface (PAPER.md:150-152:

@@ -136,7 +136,7 @@ static int reduce_ctas_for(const bem_ctx *c)
     if (c->reduce_ctas > 0) return c->reduce_ctas;
     const bool f32 = c->p2p_precision == 1;
     const double t_p2p = (double)c->p2p_pairs / (f32 ? 1400e9 : 700e9);
-    const double t_sum = (double)c->m2l_pairs * 8.0 * c->nst / 4e12;
+    const double t_sum = c->m2l_row_bytes / 4e12;
     const int k = (int)std::ceil(16.0 * 1.3 * t_sum / std::max(t_p2p, 1e-9));
     return std::max(3, std::min(k, f32 ? 6 : 16));
 }
@@ -534,6 +534,8 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "p2p_precision")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->p2p_precision = v; }
     else if (!strcmp(key, "direct_pairs")) { if (value < -1 || value > 1e9) return BEM_ERR_INVALID_ARG; c->direct_max = (int64_t)value; c->ready = false; }
     else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
+    else if (!strcmp(key, "m2l_order_radius")) { if (!(value >= 0 && value < 1.0)) return BEM_ERR_INVALID_ARG; c->m2l_order_radius = value; c->ready = false; }
+    else if (!strcmp(key, "m2l_order_extra")) { if (v < -8 || v > 8) return BEM_ERR_INVALID_ARG; c->m2l_order_extra = v; c->ready = false; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
     return BEM_OK;
@@ -616,6 +618,8 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
         s[BEM_S_N_TGT_LEAVES] = c->tb.nbox[c->tb.lmax];
         s[BEM_S_P2P_PAIRS] = (double)c->p2p_pairs;
         s[BEM_S_M2L_PAIRS] = (double)c->m2l_pairs;
+        s[BEM_S_M2L_FLOP] = c->m2l_flop;
+        s[BEM_S_M2L_ROW_BYTES] = c->m2l_row_bytes;
         s[BEM_S_N_SRC_BOXES] = c->sb.total();
         s[BEM_S_N_TGT_BOXES] = c->tb.total();
     } else {

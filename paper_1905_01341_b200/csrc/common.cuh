@@ -113,7 +113,11 @@ struct BoxSet {                     // the non-empty boxes of one point set on l
 
 // One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
 // executed as (tiles of a dense GEMM per matrix) -> scratch rows in target-major order -> fixed-order row sums.
-struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split)
+struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split),
+                                                      // bits 8..: truncation class of the matrix (graded M2L, translate.cu)
+constexpr int M2L_NCLS = 5;        // truncation classes of the M2L tiles: degrees < pl - i, i = 0..4
+// k-steps (4 dofs each, in pairs) of either block that hold the degrees < pp: 4 ke_of(pl) = nre of the layout
+__host__ __device__ constexpr int ke_of(int pp) { return pp < 2 ? 2 : 2 * ((pp * (pp + 1) / 2 + 7) / 8); }
 constexpr int TILES_ALL = 0, TILES_SPLIT = 1, TILES_DENSE = 2;
 struct Stage {
     int64_t npairs = 0;
@@ -125,7 +129,8 @@ struct Stage {
     dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
     dvec<int32_t> krow;             // [npairs] target-major index k of the pair in tile row r: its scratch row (the rows of a target are
                                     // contiguous in scratch, so the row sums stream them; the tiles scatter whole 8 nst-byte rows)
-    dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order): the reduce pass rotates back by its azimuth
+    dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order) | dofs its scratch row carries << 16: the reduce
+                                    // pass rotates back by the azimuth of the matrix
     dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
     dvec<Tile> tiles;
     int ntiles = 0;
@@ -197,6 +202,12 @@ struct bem_ctx {
     bem::dvec<double> mats;         // [N_MATS * nst * nst] real translation matrices, row = input dof k, col = output dof
     bem::dvec<double2> rot;         // [N_MATS * ROT_M] (cos m a, sin m a): azimuth a of the M2L offset, identity for M2M / L2L
     bem::dvec<int32_t> kinfo;       // [nst] order m of every stored dof (0 for padding)
+    bem::dvec<int32_t> mat_ne;      // [N_MATS] leading dofs of the real-part block that take part in the translation (graded truncation)
+    std::vector<int32_t> mat_ne_host, mat_cls_host;   // host copies: dofs and tile class (min(M2L_NCLS - 1, pl - p_o)) per matrix
+    double m2l_order_radius = 0.5;  // option "m2l_order_radius": cluster radius a (box edges) of the graded truncation, 0 = off
+    int m2l_order_extra = 1;        // option "m2l_order_extra": degrees added to the graded order of every offset
+    double m2l_flop = 0;            // executed flop of the M2L tiles of one product: 4 (4 KE)^2 per pair, KE the k-steps of its class
+    double m2l_row_bytes = 0;       // bytes of translated rows the sums read per product: 16 x dofs carried per pair
     bem::dvec<double> Mexp, Lexp;   // [total boxes * nst]
     bem::dvec<double> scratch;      // [pairs of all M2L (+ L2L) stages * nst]: one region per level, so that the tiles of all
                                     // levels can be issued before the first reduce pass

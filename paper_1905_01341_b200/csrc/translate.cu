@@ -14,6 +14,7 @@
 #include "morton.cuh"
 
 #include <cmath>
+#include <mutex>
 
 namespace bem {
 
@@ -40,7 +41,7 @@ __global__ void harmonic_tables(int p, double *tab_re, double *tab_im, int strid
     }
 }
 // mats[m][k][c] = T_m[c][k]  (row = input dof, column = output dof); padding dofs and degrees >= p are zero
-__global__ void fill_matrices(int p, int nre, int nst, const double *tab_re, const double *tab_im, int stride, double *mats)
+__global__ void fill_matrices(int p, int nre, int nst, const double *tab_re, const double *tab_im, int stride, const int32_t *mat_ne, double *mats)
 {
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t per = (int64_t)nst * nst;
@@ -51,7 +52,10 @@ __global__ void fill_matrices(int p, int nre, int nst, const double *tab_re, con
     const double *re = tab_re + (size_t)m * stride, *im = tab_im + (size_t)m * stride;
     if (m < MAT_L2L) {
         const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
-        if (max(max(abs(ox), abs(oy)), abs(oz)) >= 2 && ((k < nre) == (cc < nre))) v = m2l_entry(re, im, p, nre, cc, k);
+        // graded truncation: only the leading mat_ne[m] dofs of either part take part (build_matrices)
+        const int ne = mat_ne[m];
+        if (max(max(abs(ox), abs(oy)), abs(oz)) >= 2 && ((k < nre) == (cc < nre)) && (k < nre ? k : k - nre) < ne && (cc < nre ? cc : cc - nre) < ne)
+            v = m2l_entry(re, im, p, nre, cc, k);
     } else if (m < MAT_M2M) v = l2l_entry(re, im, p, nre, cc, k);
     else v = m2m_entry(re, im, p, nre, cc, k);
     mats[idx] = v;
@@ -68,9 +72,32 @@ void build_matrices(bem_ctx *c)
     tim.zero(c->stream);
     harmonic_tables<<<cdiv(N_MATS, 64), 64, 0, c->stream>>>(p, tre.get(), tim.get(), stride);
     KERNEL_CHECK();
+    // Graded truncation of the M2L translations by separation (option "m2l_order_radius" = a > 0, in box edges).  The
+    // truncation error of a translation over the offset o falls like kappa(o)^p, kappa = a / (|o| - a) for clusters of
+    // radius a; the nearest offsets (|o| = 2) set the error of the product, and an offset further away reaches the same
+    // error with p_o = ceil(p ln kappa(2) / ln kappa(|o|)) + extra degrees (option "m2l_order_extra").  Only the leading
+    // mat_ne[m] = p_o (p_o + 1) / 2 dofs of the real-part block (= of the imaginary-part block) of matrix m are non-zero,
+    // and the M2L tile kernels run the k-steps and n-tiles of class min(M2L_NCLS - 1, pl - p_o) only.  a = 0: p_o = p.
+    std::vector<int32_t> ne(N_MATS, c->nre), cls(N_MATS, 0);
+    for (int m = 0; m < MAT_L2L; ++m) {
+        const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
+        int po = p;
+        if (c->m2l_order_radius > 0 && std::max(std::max(std::abs(ox), std::abs(oy)), std::abs(oz)) >= 2) {
+            const double a = c->m2l_order_radius, d = std::sqrt((double)(ox * ox + oy * oy + oz * oz));
+            const double k2 = a / (2.0 - a), kd = a / (d - a);
+            po = (int)std::ceil(p * std::log(k2) / std::log(kd) - 1e-9) + c->m2l_order_extra;
+            po = std::max(std::min(po, p), std::min(p, 2));
+        }
+        ne[m] = std::min(c->nre, po * (po + 1) / 2);
+        cls[m] = std::max(0, std::min(M2L_NCLS - 1, c->pl - po));
+    }
+    c->mat_ne_host = ne;
+    c->mat_cls_host = cls;
+    c->mat_ne.alloc(N_MATS);
+    CUDA_TRY(cudaMemcpyAsync(c->mat_ne.get(), ne.data(), N_MATS * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     const int64_t tot = (int64_t)N_MATS * nst * nst;
     c->mats.alloc(tot);
-    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, c->nre, nst, tre.get(), tim.get(), stride, c->mats.get());
+    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, c->nre, nst, tre.get(), tim.get(), stride, c->mat_ne.get(), c->mats.get());
     KERNEL_CHECK();
     // azimuth table (cos m a, sin m a) and the per-dof table (m, partner = the other part of the same (l, m), part)
     std::vector<double2> rot((size_t)N_MATS * ROT_M);
@@ -346,20 +373,22 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
 // L2 hits) the rotated imaginary parts for the imaginary-part columns: 2 KSH instead of 4 KSH registers for A,
 // so three CTAs (24 warps) fit an SM instead of two and the row gather of one CTA hides behind the DMMAs of the
 // others (ncu on the two-CTA version: tensor pipe 65% active, 30% of the samples in the gather prologue).
-template <int KSH>
-__global__ void __launch_bounds__(DM_THREADS, (KSH <= 20 ? 3 : 2))
-translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
-                     const double *__restrict__ Mexp, const double *__restrict__ mats,
-                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+//
+// Graded truncation (build_matrices): a tile of class i runs only the KE = ke_of(PL - i) k-steps and KE / 2 n-tiles
+// of either block that hold the degrees < PL - i; KSH = ke_of(PL) is the layout (row stride, place of the imaginary
+// parts).  Every class is its own fully unrolled body (the k-loop must stay free of branches: the B fragments of the
+// next k-steps are loaded while the DMMAs of this one run), selected per tile by a CTA-uniform switch.
+template <int KSH, int KE>
+__device__ __forceinline__ void m2l_body8(const Tile &tile, const int32_t *__restrict__ src_sorted, const double *__restrict__ Mexp,
+                                          const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+                                          const int32_t *__restrict__ krow, double *__restrict__ scratch, double *dm_smem, double2 *cs_k)
 {
-    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
-    __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
-    constexpr int NRE = 4 * KSH, NST = 2 * NRE;
-    constexpr int NTH = KSH / 2;                               // n-tiles (8 columns) of one block
+    constexpr int NRE = 4 * KSH, NST = 2 * NRE;               // layout of the stored rows and matrices
+    constexpr int KR = 4 * KE;                                 // dofs of either block that take part
+    constexpr int NTH = KE / 2;                                // n-tiles (8 columns) of one block
     constexpr int CPB = (NTH + DM_NT - 1) / DM_NT;             // chunks per block
     constexpr int CW = (NTH + CPB - 1) / CPB;                  // chunk width in n-tiles
-    const Tile tile = tiles[blockIdx.x];
-    double *Bs0 = dm_smem, *Bs1 = dm_smem + NRE * DM_S;
+    double *Bs0 = dm_smem, *Bs1 = dm_smem + KR * DM_S;
     const double *B = mats + (size_t)tile.mat * NST * NST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int lr = lane >> 2, lk = lane & 3;
@@ -368,20 +397,20 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
 
     auto issue = [&](int ch, double *dst) {
         const int blk = ch >= CPB, cl = blk ? ch - CPB : ch;
-        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
-        const int c0 = 8 * t0, per_row = 4 * nt, k0 = blk * NRE;
-        for (int i = threadIdx.x; i < NRE * per_row; i += DM_THREADS) {
+        const int t0 = CW * cl, nt = min(CW, NTH - t0);
+        const int c0 = blk * NRE + 8 * t0, per_row = 4 * nt, k0 = blk * NRE;
+        for (int i = threadIdx.x; i < KR * per_row; i += DM_THREADS) {
             const int k = i / per_row, j = (i % per_row) * 2;
             cp_async16(dst + k * DM_S + j, B + (size_t)(k0 + k) * NST + c0 + j);
         }
         cp_async_commit();
     };
     issue(0, Bs0);
-    for (int k = threadIdx.x; k < NRE; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
+    for (int k = threadIdx.x; k < KR; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
     const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
     const double2 *ap = reinterpret_cast<const double2 *>(Mexp + (size_t)(arow < 0 ? 0 : arow) * NST) + lk;
     double *orow = scratch + (size_t)(rvalid ? krow[tile.row0 + row] : 0) * NST + 2 * lk;
-    double a[KSH];
+    double a[KE];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
         double *cur = (ch & 1) ? Bs1 : Bs0;
@@ -391,7 +420,7 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
         if (ch + 1 < 2 * CPB) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
         if (cl == 0) {                                          // first chunk of a block: this block's half of A
 #pragma unroll
-            for (int j = 0; j < KSH / 2; ++j) {
+            for (int j = 0; j < KE / 2; ++j) {
                 double2 re = make_double2(0.0, 0.0), im = re;
                 if (arow >= 0) { re = ap[4 * j]; im = ap[4 * j + NRE / 2]; }
                 const double2 c0 = cs_k[8 * j + 2 * lk], c1 = cs_k[8 * j + 2 * lk + 1];
@@ -399,8 +428,30 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
                 else { a[2 * j] = fma(c0.x, im.x, c0.y * re.x); a[2 * j + 1] = fma(c1.x, im.y, c1.y * re.y); }
             }
         }
-        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
-        dm_chunk<KSH, 0, KSH, 0>(a, cur, nt, lr, lk, rvalid, orow + 8 * t0);
+        const int t0 = CW * cl, nt = min(CW, NTH - t0);
+        dm_chunk<KE, 0, KE, 0>(a, cur, nt, lr, lk, rvalid, orow + blk * NRE + 8 * t0);
+    }
+}
+
+constexpr int M2L_NCLS_K = M2L_NCLS;
+static_assert(M2L_NCLS_K == 5, "the switches below list the classes");
+
+template <int PL>
+__global__ void __launch_bounds__(DM_THREADS, (ke_of(PL) <= 20 ? 3 : 2))
+translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
+                     const double *__restrict__ Mexp, const double *__restrict__ mats,
+                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+{
+    constexpr int KSH = ke_of(PL);
+    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
+    __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
+    const Tile tile = tiles[blockIdx.x];
+    switch (tile.flags >> 8) {                                  // truncation class of the tile's matrix (CTA-uniform)
+    case 0: m2l_body8<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 1: m2l_body8<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 2: m2l_body8<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 3: m2l_body8<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    default: m2l_body8<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
     }
 }
 
@@ -408,8 +459,8 @@ translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__
 // warp).  ncu on the 8 x 8-row version: LSU wavefronts 55% with the tensor pipe at 65% -- the fragment loads
 // (2 wavefronts per DMMA), the cp.async fills, the row gather and the stores share one pipe.
 constexpr int DM16_THREADS = 128;
-template <int KSH, int NT>
-__device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KSH], const double (&a1)[KSH], const double *cur, int lr, int lk,
+template <int KE, int NT>
+__device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KE], const double (&a1)[KE], const double *cur, int lr, int lk,
                                               bool v0, bool v1, double *o0, double *o1)
 {
     const double *bp = cur + 2 * lk * DM_S + lr;
@@ -417,7 +468,7 @@ __device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KSH], const dou
 #pragma unroll
     for (int j = 0; j < NT; ++j) c0[j][0] = c0[j][1] = c1[j][0] = c1[j][1] = 0.0;
 #pragma unroll
-    for (int s = 0; s < KSH; ++s) {
+    for (int s = 0; s < KE; ++s) {
         const double *b = bp + (8 * (s >> 1) + (s & 1)) * DM_S;
 #pragma unroll
         for (int j = 0; j < NT; ++j) {
@@ -433,20 +484,17 @@ __device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KSH], const dou
     }
 }
 
-template <int KSH>
-__global__ void __launch_bounds__(DM16_THREADS, 3)
-translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
-                       const double *__restrict__ Mexp, const double *__restrict__ mats,
-                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+template <int KSH, int KE>
+__device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__restrict__ src_sorted, const double *__restrict__ Mexp,
+                                           const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+                                           const int32_t *__restrict__ krow, double *__restrict__ scratch, double *dm_smem, double2 *cs_k)
 {
-    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
-    __shared__ double2 cs_k[4 * KSH];
     constexpr int NRE = 4 * KSH, NST = 2 * NRE;
-    constexpr int NTH = KSH / 2;
+    constexpr int KR = 4 * KE;
+    constexpr int NTH = KE / 2;
     constexpr int CPB = (NTH + DM_NT - 1) / DM_NT;
     constexpr int CW = (NTH + CPB - 1) / CPB;
-    const Tile tile = tiles[blockIdx.x];
-    double *Bs0 = dm_smem, *Bs1 = dm_smem + NRE * DM_S;
+    double *Bs0 = dm_smem, *Bs1 = dm_smem + KR * DM_S;
     const double *B = mats + (size_t)tile.mat * NST * NST;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int lr = lane >> 2, lk = lane & 3;
@@ -455,22 +503,22 @@ translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict
 
     auto issue = [&](int ch, double *dst) {
         const int blk = ch >= CPB, cl = blk ? ch - CPB : ch;
-        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
-        const int c0 = 8 * t0, per_row = 4 * nt, k0 = blk * NRE;
-        for (int i = threadIdx.x; i < NRE * per_row; i += DM16_THREADS) {
+        const int t0 = CW * cl, nt = min(CW, NTH - t0);
+        const int c0 = blk * NRE + 8 * t0, per_row = 4 * nt, k0 = blk * NRE;
+        for (int i = threadIdx.x; i < KR * per_row; i += DM16_THREADS) {
             const int k = i / per_row, j = (i % per_row) * 2;
             cp_async16(dst + k * DM_S + j, B + (size_t)(k0 + k) * NST + c0 + j);
         }
         cp_async_commit();
     };
     issue(0, Bs0);
-    for (int k = threadIdx.x; k < NRE; k += DM16_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
+    for (int k = threadIdx.x; k < KR; k += DM16_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
     const int ar0 = v0 ? src_sorted[tile.row0 + row0] : -1, ar1 = v1 ? src_sorted[tile.row0 + row1] : -1;
     const double2 *ap0 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar0 < 0 ? 0 : ar0) * NST) + lk;
     const double2 *ap1 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar1 < 0 ? 0 : ar1) * NST) + lk;
     double *o0 = scratch + (size_t)(v0 ? krow[tile.row0 + row0] : 0) * NST + 2 * lk;
     double *o1 = scratch + (size_t)(v1 ? krow[tile.row0 + row1] : 0) * NST + 2 * lk;
-    double a0[KSH], a1[KSH];
+    double a0[KE], a1[KE];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
         double *cur = (ch & 1) ? Bs1 : Bs0;
@@ -480,7 +528,7 @@ translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict
         if (ch + 1 < 2 * CPB) issue(ch + 1, (ch & 1) ? Bs0 : Bs1);
         if (cl == 0) {
 #pragma unroll
-            for (int j = 0; j < KSH / 2; ++j) {
+            for (int j = 0; j < KE / 2; ++j) {
                 const double2 z = make_double2(0.0, 0.0);
                 const double2 re0 = ar0 >= 0 ? ap0[4 * j] : z, im0 = ar0 >= 0 ? ap0[4 * j + NRE / 2] : z;
                 const double2 re1 = ar1 >= 0 ? ap1[4 * j] : z, im1 = ar1 >= 0 ? ap1[4 * j + NRE / 2] : z;
@@ -494,35 +542,65 @@ translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict
                 }
             }
         }
-        const int t0 = blk * NTH + CW * cl, nt = min(CW, (blk + 1) * NTH - t0);
+        const int t0 = CW * cl, nt = min(CW, NTH - t0), oc = blk * NRE + 8 * t0;
         switch (nt) {
-        case 5: dm16_chunk_nt<KSH, 5>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
-        case 4: dm16_chunk_nt<KSH, 4>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
-        case 3: dm16_chunk_nt<KSH, 3>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
-        case 2: dm16_chunk_nt<KSH, 2>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
-        default: dm16_chunk_nt<KSH, 1>(a0, a1, cur, lr, lk, v0, v1, o0 + 8 * t0, o1 + 8 * t0); break;
+        case 5: dm16_chunk_nt<KE, 5>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
+        case 4: dm16_chunk_nt<KE, 4>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
+        case 3: dm16_chunk_nt<KE, 3>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
+        case 2: dm16_chunk_nt<KE, 2>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
+        default: dm16_chunk_nt<KE, 1>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
         }
     }
 }
 
-template <int KSH>
+template <int PL>
+__global__ void __launch_bounds__(DM16_THREADS, 3)
+translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
+                       const double *__restrict__ Mexp, const double *__restrict__ mats,
+                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+{
+    constexpr int KSH = ke_of(PL);
+    extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
+    __shared__ double2 cs_k[4 * KSH];
+    const Tile tile = tiles[blockIdx.x];
+    switch (tile.flags >> 8) {
+    case 0: m2l_body16<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 1: m2l_body16<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 2: m2l_body16<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 3: m2l_body16<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    default: m2l_body16<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    }
+}
+
+// attributes of a kernel are per device: one flag per device, under a mutex (several contexts, several devices)
+static bool first_use_on_device(std::vector<char> &done, int device)
+{
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    if ((int)done.size() <= device) done.resize(device + 1, 0);
+    if (done[device]) return false;
+    done[device] = 1;
+    return true;
+}
+
+template <int PL>
 static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t stream, double *scratch)
 {
+    constexpr int KSH = ke_of(PL);
     const size_t smem = (size_t)2 * 4 * KSH * DM_S * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
+    static std::vector<char> attr_done;
+    if (first_use_on_device(attr_done, c->device)) {
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        if (KSH == 20) CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split16<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
+        CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split<PL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (PL == 12) CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split16<(PL == 12 ? PL : 4)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     }
     if (which != TILES_DENSE && st.ntiles_split > 0) {
-        if (KSH == 20 && c->m2l_rows16)                          // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
-            translate_dmma_split16<(KSH == 20 ? KSH : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
+        if (PL == 12 && c->m2l_rows16)                           // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
+            translate_dmma_split16<(PL == 12 ? PL : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
                 st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
         else
-            translate_dmma_split<KSH><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                    c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
+            translate_dmma_split<PL><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
+                                                                                   c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
     }
     if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
         translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
@@ -533,34 +611,52 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
 // out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[k][:]   (fixed order; a_k = azimuth of
 // pair k's matrix, the identity for M2M / L2L pairs).  One CTA per target box, one thread per coefficient (l, m):
 // it reads the real and the imaginary part (nre apart) of every row once and writes both.
+constexpr int RED_CHUNK = 192;     // pairs of a target staged at a time (an M2L list holds at most 189)
 __global__ void __launch_bounds__(160)
 translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t,
                  const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
                  int nre, int accumulate, int ntgt, double *__restrict__ out)
 {
+    // mat_t[k] = matrix id | (dofs the row carries << 16): a row of a graded (truncated) translation holds its leading
+    // dofs only (tree.cu pack_row_dofs); the rest of the scratch row was never written.  The words of the target's pairs
+    // are staged in shared memory so that the row loads do not wait for a global load of their predicate.
+    __shared__ int s_mt[RED_CHUNK];
     const int nst = 2 * nre;
     for (int t = blockIdx.x; t < ntgt; t += gridDim.x) {            // grid < ntgt: a persistent pass (see launch_stage_reduce)
         const int b = ptr[t], e = ptr[t + 1];
         double *o = out + (size_t)t * nst;
-        for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
-            const int m = kinfo[cc];
-            double sr = 0.0, si = 0.0;
-            if (m == 0) {
+        if (b == e && !accumulate)
+            for (int cc = threadIdx.x; cc < nst; cc += blockDim.x) o[cc] = 0.0;
+        for (int k0 = b; k0 < e; k0 += RED_CHUNK) {                 // one round for every list the library builds
+            const int n = min(RED_CHUNK, e - k0);
+            __syncthreads();
+            for (int i = threadIdx.x; i < n; i += blockDim.x) s_mt[i] = mat_t[k0 + i];
+            __syncthreads();
+            for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
+                const int m = kinfo[cc];
+                const double *base = scratch + (size_t)k0 * nst + cc;
+                double sr = 0.0, si = 0.0;
+                if (m == 0) {
 #pragma unroll 8
-                for (int k = b; k < e; ++k) sr += scratch[(size_t)k * nst + cc];
-            } else {
+                    for (int i = 0; i < n; ++i)
+                        if (cc < (s_mt[i] >> 16)) sr += base[(size_t)i * nst];
+                } else {
 #pragma unroll 8
-                for (int k = b; k < e; ++k) {
-                    const double *row = scratch + (size_t)k * nst + cc;
-                    double vr = row[0], vi = row[nre];
-                    azimuth(__ldg(rot + (size_t)mat_t[k] * ROT_M + m), vr, vi);
-                    sr += vr;
-                    si += vi;
+                    for (int i = 0; i < n; ++i) {
+                        const int mt = s_mt[i];
+                        if (cc < (mt >> 16)) {
+                            const double *row = base + (size_t)i * nst;
+                            double vr = row[0], vi = row[nre];
+                            azimuth(__ldg(rot + (size_t)(mt & 0xffff) * ROT_M + m), vr, vi);
+                            sr += vr;
+                            si += vi;
+                        }
+                    }
                 }
+                if (accumulate || k0 > b) { sr += o[cc]; si += o[cc + nre]; }
+                o[cc] = sr;
+                o[cc + nre] = si;
             }
-            if (accumulate) { sr += o[cc]; si += o[cc + nre]; }
-            o[cc] = sr;
-            o[cc + nre] = si;
         }
     }
 }
@@ -578,13 +674,13 @@ void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stre
         translate_gemm<<<grid, GEMM_THREADS, 0, stream>>>(st.tiles.get() + first, st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
                                                           c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, st.krow.get(), scratch);
     }
-    else if (pl == 4) launch_dmma<4>(c, st, which, stream, scratch);     // nre / 4 of the layout for pl = 4, 6, .., 16
+    else if (pl == 4) launch_dmma<4>(c, st, which, stream, scratch);     // layout degree -> ke_of(pl) = nre / 4 k-steps per block
     else if (pl == 6) launch_dmma<6>(c, st, which, stream, scratch);
-    else if (pl == 8) launch_dmma<10>(c, st, which, stream, scratch);
-    else if (pl == 10) launch_dmma<14>(c, st, which, stream, scratch);
-    else if (pl == 12) launch_dmma<20>(c, st, which, stream, scratch);
-    else if (pl == 14) launch_dmma<28>(c, st, which, stream, scratch);
-    else launch_dmma<34>(c, st, which, stream, scratch);
+    else if (pl == 8) launch_dmma<8>(c, st, which, stream, scratch);
+    else if (pl == 10) launch_dmma<10>(c, st, which, stream, scratch);
+    else if (pl == 12) launch_dmma<12>(c, st, which, stream, scratch);
+    else if (pl == 14) launch_dmma<14>(c, st, which, stream, scratch);
+    else launch_dmma<16>(c, st, which, stream, scratch);
     KERNEL_CHECK();
 }
 
@@ -597,11 +693,9 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
     if (st.ntgt == 0) return;
     double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
     const int grid = ctas_per_sm > 0 ? std::min(st.ntgt, c->n_sm * ctas_per_sm) : st.ntgt;
-    static bool attr_set = false;
-    if (!attr_set) {                                                   // same carve-out as the pair kernels it runs beside (common.cuh)
+    static std::vector<char> attr_done;
+    if (first_use_on_device(attr_done, c->device))                     // same carve-out as the pair kernels it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-        attr_set = true;
-    }
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
         st.ptr.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
         c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : 0, st.ntgt, out);

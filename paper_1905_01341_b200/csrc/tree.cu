@@ -233,8 +233,15 @@ __global__ void stage_finish(const uint32_t *order, const int32_t *src, int64_t 
 
 constexpr int GEMM_TM = 64;   // rows per GEMM tile (translate.cu uses the same constant)
 
+// mat_t[k] = matrix id | (dofs of either block the scratch row of pair k carries << 16)   (graded M2L, translate.cu)
+__global__ void pack_row_dofs(int32_t *mat_t, int64_t n, const int32_t *mat_ne)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) mat_t[k] |= mat_ne[mat_t[k]] << 16;
+}
+
 // from target-major (src, mat) pairs to a Stage: rows sorted by matrix, tiles, inverse positions
-static void finish_stage(Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cudaStream_t s)
+static void finish_stage(bem_ctx *c, Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cudaStream_t s)
 {
     const int64_t n = st.npairs;
     st.src_sorted.alloc(n);
@@ -258,23 +265,36 @@ static void finish_stage(Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cuda
     }
     std::vector<Tile> tiles;
     int row = 0;
+    for (int m = 0; m < MAT_L2L; ++m) {                                 // executed work of the M2L tiles (bem_get_stats)
+        const bool dmma = c->gemm_path == 0 && c->pl <= 16;             // the plain-FMA tiles run every matrix in full
+        const double kr = dmma ? 4.0 * ke_of(c->pl - c->mat_cls_host[m]) : (double)c->nre;
+        c->m2l_flop += (double)h[m] * 4.0 * kr * kr;
+        c->m2l_row_bytes += (double)h[m] * 16.0 * c->mat_ne_host[m];
+    }
     for (int m = 0; m < N_MATS; ++m) {
         for (int r = 0; r < h[m]; r += GEMM_TM) {
             Tile t;
             t.mat = m;
             t.row0 = row + r;
             t.nrows = std::min(GEMM_TM, h[m] - r);
-            t.flags = ((m >= MAT_L2L && m < MAT_M2M) ? 1 : 0) | (m < MAT_L2L ? 2 : 0);
+            t.flags = ((m >= MAT_L2L && m < MAT_M2M) ? 1 : 0) | (m < MAT_L2L ? 2 : 0) | (c->mat_cls_host[m] << 8);
             tiles.push_back(t);
         }
         row += h[m];
     }
     st.mat_t = std::move(mat);
+    if (n > 0) {
+        pack_row_dofs<<<cdiv(n, 256), 256, 0, s>>>(st.mat_t.get(), n, c->mat_ne.get());
+        KERNEL_CHECK();
+    }
     st.ntiles = (int)tiles.size();
     st.ntiles_split = 0;
     for (const Tile &t : tiles) st.ntiles_split += (t.flags & 2) ? 1 : 0;
     st.tiles.alloc(tiles.size());
-    if (!tiles.empty()) CUDA_TRY(cudaMemcpy(st.tiles.get(), tiles.data(), tiles.size() * sizeof(Tile), cudaMemcpyHostToDevice));
+    if (!tiles.empty()) {
+        CUDA_TRY(cudaMemcpyAsync(st.tiles.get(), tiles.data(), tiles.size() * sizeof(Tile), cudaMemcpyHostToDevice, s));
+        CUDA_TRY(cudaStreamSynchronize(s));                              // `tiles` is a local
+    }
 }
 
 void build_lists(bem_ctx *c)
@@ -302,6 +322,7 @@ void build_lists(bem_ctx *c)
     c->m2l.clear();
     c->m2l.resize(lmax + 1);
     c->m2l_pairs = 0;
+    c->m2l_flop = c->m2l_row_bytes = 0;
     int64_t max_pairs = 0;
     for (int l = 2; l <= lmax; ++l) {
         Stage &st = c->m2l[l];
@@ -342,7 +363,7 @@ void build_lists(bem_ctx *c)
                                                         tb.begin.get(), sb.begin.get(), dmax, nullptr, dmax > 0 ? c->xdir_ptr.get() : nullptr,
                                                         dmax > 0 ? c->xdir_src.get() : nullptr, pc.get());
         KERNEL_CHECK();
-        finish_stage(st, src, mat, s);
+        finish_stage(c, st, src, mat, s);
         c->m2l_pairs += total;
         st.scratch_off = max_pairs;                           // regions of the levels one after the other
         max_pairs += total;
@@ -364,7 +385,7 @@ void build_lists(bem_ctx *c)
         mat.alloc(nc);
         m2m_pairs<<<cdiv(nc, 256), 256, 0, s>>>(sb.bkey[l + 1].get(), nc, sb.base[l + 1], src.get(), mat.get());
         KERNEL_CHECK();
-        finish_stage(st, src, mat, s);
+        finish_stage(c, st, src, mat, s);
         st.scratch_off = 0;                                   // M2M runs before any M2L tile: aliases the first region
         max_pairs = std::max<int64_t>(max_pairs, nc);
     }
@@ -385,7 +406,7 @@ void build_lists(bem_ctx *c)
         mat.alloc(nt);
         l2l_pairs<<<cdiv(nt + 1, 256), 256, 0, s>>>(tb.bkey[l].get(), tb.parent[l].get(), nt, tb.base[l - 1], src.get(), mat.get(), st.ptr.get());
         KERNEL_CHECK();
-        finish_stage(st, src, mat, s);
+        finish_stage(c, st, src, mat, s);
         st.scratch_off = 0;
         max_pairs = std::max<int64_t>(max_pairs, nt);
     }
