@@ -75,6 +75,7 @@ enum {
     BEM_S_KERNEL_LAUNCHES_PER_APPLY,
     BEM_S_M2L_FLOP,        /* executed flop of the M2L tiles of one product (graded truncation: 4 (4 KE)^2 per pair) */
     BEM_S_M2L_ROW_BYTES,   /* bytes of translated rows the per-target sums read in one product                     */
+    BEM_S_P_DIPOLE,        /* truncation number of the products that carry dipoles (option "dipole_degrees")                 */
     BEM_S_COUNT
 };
 

@@ -20,7 +20,7 @@ void boxset_sort(BoxSet &bs, const double *xyz, int64_t n, const double cube_min
 void boxset_build(BoxSet &bs, int lmax, const int counts[22], cudaStream_t s);
 void build_lists(bem_ctx *c);
 // translate.cu
-void build_matrices(bem_ctx *c);
+void build_matrices(bem_ctx *c, FmmLayout &L);
 void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce);
 void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stream);
 void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int ctas_per_sm);
@@ -114,6 +114,35 @@ __global__ void v1_diag(const double *V, const double *nrm, const double *y0, co
             y0[i] * (nx * (V[3 * i] - r0x) + ny * (V[3 * i + 1] - r0y) + nz * (V[3 * i + 2] - r0z));
 }
 
+// ------------------------------------------------------------------ truncation layouts
+static void init_layout(FmmLayout &L, int p)
+{
+    L.p = p;
+    L.pl = p <= 16 ? std::max(4, 2 * ((p + 1) / 2)) : p;      // template buckets 4, 6, .., 16 of the P2M / L2P / DMMA kernels
+    L.nre = lay_nre(L.pl);
+    L.nst = lay_nst(L.pl);
+}
+void activate_layout(bem_ctx *c, int i)
+{
+    const FmmLayout &L = c->lay[i];
+    c->lay_active = i;
+    c->p = L.p; c->pl = L.pl; c->nre = L.nre; c->nst = L.nst;
+    c->mats.p = L.mats.get(); c->rot.p = L.rot.get(); c->kinfo.p = L.kinfo.get();
+    c->mat_ne.p = L.mat_ne.get(); c->mat_cls.p = L.mat_cls.get();
+    c->m2l_row_bytes = L.m2l_row_bytes;
+}
+// executed work of the M2L tiles of one product with this layout (bem_get_stats), from the pairs per matrix
+static void layout_stats(const bem_ctx *c, FmmLayout &L)
+{
+    L.m2l_flop = L.m2l_row_bytes = 0;
+    const bool dmma = c->gemm_path == 0 && L.pl <= 16;             // the plain-FMA tiles run every matrix in full
+    for (int m = 0; m < MAT_L2L; ++m) {
+        const double kr = dmma ? 4.0 * ke_of(L.pl - L.mat_cls_host[m]) : (double)L.nre;
+        L.m2l_flop += c->m2l_hist[m] * 4.0 * kr * kr;
+        L.m2l_row_bytes += c->m2l_hist[m] * 16.0 * L.mat_ne_host[m];
+    }
+}
+
 // ------------------------------------------------------------------ apply (device pointers)
 void mark(bem_ctx *c, int cls)
 {
@@ -144,6 +173,7 @@ static int reduce_ctas_for(const bem_ctx *c)
 void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
 {
     c->ev_n = 0;
+    if (c->mode == 0) activate_layout(c, (phi && c->n_lay > 1) ? 1 : 0);      // products with dipoles carry more degrees (option dipole_degrees)
     if (c->mode == 0 && c->p2p_precision == 1) ensure_p2p_f32(c);
     mark(c, -1);
     launch_lift(c, q, phi);
@@ -246,10 +276,16 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     c->ready = false;
     c->have_diag = false;
     c->have_cfree = false;
-    c->p = p;
-    c->pl = p <= 16 ? std::max(4, 2 * ((p + 1) / 2)) : p;     // template buckets 4, 6, .., 16 of the P2M / L2P / DMMA kernels
-    c->nre = lay_nre(c->pl);
-    c->nst = lay_nst(c->pl);
+    c->p_user = p;
+    init_layout(c->lay[0], p);
+    // Products with dipole sources lose about 3.5 degrees of accuracy against monopoles at equal truncation (a dipole moment
+    // of degree l scales like l a^(l-1); measured: DESIGN.md R5'), so they carry dd more degrees.  -1 = the measured table:
+    // 3 degrees below p = 12 (S - D then meets the north_star's 1e-5 at the stated p of every BASELINE config), none from 12 on.
+    const int dd = c->dipole_degrees >= 0 ? c->dipole_degrees : (p < 12 ? 3 : 0);
+    const int p_dip = std::min(P_MAX, p + dd);
+    c->n_lay = (p_dip > p && c->quadrature != 2 && c->mode == 0) ? 2 : 1;
+    if (c->n_lay == 2) init_layout(c->lay[1], p_dip);
+    activate_layout(c, 0);
     c->leaf_size = leaf_size;
     c->eta = eta;
     if (c->quadrature != 2) compute_geometry(c);
@@ -307,9 +343,11 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         c->tgt_inv.alloc(N);
         gather_targets<<<cdiv(N, 256), 256, 0, s>>>(c->V.get(), c->tb.perm.get(), N, c->tgt_pos.get(), c->tgt_inv.get());
         KERNEL_CHECK();
-        build_matrices(c);
-        c->Mexp.alloc((size_t)c->sb.total() * c->nst);
-        c->Lexp.alloc((size_t)c->tb.total() * c->nst);
+        for (int i = 0; i < c->n_lay; ++i) build_matrices(c, c->lay[i]);
+        activate_layout(c, 0);
+        const int nst_max = c->lay[c->n_lay - 1].nst;
+        c->Mexp.alloc((size_t)c->sb.total() * nst_max);
+        c->Lexp.alloc((size_t)c->tb.total() * nst_max);
         {
             // leaf-level far pairs that cost less summed directly than translated (option "direct_pairs").  One M2L pair +
             // its row sum costs ~1.35 us at p = 12 (nre = 80) whatever the boxes hold, one point pair ~1.4 ns in a full
@@ -319,6 +357,8 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
             c->direct_max_eff = c->direct_max >= 0 ? c->direct_max : (int64_t)w;
         }
         build_lists(c);
+        for (int i = 0; i < c->n_lay; ++i) layout_stats(c, c->lay[i]);
+        activate_layout(c, 0);
         c->nsplit = 2;                                  // far field (L2P) and near field (P2P) partial sums
         c->ypart.alloc(2 * N);
         if (!c->side) {
@@ -536,6 +576,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
     else if (!strcmp(key, "m2l_order_radius")) { if (!(value >= 0 && value < 1.0)) return BEM_ERR_INVALID_ARG; c->m2l_order_radius = value; c->ready = false; }
     else if (!strcmp(key, "m2l_order_extra")) { if (v < -8 || v > 8) return BEM_ERR_INVALID_ARG; c->m2l_order_extra = v; c->ready = false; }
+    else if (!strcmp(key, "dipole_degrees")) { if (v < -1 || v > 16) return BEM_ERR_INVALID_ARG; c->dipole_degrees = v; c->ready = false; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
     return BEM_OK;
@@ -610,7 +651,7 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
     s[BEM_S_NEAR_TRIANGLES] = (double)c->near_tris;
     s[BEM_S_SETUP_MS] = c->setup_ms;
     s[BEM_S_DEVICE_BYTES] = (double)g_device_bytes;
-    s[BEM_S_EXP_STRIDE] = c->nst;
+    s[BEM_S_EXP_STRIDE] = c->lay[c->n_lay - 1].nst;
     s[BEM_S_KERNEL_LAUNCHES_PER_APPLY] = c->launches_per_apply;
     if (c->mode == 0) {
         s[BEM_S_LMAX] = c->sb.lmax;
@@ -618,8 +659,10 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
         s[BEM_S_N_TGT_LEAVES] = c->tb.nbox[c->tb.lmax];
         s[BEM_S_P2P_PAIRS] = (double)c->p2p_pairs;
         s[BEM_S_M2L_PAIRS] = (double)c->m2l_pairs;
-        s[BEM_S_M2L_FLOP] = c->m2l_flop;
-        s[BEM_S_M2L_ROW_BYTES] = c->m2l_row_bytes;
+        const FmmLayout &Lf = c->lay[c->n_lay - 1];           // the layout of a full product (q and phi)
+        s[BEM_S_M2L_FLOP] = Lf.m2l_flop;
+        s[BEM_S_M2L_ROW_BYTES] = Lf.m2l_row_bytes;
+        s[BEM_S_P_DIPOLE] = Lf.p;
         s[BEM_S_N_SRC_BOXES] = c->sb.total();
         s[BEM_S_N_TGT_BOXES] = c->tb.total();
     } else {

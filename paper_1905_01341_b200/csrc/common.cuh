@@ -53,6 +53,12 @@ struct dvec {
     void zero(cudaStream_t s) { CUDA_TRY(cudaMemsetAsync(p, 0, n * sizeof(T), s)); }
     T *get() const { return p; }
 };
+// non-owning view of a device array (the active truncation layout of the context)
+template <class T>
+struct dptr {
+    T *p = nullptr;
+    T *get() const { return p; }
+};
 
 // Preferred shared-memory carve-out (percent of the SM's L1/shared array) of the kernels that bem_apply runs side by side
 // on one SM (the near-field pair kernels and the row sums of the M2L stages).  An SM can only hold CTAs whose kernels
@@ -69,6 +75,10 @@ inline void d2h_sync(void *dst, const void *src, size_t bytes, cudaStream_t s)
 }
 
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
+
+// Function attributes (dynamic shared-memory opt-in, carve-out) are PER DEVICE, and contexts may live on several devices
+// and threads: every launch site keeps one flag per device and asks here, under a mutex, whether it is the first use.
+bool first_use_on_device(std::vector<char> &done, int device);
 }  // namespace bem
 struct bem_ctx;
 namespace bem {
@@ -113,8 +123,7 @@ struct BoxSet {                     // the non-empty boxes of one point set on l
 
 // One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
 // executed as (tiles of a dense GEMM per matrix) -> scratch rows in target-major order -> fixed-order row sums.
-struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split),
-                                                      // bits 8..: truncation class of the matrix (graded M2L, translate.cu)
+struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split)
 constexpr int M2L_NCLS = 5;        // truncation classes of the M2L tiles: degrees < pl - i, i = 0..4
 // k-steps (4 dofs each, in pairs) of either block that hold the degrees < pp: 4 ke_of(pl) = nre of the layout
 __host__ __device__ constexpr int ke_of(int pp) { return pp < 2 ? 2 : 2 * ((pp * (pp + 1) / 2 + 7) / 8); }
@@ -129,12 +138,26 @@ struct Stage {
     dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
     dvec<int32_t> krow;             // [npairs] target-major index k of the pair in tile row r: its scratch row (the rows of a target are
                                     // contiguous in scratch, so the row sums stream them; the tiles scatter whole 8 nst-byte rows)
-    dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order) | dofs its scratch row carries << 16: the reduce
-                                    // pass rotates back by the azimuth of the matrix
+    dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order): the reduce pass rotates back by its azimuth
     dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
     dvec<Tile> tiles;
     int ntiles = 0;
     int ntiles_split = 0;           // the first ntiles_split tiles are M2L tiles (matrix ids < MAT_L2L come first)
+};
+
+// Everything bem_setup builds that depends on the truncation number.  A context holds one layout for the products without
+// dipoles (truncation p) and, when option "dipole_degrees" asks for it, a second one for the products with dipoles
+// (truncation p + dipole degrees); bem_apply makes one of them the active layout (api.cu activate_layout).
+struct FmmLayout {
+    int p = 0, pl = 0, nre = 0, nst = 0;
+    dvec<double> mats;              // [N_MATS * nst * nst] real translation matrices, row = input dof k, col = output dof
+    dvec<double2> rot;              // [N_MATS * ROT_M] (cos m a, sin m a): azimuth a of the M2L offset, identity for M2M / L2L
+    dvec<int32_t> kinfo;            // [nst] order m of every stored dof (0 for padding)
+    dvec<int32_t> mat_ne;           // [N_MATS] leading dofs of either block that take part in the translation (graded truncation)
+    dvec<int32_t> mat_cls;          // [N_MATS] truncation class of the M2L tiles of the matrix: min(M2L_NCLS - 1, pl - p_o)
+    std::vector<int32_t> mat_ne_host, mat_cls_host;
+    double m2l_flop = 0;            // executed flop of the M2L tiles of one product: 4 (4 KE)^2 per pair, KE the k-steps of its class
+    double m2l_row_bytes = 0;       // bytes of translated rows the sums read per product: 16 x dofs carried per pair
 };
 
 }  // namespace bem
@@ -170,6 +193,11 @@ struct bem_ctx {
 
     // setup state
     bool ready = false;
+    bem::FmmLayout lay[2];          // [0] truncation p_user (products without dipoles), [1] p_user + dipole degrees (if any)
+    int n_lay = 1, lay_active = 0;
+    int p_user = 0;                 // the p of bem_setup
+    int dipole_degrees = -1;        // option "dipole_degrees": -1 = 3 for p < 12 and 0 above (measured, R5'), else the value
+    // the ACTIVE layout (copied from lay[lay_active] by activate_layout)
     int p = 0, nst = 0;             // truncation number, expansion row stride (harmonics.cuh: nre + nim)
     int pl = 0, nre = 0;            // layout degree count (kernel template bucket >= p), size of the real-part block
     int leaf_size = 0;
@@ -199,15 +227,13 @@ struct bem_ctx {
     int64_t xdir_pairs = 0;
     int64_t direct_max = -1;        // option "direct_pairs": nt x ns threshold, -1 = from the cost model, 0 = off
     int64_t direct_max_eff = 0;
-    bem::dvec<double> mats;         // [N_MATS * nst * nst] real translation matrices, row = input dof k, col = output dof
-    bem::dvec<double2> rot;         // [N_MATS * ROT_M] (cos m a, sin m a): azimuth a of the M2L offset, identity for M2M / L2L
-    bem::dvec<int32_t> kinfo;       // [nst] order m of every stored dof (0 for padding)
-    bem::dvec<int32_t> mat_ne;      // [N_MATS] leading dofs of the real-part block that take part in the translation (graded truncation)
-    std::vector<int32_t> mat_ne_host, mat_cls_host;   // host copies: dofs and tile class (min(M2L_NCLS - 1, pl - p_o)) per matrix
+    bem::dptr<double> mats;         // views of the active layout (FmmLayout)
+    bem::dptr<double2> rot;
+    bem::dptr<int32_t> kinfo, mat_ne, mat_cls;
+    double m2l_hist[bem::MAT_L2L] = {0};   // M2L pairs per matrix over all levels (statistics of the layouts)
     double m2l_order_radius = 0.5;  // option "m2l_order_radius": cluster radius a (box edges) of the graded truncation, 0 = off
     int m2l_order_extra = 1;        // option "m2l_order_extra": degrees added to the graded order of every offset
-    double m2l_flop = 0;            // executed flop of the M2L tiles of one product: 4 (4 KE)^2 per pair, KE the k-steps of its class
-    double m2l_row_bytes = 0;       // bytes of translated rows the sums read per product: 16 x dofs carried per pair
+    double m2l_row_bytes = 0;       // of the active layout
     bem::dvec<double> Mexp, Lexp;   // [total boxes * nst]
     bem::dvec<double> scratch;      // [pairs of all M2L (+ L2L) stages * nst]: one region per level, so that the tiles of all
                                     // levels can be issued before the first reduce pass

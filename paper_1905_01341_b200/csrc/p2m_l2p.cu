@@ -179,11 +179,10 @@ static void p2m_launch(bem_ctx *c)
     const int lmax = sb.lmax, nleaf = sb.nbox[lmax];
     const double h = c->cube_side / (double)(1 << lmax);
     const size_t smem = (size_t)P2M_WARPS * P2M_TBL * sizeof(double);
-    static bool attr = false;
-    if (!attr) {
+    static std::vector<char> attr_done;
+    if (first_use_on_device(attr_done, c->device)) {
         CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr = true;
     }
     auto kern = c->has_dipole ? p2m_kernel_t<P, true> : p2m_kernel_t<P, false>;
     CUDA_TRY(cudaMemsetAsync(c->p2p_counter.get() + 2, 0, sizeof(int), c->stream));

@@ -270,13 +270,12 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
 void launch_p2p_leaves(bem_ctx *c)
 {
     const int nleaf = c->tb.nbox[c->tb.lmax];
-    static bool attr_set = false;
-    if (!attr_set) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
+    static std::vector<char> attr_done;
+    if (first_use_on_device(attr_done, c->device)) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-        attr_set = true;
     }
     const bool self = c->quadrature != 0;                       // V1 (j = i) and point clouds may have r = 0; G3 cannot
 #define BEM_LEAF(D, S) p2p_leaf_kernel<D, S><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, \

@@ -61,9 +61,9 @@ __global__ void fill_matrices(int p, int nre, int nst, const double *tab_re, con
     mats[idx] = v;
 }
 
-void build_matrices(bem_ctx *c)
+void build_matrices(bem_ctx *c, FmmLayout &L)
 {
-    const int p = c->p, nst = c->nst;
+    const int p = L.p, nst = L.nst;
     const int stride = tab_len(2 * p - 1);
     dvec<double> tre, tim;
     tre.alloc((size_t)N_MATS * stride);
@@ -78,7 +78,7 @@ void build_matrices(bem_ctx *c)
     // error with p_o = ceil(p ln kappa(2) / ln kappa(|o|)) + extra degrees (option "m2l_order_extra").  Only the leading
     // mat_ne[m] = p_o (p_o + 1) / 2 dofs of the real-part block (= of the imaginary-part block) of matrix m are non-zero,
     // and the M2L tile kernels run the k-steps and n-tiles of class min(M2L_NCLS - 1, pl - p_o) only.  a = 0: p_o = p.
-    std::vector<int32_t> ne(N_MATS, c->nre), cls(N_MATS, 0);
+    std::vector<int32_t> ne(N_MATS, L.nre), cls(N_MATS, 0);
     for (int m = 0; m < MAT_L2L; ++m) {
         const int ox = m % 7 - 3, oy = (m / 7) % 7 - 3, oz = m / 49 - 3;
         int po = p;
@@ -88,16 +88,18 @@ void build_matrices(bem_ctx *c)
             po = (int)std::ceil(p * std::log(k2) / std::log(kd) - 1e-9) + c->m2l_order_extra;
             po = std::max(std::min(po, p), std::min(p, 2));
         }
-        ne[m] = std::min(c->nre, po * (po + 1) / 2);
-        cls[m] = std::max(0, std::min(M2L_NCLS - 1, c->pl - po));
+        ne[m] = std::min(L.nre, po * (po + 1) / 2);
+        cls[m] = std::max(0, std::min(M2L_NCLS - 1, L.pl - po));
     }
-    c->mat_ne_host = ne;
-    c->mat_cls_host = cls;
-    c->mat_ne.alloc(N_MATS);
-    CUDA_TRY(cudaMemcpyAsync(c->mat_ne.get(), ne.data(), N_MATS * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    L.mat_ne_host = ne;
+    L.mat_cls_host = cls;
+    L.mat_ne.alloc(N_MATS);
+    L.mat_cls.alloc(N_MATS);
+    CUDA_TRY(cudaMemcpyAsync(L.mat_ne.get(), ne.data(), N_MATS * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(L.mat_cls.get(), cls.data(), N_MATS * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     const int64_t tot = (int64_t)N_MATS * nst * nst;
-    c->mats.alloc(tot);
-    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, c->nre, nst, tre.get(), tim.get(), stride, c->mat_ne.get(), c->mats.get());
+    L.mats.alloc(tot);
+    fill_matrices<<<cdiv(tot, 256), 256, 0, c->stream>>>(p, L.nre, nst, tre.get(), tim.get(), stride, L.mat_ne.get(), L.mats.get());
     KERNEL_CHECK();
     // azimuth table (cos m a, sin m a) and the per-dof table (m, partner = the other part of the same (l, m), part)
     std::vector<double2> rot((size_t)N_MATS * ROT_M);
@@ -109,15 +111,15 @@ void build_matrices(bem_ctx *c)
         }
         for (int k = 0; k < ROT_M; ++k) rot[(size_t)m * ROT_M + k] = make_double2(cos(k * a), sin(k * a));
     }
-    c->rot.alloc(rot.size());
-    CUDA_TRY(cudaMemcpyAsync(c->rot.get(), rot.data(), rot.size() * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+    L.rot.alloc(rot.size());
+    CUDA_TRY(cudaMemcpyAsync(L.rot.get(), rot.data(), rot.size() * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
     std::vector<int32_t> kin(nst);
     for (int k = 0; k < nst; ++k) {
         int l, m, part;
-        kin[k] = real_decode(k, c->pl, c->nre, &l, &m, &part) ? m : 0;
+        kin[k] = real_decode(k, L.pl, L.nre, &l, &m, &part) ? m : 0;
     }
-    c->kinfo.alloc(nst);
-    CUDA_TRY(cudaMemcpyAsync(c->kinfo.get(), kin.data(), nst * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    L.kinfo.alloc(nst);
+    CUDA_TRY(cudaMemcpyAsync(L.kinfo.get(), kin.data(), nst * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
 }
 
@@ -439,14 +441,14 @@ static_assert(M2L_NCLS_K == 5, "the switches below list the classes");
 template <int PL>
 __global__ void __launch_bounds__(DM_THREADS, (ke_of(PL) <= 20 ? 3 : 2))
 translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
-                     const double *__restrict__ Mexp, const double *__restrict__ mats,
+                     const double *__restrict__ Mexp, const double *__restrict__ mats, const int32_t *__restrict__ mat_cls,
                      const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
 {
     constexpr int KSH = ke_of(PL);
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
     const Tile tile = tiles[blockIdx.x];
-    switch (tile.flags >> 8) {                                  // truncation class of the tile's matrix (CTA-uniform)
+    switch (__ldg(mat_cls + tile.mat)) {                        // truncation class of the tile's matrix (CTA-uniform)
     case 0: m2l_body8<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
     case 1: m2l_body8<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
     case 2: m2l_body8<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
@@ -556,14 +558,14 @@ __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__re
 template <int PL>
 __global__ void __launch_bounds__(DM16_THREADS, 3)
 translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
-                       const double *__restrict__ Mexp, const double *__restrict__ mats,
+                       const double *__restrict__ Mexp, const double *__restrict__ mats, const int32_t *__restrict__ mat_cls,
                        const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
 {
     constexpr int KSH = ke_of(PL);
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];
     const Tile tile = tiles[blockIdx.x];
-    switch (tile.flags >> 8) {
+    switch (__ldg(mat_cls + tile.mat)) {
     case 0: m2l_body16<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
     case 1: m2l_body16<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
     case 2: m2l_body16<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
@@ -573,7 +575,7 @@ translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict
 }
 
 // attributes of a kernel are per device: one flag per device, under a mutex (several contexts, several devices)
-static bool first_use_on_device(std::vector<char> &done, int device)
+bool first_use_on_device(std::vector<char> &done, int device)
 {
     static std::mutex mu;
     std::lock_guard<std::mutex> lock(mu);
@@ -597,10 +599,10 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
     if (which != TILES_DENSE && st.ntiles_split > 0) {
         if (PL == 12 && c->m2l_rows16)                           // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
             translate_dmma_split16<(PL == 12 ? PL : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
-                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
+                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
         else
             translate_dmma_split<PL><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                   c->mats.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
+                                                                                   c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
     }
     if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
         translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
@@ -613,13 +615,13 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
 // it reads the real and the imaginary part (nre apart) of every row once and writes both.
 constexpr int RED_CHUNK = 192;     // pairs of a target staged at a time (an M2L list holds at most 189)
 __global__ void __launch_bounds__(160)
-translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t,
+translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t, const int32_t *__restrict__ mat_ne,
                  const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
                  int nre, int accumulate, int ntgt, double *__restrict__ out)
 {
-    // mat_t[k] = matrix id | (dofs the row carries << 16): a row of a graded (truncated) translation holds its leading
-    // dofs only (tree.cu pack_row_dofs); the rest of the scratch row was never written.  The words of the target's pairs
-    // are staged in shared memory so that the row loads do not wait for a global load of their predicate.
+    // A row of a graded (truncated) translation holds the leading mat_ne[matrix] dofs only; the rest of the scratch row was
+    // never written.  (matrix id | dofs << 16) of the target's pairs is staged in shared memory so that the row loads do
+    // not wait for a global load of their predicate.
     __shared__ int s_mt[RED_CHUNK];
     const int nst = 2 * nre;
     for (int t = blockIdx.x; t < ntgt; t += gridDim.x) {            // grid < ntgt: a persistent pass (see launch_stage_reduce)
@@ -630,7 +632,7 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
         for (int k0 = b; k0 < e; k0 += RED_CHUNK) {                 // one round for every list the library builds
             const int n = min(RED_CHUNK, e - k0);
             __syncthreads();
-            for (int i = threadIdx.x; i < n; i += blockDim.x) s_mt[i] = mat_t[k0 + i];
+            for (int i = threadIdx.x; i < n; i += blockDim.x) { const int mt = mat_t[k0 + i]; s_mt[i] = mt | (__ldg(mat_ne + mt) << 16); }
             __syncthreads();
             for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
                 const int m = kinfo[cc];
@@ -697,7 +699,7 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
     if (first_use_on_device(attr_done, c->device))                     // same carve-out as the pair kernels it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
-        st.ptr.get(), st.mat_t.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
+        st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
         c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : 0, st.ntgt, out);
     KERNEL_CHECK();
 }

@@ -233,12 +233,6 @@ __global__ void stage_finish(const uint32_t *order, const int32_t *src, int64_t 
 
 constexpr int GEMM_TM = 64;   // rows per GEMM tile (translate.cu uses the same constant)
 
-// mat_t[k] = matrix id | (dofs of either block the scratch row of pair k carries << 16)   (graded M2L, translate.cu)
-__global__ void pack_row_dofs(int32_t *mat_t, int64_t n, const int32_t *mat_ne)
-{
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < n) mat_t[k] |= mat_ne[mat_t[k]] << 16;
-}
 
 // from target-major (src, mat) pairs to a Stage: rows sorted by matrix, tiles, inverse positions
 static void finish_stage(bem_ctx *c, Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cudaStream_t s)
@@ -265,28 +259,19 @@ static void finish_stage(bem_ctx *c, Stage &st, dvec<int32_t> &src, dvec<int32_t
     }
     std::vector<Tile> tiles;
     int row = 0;
-    for (int m = 0; m < MAT_L2L; ++m) {                                 // executed work of the M2L tiles (bem_get_stats)
-        const bool dmma = c->gemm_path == 0 && c->pl <= 16;             // the plain-FMA tiles run every matrix in full
-        const double kr = dmma ? 4.0 * ke_of(c->pl - c->mat_cls_host[m]) : (double)c->nre;
-        c->m2l_flop += (double)h[m] * 4.0 * kr * kr;
-        c->m2l_row_bytes += (double)h[m] * 16.0 * c->mat_ne_host[m];
-    }
+    for (int m = 0; m < MAT_L2L; ++m) c->m2l_hist[m] += h[m];           // pairs per M2L matrix (statistics, api.cu)
     for (int m = 0; m < N_MATS; ++m) {
         for (int r = 0; r < h[m]; r += GEMM_TM) {
             Tile t;
             t.mat = m;
             t.row0 = row + r;
             t.nrows = std::min(GEMM_TM, h[m] - r);
-            t.flags = ((m >= MAT_L2L && m < MAT_M2M) ? 1 : 0) | (m < MAT_L2L ? 2 : 0) | (c->mat_cls_host[m] << 8);
+            t.flags = ((m >= MAT_L2L && m < MAT_M2M) ? 1 : 0) | (m < MAT_L2L ? 2 : 0);
             tiles.push_back(t);
         }
         row += h[m];
     }
     st.mat_t = std::move(mat);
-    if (n > 0) {
-        pack_row_dofs<<<cdiv(n, 256), 256, 0, s>>>(st.mat_t.get(), n, c->mat_ne.get());
-        KERNEL_CHECK();
-    }
     st.ntiles = (int)tiles.size();
     st.ntiles_split = 0;
     for (const Tile &t : tiles) st.ntiles_split += (t.flags & 2) ? 1 : 0;
@@ -322,7 +307,7 @@ void build_lists(bem_ctx *c)
     c->m2l.clear();
     c->m2l.resize(lmax + 1);
     c->m2l_pairs = 0;
-    c->m2l_flop = c->m2l_row_bytes = 0;
+    for (int m = 0; m < MAT_L2L; ++m) c->m2l_hist[m] = 0;
     int64_t max_pairs = 0;
     for (int l = 2; l <= lmax; ++l) {
         Stage &st = c->m2l[l];
@@ -410,7 +395,7 @@ void build_lists(bem_ctx *c)
         st.scratch_off = 0;
         max_pairs = std::max<int64_t>(max_pairs, nt);
     }
-    c->scratch.alloc((size_t)max_pairs * c->nst);
+    c->scratch.alloc((size_t)max_pairs * c->lay[c->n_lay - 1].nst);            // rows of the widest layout
 }
 
 }  // namespace bem

@@ -127,17 +127,21 @@ def test_direct_tiny_meshes_and_eta(lvl, eta):
 #  * SINGLE layer (monopole sources -- the workload of the paper's Table 1):
 #    within 3x of the value Table 1 prints at that p (1e-5 at p = 8, 5e-7 at p = 12; p = 10 by
 #    geometric interpolation).
-#  * Full operator S - D: dipole sources lose accuracy by the factor ~p/a derived in DESIGN.md
-#    (measured: about 4 degrees), so at the stated p it is held to 1e-4 -- one decade above the
-#    north_star's 1e-5, which is asserted at p + 4 -- and to the north_star's 1e-8 at high p = 24.
+#  * Full operator S - D: the north_star's 1e-5 at the stated p (8, 10, 12) and 1e-8 at high p = 24.
+#    Dipole sources lose accuracy against monopoles at equal truncation (R5': a dipole moment of degree l
+#    scales like l a^(l-1); test_dipole_penalty_is_a_truncation_effect measures it: 3-4 degrees), so the library carries
+#    products WITH dipoles 3 degrees higher below p = 12 (option dipole_degrees = -1, the default).  With
+#    dipole_degrees = 0 -- the paper's convention, one truncation for everything -- the full operator at
+#    p = 8, 10 only reaches TOL_FULL_PAPER_CONVENTION; that reading is NOT the default because it misses the north_star.
 TABLE1 = {4: 7e-4, 8: 1e-5, 10: 2.2e-6, 12: 5e-7, 16: 3e-8, 20: 4e-9}      # tests/golden/table1_fmm_error.txt
 TOL_S = {p: 3.0 * v for p, v in TABLE1.items()}
-TOL_FULL = {8: 1e-4, 10: 1e-4, 12: 1e-4}
+TOL_FULL = {8: 1e-5, 10: 1e-5, 12: 1e-5}                                    # BASELINE.json north_star
+TOL_FULL_PAPER_CONVENTION = 1e-4                                            # dipole_degrees = 0 (measured 1.5e-5 .. 6e-5)
 HIGH_P = 24
 
 
-def _fmm_errors(c, rows, p):
-    ctx = _ctx(c, p=p)
+def _fmm_errors(c, rows, p, **opts):
+    ctx = _ctx(c, p=p, **opts)
     yS = _apply(ctx, c["q"], None)
     yB = _apply(ctx, c["q"], c["phi"])
     eS = _rel(yS[rows], oracle_rows(c, rows, 0, "q", None))
@@ -160,13 +164,44 @@ def test_fmm_stated_p(n):
 
 
 @pytest.mark.parametrize("n", [1, 2, 3])
-def test_fmm_1e5_at_p_plus_4(n):
+def test_fmm_stated_p_paper_convention(n):
+    """dipole_degrees = 0: one truncation number for monopoles and dipoles, as PAPER.md:438 states it.  The single layer
+    is unchanged (Table 1); the full operator stays within a decade of the north_star's figure and reaches it at p + 4."""
     c = cfg(n)
     N = c["V"].shape[0]
     rows = np.arange(N, dtype=np.int64) if N < 3000 else sample_rows(n, N, 2000)
-    eS, eB, _ = _fmm_errors(c, rows, c["p"] + 4)
-    print(f"cfg{n} p={c['p'] + 4}: single layer {eS:.2e}, S-D {eB:.2e}")
-    assert eB <= 1e-5 and eS <= 1e-5
+    eS, eB, st = _fmm_errors(c, rows, c["p"], dipole_degrees=0)
+    eS4, eB4, _ = _fmm_errors(c, rows, c["p"] + 4, dipole_degrees=0)
+    print(f"cfg{n} dipole_degrees=0: p={c['p']}: single layer {eS:.2e}, S-D {eB:.2e}; p={c['p'] + 4}: {eS4:.2e}, {eB4:.2e}")
+    assert st["p_dipole"] == c["p"]
+    assert eS <= TOL_S[c["p"]] and eB <= TOL_FULL_PAPER_CONVENTION
+    assert eB4 <= 1e-5 and eS4 <= 1e-5
+
+
+@pytest.mark.parametrize("n,nb", [(2, None), (3, None), (4, 60)])
+def test_dipole_penalty_is_a_truncation_effect(n, nb):
+    """DESIGN.md R5' as a tested fact.  With ONE truncation number (dipole_degrees = 0) the relative error of the double
+    layer alone (q = NULL) is 5-60x that of the single layer alone (phi = NULL) at every p, both fall at the same rate
+    (2-3x per degree), and the double layer at p + 4 is as accurate as the single layer at p (within 3x) -- a constant
+    shift in p, i.e. truncation, not a defect of the dipole path of P2M (whose formulas test_fmm_operator_chains pins
+    to rounding)."""
+    c = cfg(n) if nb is None else cfg(n, n_bubbles=nb)
+    N = c["V"].shape[0]
+    rows = sample_rows(n, N, 1000)
+    yoS, yoD = oracle_rows(c, rows, 0, "q", None), oracle_rows(c, rows, 0, None, "phi")
+    eS, eD = {}, {}
+    for p in (6, 8, 10, 12, 14):
+        ctx = _ctx(c, p=p, dipole_degrees=0)
+        eS[p] = _rel(_apply(ctx, c["q"], None)[rows], yoS)
+        eD[p] = _rel(_apply(ctx, None, c["phi"])[rows], yoD)
+        ctx.bem_destroy()
+    print(f"cfg{n}: S-only", {p: f"{e:.2e}" for p, e in eS.items()}, "D-only", {p: f"{e:.2e}" for p, e in eD.items()})
+    for p in eS:
+        assert 5.0 <= eD[p] / eS[p] <= 60.0, (p, eD[p] / eS[p])
+    for a, b in ((6, 8), (8, 10), (10, 12), (12, 14)):
+        assert 3.0 <= eS[a] / eS[b] <= 12.0 and 3.0 <= eD[a] / eD[b] <= 12.0, (a, b)
+    for p in (6, 8, 10):
+        assert eD[p + 4] <= 3.0 * eS[p], (p, eD[p + 4], eS[p])
 
 
 @pytest.mark.parametrize("n", [1, 2, 3])
@@ -182,7 +217,10 @@ def test_fmm_high_p(n):
 def test_fmm_error_decays_with_p_like_table1():
     """P9: the truncation convention (degrees 0..p-1) reproduces the decay of the paper's Table 1
      for monopole sources: same order of magnitude (within 5x) as every printed value -- the paper's
-    points fill a cube, ours lie on bubble surfaces, so equality is not expected."""
+    points fill a cube, ours lie on bubble surfaces, so equality is not expected.  The bound is two-sided and 5x because
+    SURVEY.md 8(c) pin P9 asks for "same order of magnitude as PAPER.md:464-471 (Table 1)", not for an upper bound: the
+    first hardware run measured p = 4 at 1.4x ABOVE and p = 16 at 3x BELOW the printed values (surface data converge
+    faster at high p), which a one-sided 3x bound misread as a failure."""
     c = cfg(2)
     rows = sample_rows(2, c["V"].shape[0], 1000)
     errs = {}
@@ -302,7 +340,7 @@ def test_point_cloud_fmm_reproduces_table1():
 
 
 # ------------------------------------------------------------------ full-size configs 4 and 5, as bench.py runs them
-@pytest.mark.parametrize("n,nrows", [(4, 1000), (5, 400)])
+@pytest.mark.parametrize("n,nrows", [(4, 2000), (5, 2000)])
 def test_fmm_full_size_clusters_sampled_rows(n, nrows):
     """BASELINE.json configs 4 (642,000 nodes, p = 10) and 5 (2,568,000 nodes, p = 12) at full size, in the launch
     configuration bench.py times (same leaf_size, device-resident q, phi, y, two streams), on seeded sampled rows the
@@ -323,7 +361,7 @@ def test_fmm_full_size_clusters_sampled_rows(n, nrows):
     e = _rel(y1[rows], oracle_rows(c, rows))
     print(f"cfg{n} full size p={c['p']} lmax {st['lmax']:.0f}: S-D on {nrows} rows {e:.2e}")
     assert np.isfinite(y1).all()
-    assert e <= (3e-5 if n == 4 else 1e-5)                      # p = 10: the dipole penalty of DESIGN.md R5'; p = 12: north_star's 1e-5
+    assert e <= 1e-5                                             # north_star: <= 1e-5 at the stated p
 
 
 # ------------------------------------------------------------------ single-precision near field (option p2p_precision = 1)
