@@ -131,3 +131,28 @@ def monopole_sum(src, m, tgt):
     lib.oracle_monopole_sum(_p(src), _p(m), ctypes.c_int64(src.shape[0]), _p(tgt),
                             ctypes.c_int64(tgt.shape[0]), _p(y))
     return y
+
+
+def point_sum(src, m, d, tgt):
+    """y[r] = sum_j [ m_j / (4 pi |x_r - y_j|) - d_j.(x_r - y_j) / (4 pi |x_r - y_j|^3) ], coincident points skipped
+    (Eq. 13); m [ns] or d [ns, 3] may be None."""
+    lib = _load()
+    src = _f64(src); tgt = _f64(tgt)
+    m = None if m is None else _f64(m)
+    d = None if d is None else _f64(d)
+    y = np.zeros(tgt.shape[0])
+    lib.oracle_point_sum(_p(src), _p(m), _p(d), ctypes.c_int64(src.shape[0]), _p(tgt), ctypes.c_int64(tgt.shape[0]), _p(y))
+    return y
+
+
+def g3_evaluate(V, F, q, phi, X, eta=2.5, return_near=False):
+    """u(x) = S[q](x) - D[phi](x) at points x OFF the surface (Eq. 11), mode G3."""
+    lib = _load()
+    V = _f64(V); F = np.ascontiguousarray(F, dtype=np.int32); X = _f64(X)
+    q = None if q is None else _f64(q)
+    phi = None if phi is None else _f64(phi)
+    y = np.zeros(X.shape[0]); near = np.zeros(X.shape[0], dtype=np.int64)
+    rc = lib.oracle_g3_evaluate(_p(V), ctypes.c_int64(V.shape[0]), _p(F), ctypes.c_int64(F.shape[0]), _p(q), _p(phi),
+                                ctypes.c_double(eta), _p(X), ctypes.c_int64(X.shape[0]), _p(y), _p(near))
+    assert rc == 0
+    return (y, near) if return_near else y

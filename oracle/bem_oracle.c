@@ -23,7 +23,10 @@
  *
  * Pinned by tests/test_oracle_pins.py (sphere eigen-relations, solid-angle
  * identity, closed-form incident weights, brute-force quadrature, V1
- * identities, manufactured exterior fields).  Nothing here is tuned for speed:
+ * identities, manufactured exterior fields; the point sums by the mean-value
+ * property of the sphere, hand-computed cube corners, Gauss' theorem and a
+ * finite difference; the off-surface evaluation by Gauss' theorem and Green's
+ * representation of a manufactured exterior field).  No function is unpinned.  Nothing here is tuned for speed:
  * rows are independent and run under `#pragma omp parallel for`, that is all.
  */
 #include <math.h>
@@ -479,6 +482,80 @@ int oracle_monopole_sum(const double *src, const double *m, int64_t ns,
             ksum_add(&acc, m[j] / (FOUR_PI * sqrt(r2)));
         }
         y[r] = ksum_get(&acc);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* point sums with dipoles (Eq. 13: G and dG/dn with   */
+/* the normal folded into the dipole strength d_j):                     */
+/* y[r] = sum_j [ m_j / (4 pi |x_r - y_j|)                              */
+/*              - d_j . (x_r - y_j) / (4 pi |x_r - y_j|^3) ],           */
+/* coincident points skipped; m or d may be NULL (zero strengths).      */
+/* With m_j = q_j w_j and d_j = phi_j n_j w_j this is the quadrature of */
+/* S[q] - D[phi] over points y_j with weights w_j and normals n_j.      */
+/* ------------------------------------------------------------------ */
+int oracle_point_sum(const double *src, const double *m, const double *d, int64_t ns,
+                     const double *tgt, int64_t nt, double *y)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t r = 0; r < nt; ++r) {
+        ksum acc = {0, 0};
+        for (int64_t j = 0; j < ns; ++j) {
+            double dx[3];
+            sub3(tgt + 3 * r, src + 3 * j, dx);
+            double r2 = dot3(dx, dx);
+            if (r2 == 0.0) continue;
+            double rr = sqrt(r2);
+            double v = 0.0;
+            if (m) v += m[j] / (FOUR_PI * rr);
+            if (d) v -= dot3(d + 3 * j, dx) / (FOUR_PI * r2 * rr);
+            ksum_add(&acc, v);
+        }
+        y[r] = ksum_get(&acc);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* mode G3 at points OFF the surface (Eq. 11, the cases   */
+/* r not on S): u(x) = S[q](x) - D[phi](x) with the same discretisation */
+/* as at the vertices -- 3-point Gauss per triangle with */
+/* P1 densities, and the exact flat-triangle integrals on the near set  */
+/* { k : |x - c_k| <= eta d_k }.  No triangle is incident to x.         */
+/* ------------------------------------------------------------------ */
+int oracle_g3_evaluate(const double *V, int64_t N, const int32_t *F, int64_t T,
+                       const double *q, const double *phi, double eta,
+                       const double *X, int64_t nx, double *y, int64_t *near_count)
+{
+    (void)N;
+    gl_init();
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t r = 0; r < nx; ++r) {
+        const double *x = X + 3 * r;
+        ksum acc = {0.0, 0.0};
+        int64_t nn = 0;
+        for (int64_t k = 0; k < T; ++k) {
+            tri_geom t;
+            tri_geometry(V, F, k, &t);
+            double cS[3], cD[3];
+            gauss3_coeffs(&t, x, cS, cD);
+            double dc[3];
+            sub3(x, t.c, dc);
+            if (dot3(dc, dc) <= eta * eta * t.d2) {
+                exact_weights_regular(&t, x, cS, cD);
+                ++nn;
+            }
+            double v = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                int64_t j = F[3 * k + a];
+                if (q) v += cS[a] * q[j];
+                if (phi) v -= cD[a] * phi[j];
+            }
+            ksum_add(&acc, v);
+        }
+        y[r] = ksum_get(&acc);
+        if (near_count) near_count[r] = nn;
     }
     return 0;
 }

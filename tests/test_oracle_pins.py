@@ -123,13 +123,39 @@ def test_p4_regular_weights_vs_brute_force():
 
 
 def test_p4_gauss3_is_exact_for_quadratics():
-    """The 3-point rule (2/3,1/6,1/6) integrates lambda_a lambda_b exactly:
-    int lambda_a lambda_b = A (1+delta_ab)/12; checked through the far-field limit
-    x -> infinity where G -> 1/(4 pi |x|) is constant over the triangle."""
-    tri = np.array([[0, 0, 0], [1, 0, 0], [0, 2, 0]], float)
-    x = np.array([0, 0, 1e9])
-    cS, _ = oracle.gauss3_coeffs(tri, x)
-    assert np.abs(cS * 4 * np.pi * 1e9 - 1.0 / 3.0).max() < 1e-9     # int lambda_a = A/3, A = 1
+    """The 3-point rule integrates the quadratics lambda_a lambda_b exactly: sum_g w lambda_a(g) lambda_b(g) =
+    A (1 + delta_ab) / 12.  Probed through the far field: for x = R u, 1/|x - y| = (1/R)(1 + u.y/R + O(R^-2)) is a constant
+    plus a LINEAR function of y, so R (4 pi R cS_a - A/3) -> sum_b (u.r_b) sum_g w lambda_a(g) lambda_b(g); the O(1/R)
+    remainder is removed by Richardson extrapolation over R and 2R.  (A rule with sum_g lambda_a(g) = 1 but the wrong
+    second moments -- nodes at (0.6, 0.2, 0.2), say -- passes the zeroth-order check and fails this one by 12%.)"""
+    tri = np.array([[0.3, -0.2, 0.1], [1.4, 0.1, -0.3], [0.2, 2.1, 0.4]], float)
+    A, _ = tri_areas_normals(tri, np.array([[0, 1, 2]]))
+    A = A[0]
+    rng = np.random.default_rng(3)
+    for _ in range(3):
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        f = {}
+        for R in (2e3, 4e3):
+            cS, _ = oracle.gauss3_coeffs(tri, R * u)
+            assert np.abs(cS * 4 * np.pi * R - A / 3.0).max() < 2e-3            # zeroth order: int lambda_a = A/3
+            f[R] = R * (cS * 4 * np.pi * R - A / 3.0)
+        c1 = 2.0 * f[4e3] - f[2e3]
+        M2 = A / 12.0 * (np.ones((3, 3)) + np.eye(3))                            # exact second moments of the hat functions
+        assert np.abs(c1 - M2 @ (tri @ u)).max() < 2e-6 * A
+
+
+def test_p4_gauss3_nodes_and_weights():
+    """Reading R2 pins the rule itself: nodes at the barycentric permutations of (2/3, 1/6, 1/6), weights A/3.  Next to a
+    node y_g the coefficient is dominated by that node: 4 pi eps cS_a(y_g + eps N) -> w_g lambda_a(g)."""
+    tri = np.array([[0.0, 0.0, 0.0], [1.0, 0.2, 0.0], [0.3, 1.5, 0.4]], float)
+    A, Nrm = tri_areas_normals(tri, np.array([[0, 1, 2]]))
+    lam = np.array([[2 / 3, 1 / 6, 1 / 6], [1 / 6, 2 / 3, 1 / 6], [1 / 6, 1 / 6, 2 / 3]])
+    eps = 1e-9
+    for g in range(3):
+        x = lam[g] @ tri + eps * Nrm[0]
+        cS, cD = oracle.gauss3_coeffs(tri, x)
+        assert np.abs(cS * 4 * np.pi * eps - A[0] / 3.0 * lam[g]).max() < 1e-7
+        assert np.abs(cD * 4 * np.pi * eps ** 2 - A[0] / 3.0 * lam[g]).max() < 1e-7   # N.(x - y_g) = eps: dG/dn -> 1/(4 pi eps^2)
 
 
 # ----------------------------------------------------------------- P2
@@ -329,6 +355,122 @@ def test_monopole_sum_matches_definition():
     with np.errstate(divide="ignore"):
         k = np.where(d > 0, 1.0 / (4 * np.pi * d), 0.0)
     assert _rel(y, k @ m) < 1e-14
+
+
+CUBE = np.array([[i, j, k] for i in (0.0, 1.0) for j in (0.0, 1.0) for k in (0.0, 1.0)])
+
+
+def test_point_sums_on_the_cube_corners_by_hand():
+    """Unit monopoles at the 8 corners of the unit cube.  At the centre every corner is at distance sqrt(3)/2:
+    y = 8 / (4 pi sqrt(3)/2) = 4 / (pi sqrt 3).  At a corner (itself skipped: PAPER.md:179, i != j) there are 3 corners at
+    distance 1, 3 at sqrt 2 and 1 at sqrt 3.  A dipole d at the origin seen from x: -d.x / (4 pi |x|^3)."""
+    one = np.ones(8)
+    centre = np.array([[0.5, 0.5, 0.5]])
+    corner_val = (3.0 + 3.0 / np.sqrt(2.0) + 1.0 / np.sqrt(3.0)) / (4 * np.pi)
+    for f in (lambda t: oracle.monopole_sum(CUBE, one, t), lambda t: oracle.point_sum(CUBE, one, None, t)):
+        assert abs(f(centre)[0] - 4.0 / (np.pi * np.sqrt(3.0))) < 1e-15
+        assert np.abs(f(CUBE) - corner_val).max() < 1e-15
+    d = np.zeros((8, 3)); d[0] = [0.0, 0.0, 2.0]                     # one dipole along +z at the origin
+    x = np.array([[0.0, 0.0, 0.5], [0.0, 0.0, -0.5], [1.0, 0.0, 0.0], [3.0, 0.0, 4.0]])
+    expect = np.array([-2.0 * 0.5 / (4 * np.pi * 0.125), +2.0 * 0.5 / (4 * np.pi * 0.125), 0.0, -2.0 * 4.0 / (4 * np.pi * 125.0)])
+    assert np.abs(oracle.point_sum(CUBE, None, d, x) - expect).max() < 1e-15
+    assert np.abs(oracle.point_sum(CUBE, one, d, x) - expect - oracle.monopole_sum(CUBE, one, x)).max() < 1e-15
+
+
+def test_point_sums_mean_value_property_on_the_sphere():
+    """PAPER.md:143 (Eq. 13) integrated over a sphere of radius R with unit density: the single layer is R inside and
+    R^2/|x| outside; the double layer of density 1 (outward normal) is -1 inside and 0 outside (Gauss), so the oracle's
+    -sum d.(x-y)/(4 pi r^3) with d_j = s_j n_j is +1 / 0.  Lumped at the icosphere vertices with the weights of Eq. 17
+    (here s_j, n_j from tests/helpers.py) both converge at second order: the error drops ~4x per level."""
+    R = 1.3
+    xin = np.array([[0.1, -0.2, 0.25], [0.0, 0.0, 0.0], [-0.4, 0.3, 0.1]])
+    xout = np.array([[2.0, 1.0, -0.5], [0.0, 3.0, 0.0]])
+    eS, eD = [], []
+    for lvl in (2, 3, 4):
+        v, F = bi.icosphere(lvl)
+        V = R * v
+        A, Nt = tri_areas_normals(V, F)
+        s = np.zeros(V.shape[0]); mvec = np.zeros_like(V)
+        for a in range(3):
+            np.add.at(s, F[:, a], A / 3.0)
+            np.add.at(mvec, F[:, a], Nt * A[:, None])
+        n = mvec / np.linalg.norm(mvec, axis=1, keepdims=True)
+        for f in (lambda t: oracle.monopole_sum(V, s, t), lambda t: oracle.point_sum(V, s, None, t)):
+            yi, yo = f(xin), f(xout)
+        eS.append(max(np.abs(yi - R).max() / R, np.abs(yo - R * R / np.linalg.norm(xout, axis=1)).max()))
+        assert np.array_equal(oracle.monopole_sum(V, s, xin), oracle.point_sum(V, s, None, xin))
+        d = s[:, None] * n
+        eD.append(max(np.abs(oracle.point_sum(V, None, d, xin) - 1.0).max(), np.abs(oracle.point_sum(V, None, d, xout)).max()))
+    assert eS[0] < 2e-2 and eD[0] < 3e-2
+    for e in (eS, eD):
+        assert 3.0 < e[0] / e[1] < 5.5 and 3.0 < e[1] / e[2] < 5.5, e
+
+
+def test_point_sum_dipole_is_the_derivative_of_the_monopole():
+    """-d.(x - y)/(4 pi |x - y|^3) = -d.grad_y [1/(4 pi |x - y|)]: a central difference of monopole_sum in the source point."""
+    rng = np.random.default_rng(8)
+    src = rng.uniform(0, 1, size=(40, 3)); d = rng.normal(size=(40, 3))
+    tgt = rng.uniform(2, 3, size=(15, 3))
+    h = 1e-4
+    fd = np.zeros(15)
+    for a in range(3):
+        e = np.zeros(3); e[a] = h
+        fd -= (oracle.monopole_sum(src + e, d[:, a], tgt) - oracle.monopole_sum(src - e, d[:, a], tgt)) / (2 * h)
+    y = oracle.point_sum(src, None, d, tgt)
+    assert _rel(fd, y) < 1e-7
+
+
+# ------------------------------------------------------------------ off-surface evaluation (PAPER.md:133, Eq. 11, r not on S)
+def test_evaluate_double_layer_of_one_inside_outside():
+    """Eq. 11 with q = 0, phi = 1: -D[1] = 1 inside the bubble, 0 in the liquid.  With every triangle exact (eta = inf) this
+    is the solid angle of a closed polyhedron: exact to rounding; with eta = 2.5 what is left is the 3-point Gauss error."""
+    V, F = bi.icosphere(2)
+    V = V * np.array([1.0, 0.8, 1.2]) + np.array([0.3, 0.1, -0.2])
+    X = np.array([[0.4, 0.0, -0.1], [0.3, 0.5, 0.3], [0.3, 0.1, 1.6], [2.0, -1.0, 0.5]])
+    one = np.ones(V.shape[0])
+    y, near = oracle.g3_evaluate(V, F, None, one, X, eta=ALL, return_near=True)
+    assert (near == F.shape[0]).all()
+    assert np.abs(y - np.array([1.0, 1.0, 0.0, 0.0])).max() < 1e-13
+    y25, near25 = oracle.g3_evaluate(V, F, None, one, X, eta=ETA, return_near=True)
+    assert (near25 < F.shape[0]).all() and near25[1] > 0
+    assert np.abs(y25 - y).max() < 2e-3
+
+
+def test_evaluate_reproduces_a_manufactured_exterior_field():
+    """Green's representation (Eq. 11): for phi harmonic in the liquid and vanishing at infinity,
+    S[q](x) - D[phi](x) = -phi(x) at x in the liquid and 0 at x inside a bubble, q = d phi/dn with n out of the bubble.
+    phi = field of a point source inside the bubble; the discretisation error is O(h^2): ~4x per refinement."""
+    z = np.array([0.15, -0.1, 0.05])
+    X = np.array([[1.3, 0.2, -0.4], [0.0, -2.0, 1.0], [3.0, 3.0, 3.0], [0.2, 0.1, 0.0], [-0.3, 0.0, 0.2]])
+    inside = np.array([False, False, False, True, True])
+    phi_at = lambda P: 1.0 / (4 * np.pi * np.linalg.norm(P - z, axis=1))
+    errs = []
+    for lvl in (2, 3):
+        V, F = bi.icosphere(lvl)
+        n = V / np.linalg.norm(V, axis=1, keepdims=True)                    # unit sphere: n = r
+        r = V - z
+        q = -(r * n).sum(1) / (4 * np.pi * np.linalg.norm(r, axis=1) ** 3)  # n . grad phi
+        u = oracle.g3_evaluate(V, F, q, phi_at(V), X, eta=ETA)
+        expect = np.where(inside, 0.0, -phi_at(X))
+        errs.append(np.abs(u - expect).max() / np.abs(expect).max())
+    assert errs[0] < 3e-2 and 2.5 < errs[0] / errs[1] < 6.0, errs
+
+
+def test_evaluate_far_from_the_surface_is_the_point_sum_over_gauss_points():
+    """Cross-check of two oracle routines (not a pin): beyond the near radius g3_evaluate is the quadrature sum
+    point_sum over the Gauss points with m = w q(y_g), d = w phi(y_g) N_k."""
+    V, F = bi.icosphere(2)
+    rng = np.random.default_rng(2)
+    q, ph = rng.normal(size=V.shape[0]), rng.normal(size=V.shape[0])
+    lam = np.array([[2 / 3, 1 / 6, 1 / 6], [1 / 6, 2 / 3, 1 / 6], [1 / 6, 1 / 6, 2 / 3]])
+    A, Nt = tri_areas_normals(V, F)
+    Y = np.einsum("ga,tad->tgd", lam, V[F]).reshape(-1, 3)
+    m = (np.einsum("ga,ta->tg", lam, q[F]) * (A / 3.0)[:, None]).reshape(-1)
+    d = ((np.einsum("ga,ta->tg", lam, ph[F]) * (A / 3.0)[:, None])[:, :, None] * Nt[:, None, :]).reshape(-1, 3)
+    X = rng.normal(size=(6, 3)); X = 4.0 * X / np.linalg.norm(X, axis=1, keepdims=True)
+    y, near = oracle.g3_evaluate(V, F, q, ph, X, eta=ETA, return_near=True)
+    assert (near == 0).all()
+    assert _rel(y, oracle.point_sum(Y, m, d, X)) < 1e-13
 
 
 # ------------------------------------------------------------------ surface functions and shape filter (SURVEY.md 8(f) #3)
