@@ -99,14 +99,34 @@ bem_status bem_create(const double *vertices, int64_t n_vertices,
                       const int32_t *bubble_id, bem_ctx **out);
 
 /* bem_create_points -- the same engine on a POINT CLOUD: the workload of the paper's Tables 1-2 (PAPER.md:456-490:
- * "N sources and N receivers distributed randomly and uniformly inside a cube", monopoles).
+ * "N sources and N receivers distributed randomly and uniformly inside a cube", monopoles), and the general point form
+ * of the two kernels of PAPER.md:143-145 (Eq. 13) with monopole AND dipole sources.
  *   sources  [n_sources x 3] fp64 source positions, targets [n_targets x 3] evaluation points (may be the same array).
- * bem_apply(ctx, q, NULL, y) then computes  y_i = sum_j q_j G(x_i, y_j) = sum_j q_j / (4 pi |x_i - y_j|)  over all
- * sources with x_i != y_j:  q is [n_sources], y is [n_targets]; phi must be NULL.  There is no mesh, no correction
- * matrix and no bem_solve in this mode; options "mode", "lmax", "timing", "gemm_path" and bem_setup(p, leaf_size, -)
- * work as for a mesh (near_radius is ignored).  Arrays are copied; host or device pointers. */
+ * bem_apply(ctx, q, d, y) then computes, over all sources with x_i != y_j,
+ *     y_i = sum_j [ q_j / (4 pi |x_i - y_j|)  -  d_j . (x_i - y_j) / (4 pi |x_i - y_j|^3) ],
+ * q: [n_sources] monopole strengths, d (the `phi` argument): [n_sources x 3] row-major dipole VECTORS (d_j = phi_j n_j w_j
+ * is the quadrature of -D[phi] with weights w_j and normals n_j); either may be NULL.  y is [n_targets].  There is no
+ * mesh, no correction matrix and no bem_solve in this mode; options "mode", "lmax", "timing", "gemm_path",
+ * "dipole_degrees" and bem_setup(p, leaf_size, -) work as for a mesh (near_radius is ignored).  Arrays are copied; host
+ * or device pointers. */
 bem_status bem_create_points(const double *sources, int64_t n_sources, const double *targets, int64_t n_targets,
                              bem_ctx **out);
+
+/* bem_create_evaluator -- the potential OFF the surface (Eq. 11, the cases r not on S): for x in the
+ * liquid  S[q](x) - D[phi](x) = -phi(x),  inside a bubble it is 0 -- Green's representation of the field by the surface
+ * data the solver works with.  The new context evaluates
+ *     u(x_t) = S[q](x_t) - D[phi](x_t),   t = 0 .. n_targets-1,
+ * with the SAME discretisation as bem_apply on the mesh (G3: 3-point Gauss per flat triangle with P1 densities, plus the
+ * exact flat-triangle integrals on the near set { k : |x_t - c_k| <= eta d_k } through a CSR correction matrix whose
+ * columns are the mesh vertices), the same octree / FMM engine and the same options.
+ *   mesh_ctx  a context made by bem_create (its mesh is read during bem_setup of the evaluator: it must be alive until
+ *             then; it need not be set up itself).  The evaluator runs on the device and stream of mesh_ctx.
+ *   targets   [n_targets x 3] fp64 points, host or device, copied.  A target ON the surface is not allowed (use
+ *             bem_apply for the vertices); a target closer to a triangle than ~1e-6 of its size loses accuracy.
+ * Then: bem_setup(ev, p, leaf_size, near_radius); bem_apply(ev, q, phi, u) with q, phi [n_vertices of the MESH] and
+ * u [n_targets]; bem_get_stats, bem_set_option, bem_set_stream, bem_destroy as usual.  bem_solve, the surface functions
+ * and option "quadrature" do not apply (BEM_ERR_INVALID_ARG). */
+bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_t n_targets, bem_ctx **out);
 
 /* bem_set_option -- must be called before bem_setup to take effect.
  *   "quadrature"    0 = G3 (default), 1 = V1 (paper's Eq. 17 + Eqs. 19-21)
@@ -175,7 +195,9 @@ bem_status bem_setup(bem_ctx *ctx, int p, int leaf_size, double near_radius);
  * (f, g) = (1, -1)).  q, phi: [n_vertices] fp64, either may be NULL (zero
  * density: that layer is skipped -- f or g = 0).  y: [n_vertices] fp64 output,
  * must not alias q or phi.  No free term (+-1/2 phi) is added.  Asynchronous on
- * the context's stream when all pointers are device pointers. */
+ * the context's stream when all pointers are device pointers.
+ * (Point cloud: q [n_sources], phi = dipole vectors [n_sources x 3], y [n_targets];
+ * evaluator: q, phi [n_vertices of its mesh], y [n_targets] -- see the two creators.) */
 bem_status bem_apply(bem_ctx *ctx, const double *q, const double *phi, double *y);
 
 /* bem_solve -- the Dirichlet problem of PAPER.md:125, 160-171 (Eqs. 15-16):
@@ -210,7 +232,8 @@ bem_status bem_fp64_peak(bem_ctx *ctx, double *gflops_out);
  * "tensor cores (FP64 DMMA) only if ... measured faster" -- this is that measurement. */
 bem_status bem_fp64_tensor_peak(bem_ctx *ctx, double *gflops_out);
 
-/* Last error text of this context (never NULL; valid until the next call). */
+/* Last error text of this context (never NULL; valid until the next call).  ctx == NULL: the message of this thread's
+ * last failed bem_create / bem_create_points / bem_create_evaluator (which return no context to ask). */
 const char *bem_last_error(const bem_ctx *ctx);
 
 /* Free every device allocation of the context.  NULL is allowed. */

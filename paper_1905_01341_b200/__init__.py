@@ -29,7 +29,7 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
               "kernel_launches_per_apply", "m2l_flop", "m2l_row_bytes", "p_dipole"]
 
 # every symbol include/bem.h declares
-EXPORTS = ["bem_create", "bem_create_points", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
+EXPORTS = ["bem_create", "bem_create_points", "bem_create_evaluator", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
            "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy",
            "bem_surface_velocity", "bem_surface_curvature", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy"]
 
@@ -55,6 +55,7 @@ def load_library() -> ctypes.CDLL:
     vp, i64, i32, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_double
     lib.bem_create.argtypes = [vp, i64, vp, i64, vp, ctypes.POINTER(vp)]
     lib.bem_create_points.argtypes = [vp, i64, vp, i64, ctypes.POINTER(vp)]
+    lib.bem_create_evaluator.argtypes = [vp, vp, i64, ctypes.POINTER(vp)]
     lib.bem_set_option.argtypes = [vp, ctypes.c_char_p, dbl]
     lib.bem_set_stream.argtypes = [vp, vp]
     lib.bem_setup.argtypes = [vp, i32, i32, dbl]
@@ -103,9 +104,20 @@ def _ptr(a):
 class Bem:
     """One mesh + its setup: the object the C calls operate on (an owned `bem_ctx *`)."""
 
-    def __init__(self, vertices, triangles, bubble_id=None, _points=None):
+    def __init__(self, vertices, triangles, bubble_id=None, _points=None, _evaluator=None):
         self._lib = load_library()
         self._ctx = ctypes.c_void_p(0)
+        if _evaluator is not None:                   # bem_create_evaluator(mesh_ctx, targets)
+            mesh, T = _evaluator[0], np.ascontiguousarray(_evaluator[1], dtype=np.float64)
+            if T.ndim != 2 or T.shape[1] != 3:
+                raise ValueError("targets must be [n,3]")
+            self._mesh = mesh                        # keeps the mesh context alive
+            self.n_vertices, self.n_triangles, self.n_sources = T.shape[0], 0, 3 * mesh.n_triangles
+            st = self._lib.bem_create_evaluator(mesh._ctx, T.ctypes.data, T.shape[0], ctypes.byref(self._ctx))
+            if st != BEM_OK:
+                self._ctx = ctypes.c_void_p(0)
+                raise BemError(st, self._lib.bem_last_error(None).decode())
+            return
         if _points is not None:                      # bem_create_points(sources, targets)
             S = np.ascontiguousarray(_points[0], dtype=np.float64)
             T = np.ascontiguousarray(_points[1], dtype=np.float64)
@@ -115,7 +127,7 @@ class Bem:
             st = self._lib.bem_create_points(S.ctypes.data, S.shape[0], T.ctypes.data, T.shape[0], ctypes.byref(self._ctx))
             if st != BEM_OK:
                 self._ctx = ctypes.c_void_p(0)
-                raise BemError(st, "bem_create_points failed (a CUDA device is required)")
+                raise BemError(st, "bem_create_points failed (a CUDA device is required): " + self._lib.bem_last_error(None).decode())
             return
         V = np.ascontiguousarray(vertices, dtype=np.float64)
         F = np.ascontiguousarray(triangles, dtype=np.int32)
@@ -127,7 +139,8 @@ class Bem:
                                   None if B is None else B.ctypes.data, ctypes.byref(self._ctx))
         if st != BEM_OK:
             self._ctx = ctypes.c_void_p(0)
-            raise BemError(st, "bem_create failed (mesh must be a closed, outward-oriented manifold; a CUDA device is required)")
+            raise BemError(st, "bem_create failed (mesh must be a closed, outward-oriented manifold; a CUDA device is required): "
+                           + self._lib.bem_last_error(None).decode())
 
     # -- the C calls, same names --------------------------------------------------
     def _check(self, st, allow=()):
@@ -210,8 +223,14 @@ def bem_create(vertices, triangles, bubble_id=None) -> Bem:
 
 
 def bem_create_points(sources, targets) -> Bem:
-    """Point-cloud mode (include/bem.h): bem_apply(q[n_sources], None, y[n_targets])."""
+    """Point-cloud mode (include/bem.h): bem_apply(q[n_sources], d[n_sources, 3] or None, y[n_targets])."""
     return Bem(None, None, None, _points=(sources, targets))
+
+
+def bem_create_evaluator(mesh_ctx: Bem, targets) -> Bem:
+    """Off-surface evaluation of S[q] - D[phi] of a mesh context (include/bem.h): after bem_setup,
+    bem_apply(q[n_vertices of the mesh], phi[...], u[n_targets])."""
+    return Bem(None, None, None, _evaluator=(mesh_ctx, targets))
 
 
 class BemFilter:

@@ -35,6 +35,8 @@ void launch_spmv_combine(bem_ctx *c, const double *q, const double *phi, double 
 void launch_p2p_leaves_f32(bem_ctx *c, cudaStream_t stream, int ctas_per_sm, int leaf0, int leaf1, int part);
 void ensure_p2p_f32(bem_ctx *c);
 
+const bem_ctx *mesh_of(const bem_ctx *c) { return c->parent ? c->parent : c; }
+
 bool is_device_ptr(const void *p)
 {
     if (!p) return true;
@@ -283,14 +285,22 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     // 3 degrees below p = 12 (S - D then meets the north_star's 1e-5 at the stated p of every BASELINE config), none from 12 on.
     const int dd = c->dipole_degrees >= 0 ? c->dipole_degrees : (p < 12 ? 3 : 0);
     const int p_dip = std::min(P_MAX, p + dd);
-    c->n_lay = (p_dip > p && c->quadrature != 2 && c->mode == 0) ? 2 : 1;
+    c->n_lay = (p_dip > p && c->mode == 0) ? 2 : 1;
     if (c->n_lay == 2) init_layout(c->lay[1], p_dip);
     activate_layout(c, 0);
     c->leaf_size = leaf_size;
     c->eta = eta;
-    if (c->quadrature != 2) compute_geometry(c);
+    if (c->quadrature < 2) compute_geometry(c);
+    if (c->quadrature == 3 && !c->parent->triA.p) {              // an evaluator uses the areas and normals of its parent's mesh
+        CUDA_TRY(cudaSetDevice(c->parent->device));
+        const cudaStream_t ps = c->parent->stream;
+        c->parent->stream = s;
+        compute_geometry(c->parent);
+        c->parent->stream = ps;
+        CUDA_TRY(cudaStreamSynchronize(s));
+    }
     const int64_t N = c->N;
-    c->ns = c->quadrature == 0 ? 3 * c->T : (c->quadrature == 2 ? c->np : N);
+    c->ns = (c->quadrature == 0 || c->quadrature == 3) ? 3 * mesh_of(c)->T : (c->quadrature == 2 ? c->np : N);
 
     {
         // unit-cube scaling (reading R11): cube centred on the bounding box, side = largest extent (1 + 1e-9)
@@ -299,9 +309,10 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         bbox3(c->V.get(), N, bb.get(), s);
         double hb[6];
         d2h_sync(hb, bb.get(), sizeof hb, s);
-        if (c->quadrature == 2) {                           // the cube holds sources and targets
+        if (c->quadrature >= 2) {                           // the cube holds sources and targets
             double hs[6];
-            bbox3(c->P.get(), c->np, bb.get(), s);
+            if (c->quadrature == 2) bbox3(c->P.get(), c->np, bb.get(), s);
+            else bbox3(c->parent->V.get(), c->parent->N, bb.get(), s);          // Gauss points lie inside the box of the vertices
             d2h_sync(hs, bb.get(), sizeof hs, s);
             for (int d = 0; d < 3; ++d) { hb[d] = std::min(hb[d], hs[d]); hb[3 + d] = std::max(hb[3 + d], hs[3 + d]); }
         }
@@ -378,10 +389,11 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         c->launches_per_apply = launches;
     }
 
-    if (c->quadrature == 0) build_correction(c);
+    if (c->quadrature == 0 || c->quadrature == 3) build_correction(c);
     else build_empty_correction(c);
+    if (c->mode == 0 && c->p2p_precision == 1) ensure_p2p_f32(c);
     c->ready = true;
-    if (c->quadrature == 2) {                               // point cloud: no free term, no solve
+    if (c->quadrature >= 2) {                               // point cloud, evaluator: no free term, no solve
         CUDA_TRY(cudaStreamSynchronize(s));
         c->setup_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
         return;
@@ -392,8 +404,11 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     y0.alloc(N);
     fill_const<<<cdiv(N, 256), 256, 0, s>>>(ones.get(), N, 1.0);
     KERNEL_CHECK();
-    const int timing = c->timing;
-    c->timing = 0;
+    struct TimingOff {                                           // products made inside bem_setup are not timed; restored on every exit
+        bem_ctx *c; int saved;
+        explicit TimingOff(bem_ctx *cc) : c(cc), saved(cc->timing) { c->timing = 0; }
+        ~TimingOff() { c->timing = saved; }
+    } timing_off(c);
     if (c->quadrature == 1) {
         // the paper's four products for the singular diagonal, pair j = i skipped
         dvec<double> sv, nrm, qv, pv, ya[3];
@@ -428,7 +443,6 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         KERNEL_CHECK();
     }
     CUDA_TRY(cudaStreamSynchronize(s));
-    c->timing = timing;
     c->have_cfree = true;
     c->setup_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
 }
@@ -492,6 +506,9 @@ static double time_loop(bem_ctx *c, K kern, double flop_per_thread_iter)
 
 using namespace bem;
 
+// message of this thread's last failed bem_create / bem_create_points / bem_create_evaluator (no context exists to hold it)
+static thread_local std::string g_create_error = "null context";
+
 extern "C" {
 
 bem_status bem_create(const double *vertices, int64_t n_vertices, const int32_t *triangles, int64_t n_triangles,
@@ -520,9 +537,7 @@ bem_status bem_create(const double *vertices, int64_t n_vertices, const int32_t 
         validate_mesh(c);
     });
     if (st != BEM_OK) {
-        // keep the message reachable for the binding through a static buffer
-        static thread_local std::string last;
-        last = c->err;
+        g_create_error = c->err;                                  // bem_last_error(NULL) returns it (this thread's last failed create)
         delete c;
         return st;
     }
@@ -551,7 +566,30 @@ bem_status bem_create_points(const double *sources, int64_t n_sources, const dou
         CUDA_TRY(cudaMemcpy(c->V.get(), targets, 3 * c->N * sizeof(double), cudaMemcpyDefault));
         CUDA_TRY(cudaMemcpy(c->P.get(), sources, 3 * c->np * sizeof(double), cudaMemcpyDefault));
     });
-    if (st != BEM_OK) { delete c; return st; }
+    if (st != BEM_OK) { g_create_error = c->err; delete c; return st; }
+    *out = c;
+    return BEM_OK;
+}
+
+bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_t n_targets, bem_ctx **out)
+{
+    if (!out) return BEM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!mesh_ctx || !targets || n_targets < 1 || n_targets > 2000000000ll) return BEM_ERR_INVALID_ARG;
+    if (mesh_ctx->quadrature >= 2 || mesh_ctx->T == 0) { mesh_ctx->err = "bem_create_evaluator: the context holds no mesh"; return BEM_ERR_INVALID_ARG; }
+    bem_ctx *c = new (std::nothrow) bem_ctx();
+    if (!c) return BEM_ERR_OOM;
+    c->device = mesh_ctx->device;
+    c->stream = mesh_ctx->stream;
+    c->parent = mesh_ctx;
+    c->N = n_targets;
+    c->T = 0;
+    c->quadrature = 3;
+    bem_status st = guarded(c, [&]() {
+        c->V.alloc(3 * c->N);
+        CUDA_TRY(cudaMemcpy(c->V.get(), targets, 3 * c->N * sizeof(double), cudaMemcpyDefault));
+    });
+    if (st != BEM_OK) { g_create_error = c->err; delete c; return st; }
     *out = c;
     return BEM_OK;
 }
@@ -562,7 +600,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     const int v = (int)value;
     drop_graphs(c);
     if (!strcmp(key, "graph")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->use_graph = v; return BEM_OK; }
-    if (!strcmp(key, "quadrature")) { if ((v != 0 && v != 1) || c->quadrature == 2) return BEM_ERR_INVALID_ARG; c->quadrature = v; c->ready = false; }
+    if (!strcmp(key, "quadrature")) { if ((v != 0 && v != 1) || c->quadrature >= 2) return BEM_ERR_INVALID_ARG; c->quadrature = v; c->ready = false; }
     else if (!strcmp(key, "mode")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->mode = v; c->ready = false; }
     else if (!strcmp(key, "free_term")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->free_term = v; c->ready = false; }
     else if (!strcmp(key, "gmres_restart")) { if (v < 0) return BEM_ERR_INVALID_ARG; c->gmres_restart = v; }
@@ -571,7 +609,13 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "reduce_ctas")) { if (v < 0 || v > 32) return BEM_ERR_INVALID_ARG; c->reduce_ctas = v; }
     else if (!strcmp(key, "m2l_rows16")) { c->m2l_rows16 = v != 0; }
     else if (!strcmp(key, "precond")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->precond = v; }
-    else if (!strcmp(key, "p2p_precision")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->p2p_precision = v; }
+    else if (!strcmp(key, "p2p_precision")) {
+        if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG;
+        c->p2p_precision = v;
+        // the fp32 source records are built HERE (or at the end of bem_setup), never inside a product: a product may run
+        // inside a stream capture of the caller, where an allocation is not allowed
+        if (v == 1 && c->ready && c->mode == 0) return guarded(c, [&]() { ensure_p2p_f32(c); CUDA_TRY(cudaStreamSynchronize(c->stream)); });
+    }
     else if (!strcmp(key, "direct_pairs")) { if (value < -1 || value > 1e9) return BEM_ERR_INVALID_ARG; c->direct_max = (int64_t)value; c->ready = false; }
     else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
     else if (!strcmp(key, "m2l_order_radius")) { if (!(value >= 0 && value < 1.0)) return BEM_ERR_INVALID_ARG; c->m2l_order_radius = value; c->ready = false; }
@@ -605,15 +649,17 @@ bem_status bem_apply(bem_ctx *c, const double *q, const double *phi, double *y)
     if (!c || !y) return BEM_ERR_INVALID_ARG;
     if (!c->ready) { c->err = "bem_apply before bem_setup"; return BEM_ERR_NOT_SETUP; }
     if (y == q || y == phi) { c->err = "bem_apply: y aliases an input"; return BEM_ERR_INVALID_ARG; }
-    if (c->quadrature == 2 && phi) { c->err = "bem_apply: a point cloud carries monopoles only (phi must be NULL)"; return BEM_ERR_INVALID_ARG; }
     return guarded(c, [&]() {
+        // lengths: q, phi are per mesh vertex (an evaluator: of its parent's mesh); a point cloud takes one monopole and
+        // one dipole VECTOR per source; y is per target
         const size_t bytes = c->N * sizeof(double);
-        const size_t qbytes = (c->quadrature == 2 ? c->np : c->N) * sizeof(double);
+        const size_t nq = c->quadrature == 2 ? c->np : mesh_of(c)->N, nphi = c->quadrature == 2 ? 3 * c->np : mesh_of(c)->N;
+        const size_t qbytes = nq * sizeof(double), pbytes = nphi * sizeof(double);
         const bool hq = !is_device_ptr(q), hp = !is_device_ptr(phi), hy = !is_device_ptr(y);
         const double *dq = q, *dp = phi;
         double *dy = y;
-        if (hq) { if (!c->stage_q.p) c->stage_q.alloc(qbytes / sizeof(double)); CUDA_TRY(cudaMemcpyAsync(c->stage_q.get(), q, qbytes, cudaMemcpyHostToDevice, c->stream)); dq = c->stage_q.get(); }
-        if (hp) { if (!c->stage_phi.p) c->stage_phi.alloc(c->N); CUDA_TRY(cudaMemcpyAsync(c->stage_phi.get(), phi, bytes, cudaMemcpyHostToDevice, c->stream)); dp = c->stage_phi.get(); }
+        if (hq) { if (!c->stage_q.p) c->stage_q.alloc(nq); CUDA_TRY(cudaMemcpyAsync(c->stage_q.get(), q, qbytes, cudaMemcpyHostToDevice, c->stream)); dq = c->stage_q.get(); }
+        if (hp) { if (!c->stage_phi.p) c->stage_phi.alloc(nphi); CUDA_TRY(cudaMemcpyAsync(c->stage_phi.get(), phi, pbytes, cudaMemcpyHostToDevice, c->stream)); dp = c->stage_phi.get(); }
         if (hy) { if (!c->stage_y.p) c->stage_y.alloc(c->N); dy = c->stage_y.get(); }
         if (hq || hp || hy) apply_device(c, dq, dp, dy);
         else apply_device_cached(c, dq, dp, dy);
@@ -694,7 +740,7 @@ bem_status bem_fp64_tensor_peak(bem_ctx *c, double *gflops_out)
     return guarded(c, [&]() { *gflops_out = time_loop(c, dmma_loop, 8.0 * 512.0 / 32.0); });
 }
 
-const char *bem_last_error(const bem_ctx *c) { return c ? c->err.c_str() : "null context"; }
+const char *bem_last_error(const bem_ctx *c) { return c ? c->err.c_str() : g_create_error.c_str(); }
 
 void bem_destroy(bem_ctx *c)
 {

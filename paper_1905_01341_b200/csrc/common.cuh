@@ -82,6 +82,7 @@ bool first_use_on_device(std::vector<char> &done, int device);
 }  // namespace bem
 struct bem_ctx;
 namespace bem {
+const bem_ctx *mesh_of(const bem_ctx *c);     // the context that owns the mesh: c itself, or the parent of an evaluator
 // with option "timing": record an event on the context's stream; the time since the previous mark is charged to cls
 void mark(bem_ctx *c, int cls);
 
@@ -176,12 +177,15 @@ struct bem_ctx {
     bem::dvec<int32_t> bid;         // [N]
     bem::dvec<double> P;            // point-cloud mode (quadrature == 2): [np*3] source points; V holds the targets
     int64_t np = 0;
+    bem_ctx *parent = nullptr;      // evaluator (quadrature == 3, bem_create_evaluator): the mesh context whose Gauss points are the
+                                    // sources; V holds the evaluation points (N of them), densities are indexed by the parent's vertices
 
     // vertex -> incident triangle corners, sorted by vertex (bem_surface_velocity; built at first use)
     bem::dvec<int32_t> vc_begin;    // [N+1]
     bem::dvec<uint32_t> vc_corner;  // [3T] corner index 3 k + a, in mesh order within a vertex
 
     // options
+    // quadrature: 0 = G3, 1 = V1, 2 = point cloud (bem_create_points), 3 = evaluator of a mesh context off its surface
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
     int precond = 0;                // bem_solve: 0 = unpreconditioned (the paper), 1 = right diagonal scaling by S_ii
     int reduce_ctas = 0;            // option "reduce_ctas": CTAs per SM of the persistent side-stream sums, 0 = from the cost model

@@ -210,13 +210,14 @@ __global__ void build_sources_points(const double *P, const uint32_t *order, int
 void build_sources(bem_ctx *c, const uint32_t *order)
 {
     cudaStream_t s = c->stream;
-    c->ns = c->quadrature == 0 ? 3 * c->T : (c->quadrature == 2 ? c->np : c->N);
+    const bem_ctx *mc = mesh_of(c);
+    c->ns = (c->quadrature == 0 || c->quadrature == 3) ? 3 * mc->T : (c->quadrature == 2 ? c->np : c->N);
     c->src_pos.alloc(c->ns);
     c->lift_w.alloc(c->ns);
     c->lift_vid.alloc(c->ns);
     c->src_str.alloc(c->ns);
-    if (c->quadrature == 0) {
-        build_sources_g3<<<cdiv(c->ns, 256), 256, 0, s>>>(c->V.get(), c->F.get(), c->triA.get(), c->triN.get(), order,
+    if (c->quadrature == 0 || c->quadrature == 3) {
+        build_sources_g3<<<cdiv(c->ns, 256), 256, 0, s>>>(mc->V.get(), mc->F.get(), mc->triA.get(), mc->triN.get(), order,
                                                           c->ns, c->src_pos.get(), c->lift_w.get(), c->lift_vid.get());
         KERNEL_CHECK();
     } else if (c->quadrature == 2) {
@@ -253,9 +254,10 @@ __global__ void source_points_g3(const double *V, const int32_t *F, int64_t T, d
 }
 void source_points(bem_ctx *c, dvec<double> &xyz)
 {
-    if (c->quadrature == 0) {
-        xyz.alloc(9 * c->T);
-        source_points_g3<<<cdiv(3 * c->T, 256), 256, 0, c->stream>>>(c->V.get(), c->F.get(), c->T, xyz.get());
+    if (c->quadrature == 0 || c->quadrature == 3) {
+        const bem_ctx *mc = mesh_of(c);
+        xyz.alloc(9 * mc->T);
+        source_points_g3<<<cdiv(3 * mc->T, 256), 256, 0, c->stream>>>(mc->V.get(), mc->F.get(), mc->T, xyz.get());
         KERNEL_CHECK();
     } else if (c->quadrature == 2) {
         xyz.alloc(3 * c->np);

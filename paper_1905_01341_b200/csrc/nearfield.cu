@@ -157,10 +157,13 @@ __device__ __forceinline__ int64_t lower_bound_u64(const uint64_t *a, int64_t n,
 }
 
 // pass 0: count the near triangles of vertex i; pass 1: write them at near[ptr[i]..]
-__global__ void near_search(const double *V, const int32_t *F, const double *cen, const double *d2, int64_t N, int64_t T,
-                            Grid g, const uint64_t *cell_sorted, const uint32_t *tri_sorted, double eta2,
+// X: the N collocation / evaluation points.  self: they are the vertices of the mesh (a triangle is near its own vertices
+// whatever the distance); an evaluator's points lie off the surface and have no incident triangle.
+__global__ void near_search(const double *X, const int32_t *F, const double *cen, const double *d2, int64_t N, int64_t T,
+                            Grid g, const uint64_t *cell_sorted, const uint32_t *tri_sorted, double eta2, bool self,
                             int32_t *count, const int64_t *ptr, int32_t *near)
 {
+    const double *V = X;
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const double x[3] = {V[3 * i], V[3 * i + 1], V[3 * i + 2]};
@@ -174,7 +177,7 @@ __global__ void near_search(const double *V, const int32_t *F, const double *cen
             const int64_t b = lower_bound_u64(cell_sorted, T, lo), e = lower_bound_u64(cell_sorted, T, hi + 1);
             for (int64_t j = b; j < e; ++j) {
                 const int64_t k = tri_sorted[j];
-                const bool inc = (F[3 * k] == i) || (F[3 * k + 1] == i) || (F[3 * k + 2] == i);
+                const bool inc = self && ((F[3 * k] == i) || (F[3 * k + 1] == i) || (F[3 * k + 2] == i));
                 double dc[3];
                 for (int d = 0; d < 3; ++d) dc[d] = __dadd_rn(x[d], -cen[3 * k + d]);
                 if (inc || dot3_rn(dc, dc) <= __dmul_rn(eta2, d2[k])) {
@@ -207,7 +210,7 @@ __global__ void csr_count(const int32_t *F, const int64_t *nptr, const int32_t *
 
 // fill row i: columns in order of first appearance, values = sum over near triangles of
 // (exact - Gauss) weights of the matching local vertex
-__global__ void csr_fill(const double *V, const int32_t *F, const double *A, const double *Nrm,
+__global__ void csr_fill(const double *X, bool self, const double *V, const int32_t *F, const double *A, const double *Nrm,
                          const int64_t *nptr, const int32_t *near, int64_t N,
                          const int64_t *rowptr, int32_t *col, double2 *val, double *diagS)
 {
@@ -217,7 +220,7 @@ __global__ void csr_fill(const double *V, const int32_t *F, const double *A, con
     const int64_t r0 = rowptr[i];
     int ncol = 0;
     double sii = 0.0;                                            // S_ii = exact integral of vertex i's own hat function
-    const double x[3] = {V[3 * i], V[3 * i + 1], V[3 * i + 2]};
+    const double x[3] = {X[3 * i], X[3 * i + 1], X[3 * i + 2]};
     for (int64_t j = b; j < e; ++j) {
         const int64_t k = near[j];
         const int v[3] = {F[3 * k], F[3 * k + 1], F[3 * k + 2]};
@@ -226,7 +229,7 @@ __global__ void csr_fill(const double *V, const int32_t *F, const double *A, con
             for (int d = 0; d < 3; ++d) r[a][d] = V[3 * (int64_t)v[a] + d];
         int inc = -1;
         for (int a = 0; a < 3; ++a)
-            if (v[a] == i) inc = a;
+            if (self && v[a] == i) inc = a;
         double WS[3], WD[3];
         if (inc >= 0) { tri_weights_incident(r, inc, WS, WD); sii += WS[inc]; }
         else tri_weights_regular(r, x, WS, WD);
@@ -258,22 +261,24 @@ __global__ void csr_fill(const double *V, const int32_t *F, const double *A, con
             val[r0 + c] = cur;
         }
     }
-    diagS[i] = sii;
+    if (diagS) diagS[i] = sii;
 }
 
 void build_correction(bem_ctx *c)
 {
     cudaStream_t s = c->stream;
-    const int64_t N = c->N, T = c->T;
+    const bem_ctx *mc = mesh_of(c);                                  // an evaluator corrects against its parent's mesh
+    const bool self = mc == c;
+    const int64_t N = c->N, T = mc->T;
     dvec<double> cen, d2;
     cen.alloc(3 * T);
     d2.alloc(T);
-    tri_centroids<<<cdiv(T, 256), 256, 0, s>>>(c->V.get(), c->F.get(), T, cen.get(), d2.get());
+    tri_centroids<<<cdiv(T, 256), 256, 0, s>>>(mc->V.get(), mc->F.get(), T, cen.get(), d2.get());
     KERNEL_CHECK();
     const double d2max = reduce_max(d2.get(), T, s);
     dvec<double> bb;
     bb.alloc(6);
-    bbox3(c->V.get(), N, bb.get(), s);
+    bbox3(mc->V.get(), mc->N, bb.get(), s);
     double hb[6];
     d2h_sync(hb, bb.get(), sizeof hb, s);
     Grid g;
@@ -300,7 +305,7 @@ void build_correction(bem_ctx *c)
     dvec<int64_t> nptr;
     cnt.alloc(N);
     nptr.alloc(N + 1);
-    near_search<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), c->F.get(), cen.get(), d2.get(), N, T, g, keys.get(), tri.get(), eta2,
+    near_search<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), mc->F.get(), cen.get(), d2.get(), N, T, g, keys.get(), tri.get(), eta2, self,
                                              cnt.get(), nullptr, nullptr);
     KERNEL_CHECK();
     scan_exclusive_i64(cnt.get(), nptr.get(), N, s);
@@ -309,19 +314,19 @@ void build_correction(bem_ctx *c)
     c->near_tris = nnear;
     dvec<int32_t> near;
     near.alloc(nnear);
-    near_search<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), c->F.get(), cen.get(), d2.get(), N, T, g, keys.get(), tri.get(), eta2,
+    near_search<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), mc->F.get(), cen.get(), d2.get(), N, T, g, keys.get(), tri.get(), eta2, self,
                                              nullptr, nptr.get(), near.get());
     KERNEL_CHECK();
-    csr_count<<<cdiv(N, 128), 128, 0, s>>>(c->F.get(), nptr.get(), near.get(), N, cnt.get());
+    csr_count<<<cdiv(N, 128), 128, 0, s>>>(mc->F.get(), nptr.get(), near.get(), N, cnt.get());
     KERNEL_CHECK();
     c->rowptr.alloc(N + 1);
     scan_exclusive_i64(cnt.get(), c->rowptr.get(), N, s);
     d2h_sync(&c->nnz, c->rowptr.get() + N, sizeof(int64_t), s);
     c->col.alloc(c->nnz);
     c->val.alloc(c->nnz);
-    c->diagS.alloc(N);
-    csr_fill<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), c->F.get(), c->triA.get(), c->triN.get(), nptr.get(), near.get(), N,
-                                          c->rowptr.get(), c->col.get(), c->val.get(), c->diagS.get());
+    if (self) c->diagS.alloc(N);
+    csr_fill<<<cdiv(N, 128), 128, 0, s>>>(c->V.get(), self, mc->V.get(), mc->F.get(), mc->triA.get(), mc->triN.get(), nptr.get(), near.get(), N,
+                                          c->rowptr.get(), c->col.get(), c->val.get(), self ? c->diagS.get() : nullptr);
     KERNEL_CHECK();
     CUDA_TRY(cudaStreamSynchronize(s));
 }

@@ -32,11 +32,31 @@ __global__ void lift_kernel(const double *__restrict__ q, const double *__restri
     if (strf) strf[s] = make_float4((float)(w.x * qq * ih), (float)(w.y * ff * ih * ih), (float)(w.z * ff * ih * ih), (float)(w.w * ff * ih * ih));
 }
 
+// point cloud (bem_create_points): source j carries the monopole q[j] and the dipole vector (dip[3j], dip[3j+1], dip[3j+2])
+__global__ void lift_points_kernel(const double *__restrict__ q, const double *__restrict__ dip, const int4 *__restrict__ lv, int64_t ns,
+                                   double4 *__restrict__ str, float4 *__restrict__ strf, double ih)
+{
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= ns) return;
+    const int64_t j = lv[s].x;
+    const double m = q ? q[j] : 0.0;
+    double dx = 0.0, dy = 0.0, dz = 0.0;
+    if (dip) { dx = dip[3 * j]; dy = dip[3 * j + 1]; dz = dip[3 * j + 2]; }
+    str[s] = make_double4(m, dx, dy, dz);
+    if (strf) strf[s] = make_float4((float)(m * ih), (float)(dx * ih * ih), (float)(dy * ih * ih), (float)(dz * ih * ih));
+}
+
 void launch_lift(bem_ctx *c, const double *q, const double *phi)
 {
     c->has_dipole = phi != nullptr;                 // the pair and P2M kernels skip the dipole terms otherwise
     const bool f32 = c->mode == 0 && c->p2p_precision == 1;
     const double ih = f32 ? (double)(1u << c->sb.lmax) / c->cube_side : 0.0;
+    if (c->quadrature == 2) {
+        lift_points_kernel<<<cdiv(c->ns, 256), 256, 0, c->stream>>>(q, phi, c->lift_vid.get(), c->ns, c->src_str.get(),
+                                                                    f32 ? c->src_str_f.get() : nullptr, ih);
+        KERNEL_CHECK();
+        return;
+    }
     lift_kernel<<<cdiv(c->ns, 256), 256, 0, c->stream>>>(q, phi, c->lift_w.get(), c->lift_vid.get(), c->ns, c->src_str.get(),
                                                          f32 ? c->src_str_f.get() : nullptr, ih);
     KERNEL_CHECK();

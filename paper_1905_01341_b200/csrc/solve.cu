@@ -160,8 +160,11 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
     K.part.alloc(DOT_BLOCKS);
     K.out.alloc(1);
 
-    const int timing = c->timing;
-    c->timing = 0;
+    struct TimingOff {                                           // the products of the solve are not timed; restored on every exit
+        bem_ctx *c; int saved;
+        explicit TimingOff(bem_ctx *cc) : c(cc), saved(cc->timing) { c->timing = 0; }
+        ~TimingOff() { c->timing = saved; }
+    } timing_off(c);
     // right-hand side (Eq. 16): b = -c phi + D phi
     apply_device(c, nullptr, phi.get(), w.get());
     rhs_kernel<<<cdiv(n, 256), 256, 0, s>>>(c->cfree.get(), phi.get(), w.get(), b.get(), n);
@@ -266,7 +269,6 @@ bem_status solve_impl(bem_ctx *c, const double *phi_in, double *q_io, int use_x0
             }
         }
     }
-    c->timing = timing;
     CUDA_TRY(cudaMemcpyAsync(q_io, x.get(), bytes, cudaMemcpyDefault, s));
     CUDA_TRY(cudaStreamSynchronize(s));
     if (iters_out) *iters_out = iters;
@@ -280,7 +282,7 @@ extern "C" bem_status bem_solve(bem_ctx *c, const double *phi, double *q, int us
                                 int *iters_out, double *relres_out)
 {
     if (!c || !phi || !q || !(tol > 0.0) || max_iter < 0) return BEM_ERR_INVALID_ARG;
-    if (c->quadrature == 2) { c->err = "bem_solve: not available for a point cloud"; return BEM_ERR_INVALID_ARG; }
+    if (c->quadrature >= 2) { c->err = "bem_solve: not available for a point cloud or an evaluator"; return BEM_ERR_INVALID_ARG; }
     if (!c->ready || !c->have_cfree) { c->err = "bem_solve before bem_setup"; return BEM_ERR_NOT_SETUP; }
     try {
         cudaSetDevice(c->device);
@@ -289,8 +291,14 @@ extern "C" bem_status bem_solve(bem_ctx *c, const double *phi, double *q, int us
         c->err = e.what();
         cudaGetLastError();
         return e.status;
+    } catch (const std::bad_alloc &) {
+        c->err = "bem_solve: out of host memory (Hessenberg of max_iter^2 entries: set option gmres_restart)";
+        return BEM_ERR_OOM;
     } catch (const std::exception &e) {
         c->err = e.what();
+        return BEM_ERR_CUDA;
+    } catch (...) {
+        c->err = "unknown error";
         return BEM_ERR_CUDA;
     }
 }

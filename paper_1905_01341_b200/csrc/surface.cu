@@ -421,6 +421,13 @@ bem_status bem_surface_velocity(bem_ctx *c, const double *phi, const double *q, 
         c->err = e.what();
         cudaGetLastError();
         return e.status;
+    } catch (const std::bad_alloc &) {
+        return BEM_ERR_OOM;
+    } catch (const std::exception &) {
+        cudaGetLastError();
+        return BEM_ERR_CUDA;                                  // nothing may cross the extern "C" boundary
+    } catch (...) {
+        return BEM_ERR_CUDA;
     }
 }
 
@@ -446,6 +453,13 @@ bem_status bem_surface_curvature(bem_ctx *c, double *H)
         c->err = e.what();
         cudaGetLastError();
         return e.status;
+    } catch (const std::bad_alloc &) {
+        return BEM_ERR_OOM;
+    } catch (const std::exception &) {
+        cudaGetLastError();
+        return BEM_ERR_CUDA;                                  // nothing may cross the extern "C" boundary
+    } catch (...) {
+        return BEM_ERR_CUDA;
     }
 }
 
@@ -487,6 +501,10 @@ bem_status bem_filter_create(const double *theta, const double *phi, int64_t n_d
         const bem_status st = e.status;
         delete f;
         return st;
+    } catch (...) {                                              // nothing may cross the extern "C" boundary
+        cudaGetLastError();
+        delete f;
+        return BEM_ERR_CUDA;
     }
     *out = f;
     return BEM_OK;
@@ -535,6 +553,13 @@ bem_status bem_filter_apply(bem_filter *f, const double *x, int64_t n_cols, doub
         f->err = e.what();
         cudaGetLastError();
         return e.status;
+    } catch (const std::bad_alloc &) {
+        return BEM_ERR_OOM;
+    } catch (const std::exception &) {
+        cudaGetLastError();
+        return BEM_ERR_CUDA;                                  // nothing may cross the extern "C" boundary
+    } catch (...) {
+        return BEM_ERR_CUDA;
     }
 }
 
