@@ -39,13 +39,36 @@ UNIT = "ms"
 # nominal FP64 FMA peak of B200 for the "alu" roofline: 148 SMs x 64 FP64
 # FMA lanes per SM per clock x 2 flop x 1.965 GHz (clocks.max.sm)
 FP64_NOMINAL_GFLOPS = 148 * 64 * 2 * 1.965
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels on config 5, from the committed
-# ncu --set full capture (profiles/r1_06_launches_and_full_capture.md); None for workloads that were not captured
-NCU_TRAFFIC = {"p2p_leaf": 1.351e9, "translate_dmma": 7.205e9}      # config 5, l_max 6, p 12: P2P launch; M2L tiles of level 6
+
+
+def ncu_traffic(kernel, cfg):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full capture:
+    profiles/traffic.json names the commit and the command it came from.  None when there is no capture of this kernel
+    on this config (the file says which config it was taken on)."""
+    try:
+        t = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        if int(t.get("config", -1)) != int(cfg):
+            return None
+        v = t["kernels"].get(kernel)
+        return None if v is None else float(v["dram_bytes"])
+    except Exception:
+        return None
 
 
 def workload_name(c):
     return c["name"]
+
+
+def workload_config(c, args, p):
+    """The keys that name the workload -- the SAME dict in the b200 arm and in the reference arm (the CPU oracle computes
+    the same discretised operator on the same inputs); what only the GPU run knows (tree depth, launch mode, device bytes)
+    goes to the line's "run" key."""
+    N, T = int(c["V"].shape[0]), int(c["F"].shape[0])
+    cloud = bool(c.get("cloud"))
+    return dict(workload=workload_name(c), operator="y = S[q] - D[phi] (G3 quadrature + near correction)" if not cloud else "monopole sum",
+                p=int(p), n_nodes=N, n_triangles=T, n_sources=(N if cloud else 3 * T), leaf_size=int(args.leaf_size or c["leaf_size"]),
+                eta=c["eta"], parallelism="replicas only" if args.gpus > 1 else "1 gpu",
+                l2="working set larger than L2" if N >= 100000 else "flushed between iterations (512 MB write)")
 
 
 def cloud_config(n, seed=190501341 + 6):
@@ -119,7 +142,9 @@ def run_reference(args):
     v = float(np.mean(per_step))
     line = dict(impl="reference", metric=METRIC, value=v, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
                 warmup=args.warmup, ms_per_step=v, higher_is_better=False, scaling="weak", vs_baseline=None,
-                dtype="f64", data="synthetic", config=dict(workload=workload_name(c), p=c["p"], n_nodes=int(c["V"].shape[0])),
+                dtype="f64", data="synthetic", config=workload_config(c, args, args.p or c["p"]),
+                ratio_note="this arm is the plain O(N^2) direct sum of the oracle: a b200 / reference ratio is 'FMM on a GPU vs direct sum "
+                           "on host cores' and says nothing about kernel quality (the roofline fractions do)",
                 cpu_baseline=dict(value=v, unit=UNIT, cores=info["cores"], kind="oracle", sample=info["sample"]),
                 e2e=dict(value=v, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line), flush=True)
@@ -230,7 +255,7 @@ def run_gpu(args):
 
     # L2 policy: the working set of one apply (sources, expansions, lists, CSR) is far above the 126 MB L2 for
     # configs 3-5; for the small configs a 512 MB buffer is rewritten between timed iterations.
-    flush = stats["device_bytes"] < 4 * 126e6
+    flush = N < 100000
     fbuf = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda") if flush else None
 
     def timed(fn, steps):
@@ -303,7 +328,9 @@ def run_gpu(args):
     nre = stats["exp_stride"] / 2.0
     kernels = {}
     p2p_s = tm["p2p"] * 1e-3
-    kernels["p2p"] = dict(ms=tm["p2p"], pairs=stats["p2p_pairs"], gpairs_per_s=stats["p2p_pairs"] / p2p_s / 1e9 if p2p_s > 0 else None,
+    kernels["p2p"] = dict(ms=tm["p2p"], pairs=stats["p2p_pairs"], pairs_executed=stats["p2p_pairs_executed"],
+                          executed_note="source lists are padded to rounds of 128: pairs / pairs_executed of the kernel's work is useful",
+                          gpairs_per_s=stats["p2p_pairs"] / p2p_s / 1e9 if p2p_s > 0 else None,
                           tflops=stats["p2p_pairs"] * P2P_FLOP / p2p_s / 1e12 if p2p_s > 0 else None,
                           fp64_slot_frac=stats["p2p_pairs"] * P2P_INSTR / p2p_s / 1e12 / slot_peak if p2p_s > 0 else None,
                           note=("12 FP32 instr (18 flop) + 1 MUFU.RSQ per pair; fp64_slot_frac here = share of the FP32 pipes' issue slots (nominal 37.2 T instr/s)"
@@ -339,13 +366,13 @@ def run_gpu(args):
         k = kernels["p2p"]
         roof = dict(kernel="p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", bound="alu", achieved=k["tflops"],
                     peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", frac=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
-                    fp64_slot_frac=k["fp64_slot_frac"], traffic=NCU_TRAFFIC.get("p2p_direct" if args.direct else "p2p_leaf") if args.config == 5 else None,
+                    fp64_slot_frac=k["fp64_slot_frac"], traffic=ncu_traffic("p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", args.config),
                     algorithmic="26 flop (17 FP64 instructions) per pair x %d pairs" % stats["p2p_pairs"], ms=tm["p2p"],
                     share_of_step=tm["p2p"] / tm["total"], **common)
     else:
         k = kernels["m2l"]
         roof = dict(kernel="translate_dmma", bound="tensor", achieved=k["executed_tflops"], peak=dmma / 1e3, unit="TFLOP/s",
-                    frac=k["frac_of_measured_dmma_peak"], traffic=NCU_TRAFFIC.get("translate_dmma") if args.config == 5 else None,
+                    frac=k["frac_of_measured_dmma_peak"], traffic=ncu_traffic("translate_dmma", args.config),
                     algorithmic="4 nre^2 flop per M2L pair x %d pairs (FP64 DMMA; peak = DMMA loop measured in this run)" % stats["m2l_pairs"],
                     ms=tm["m2l"], share_of_step=tm["m2l"] / tm["total"], **common)
     breakdown = {k: round(v, 4) for k, v in tm.items()}
@@ -425,20 +452,48 @@ def run_gpu(args):
             ms_s = (time.perf_counter() - t0) * 1e3
             solve[name] = dict(ms=ms_s, iterations=it, relres=rr, tol=args.solve_tol, max_iter=max_it,
                                status=bem.STATUS_NAMES[st], ms_per_iteration=ms_s / max(it, 1))
+            if pre == 0 and prec == 0:
+                q_cold = qs.clone()
+                if args.solve_check_rows > 0 and not cloud:
+                    # the residual of the returned q recomputed by the ORACLE on seeded rows:
+                    # b_i = -c_i phi_i + (D phi)_i with c_i = 1 + (D.1)_i, r_i = b_i - (S q)_i -- three oracle products
+                    import oracle
+                    rr_rows = sample_rows(c["cfg"], N, args.solve_check_rows)
+                    qh_s = qs.cpu().numpy()
+                    o = lambda a, b: oracle.g3_apply(V, F, a, b, eta=c["eta"], rows=rr_rows)
+                    t0o = time.perf_counter()
+                    cfree = 1.0 - o(None, np.ones(N))
+                    b_rows = -cfree * c["phi"][rr_rows] - o(None, c["phi"])
+                    res_rows = b_rows - o(qh_s, None)
+                    solve[name]["relres_by_oracle_on_rows"] = float(np.linalg.norm(res_rows) / np.linalg.norm(b_rows))
+                    solve[name]["oracle_rows"] = int(len(rr_rows))
+                    solve[name]["oracle_check_s"] = time.perf_counter() - t0o
+        # the paper's regime: every time step starts GMRES from the previous step's solution and needs
+        # 2-10 iterations.  Perturb phi by 1% (seeded) and solve again from the cold solution of the unperturbed phi.
+        if not cloud and "unpreconditioned (paper)" in solve and solve["unpreconditioned (paper)"]["status"] == "BEM_OK":
+            ctx.bem_set_option("precond", 0)
+            rng = np.random.default_rng(190501341 + 200 + int(c["cfg"]))
+            pd2 = pd * torch.tensor(1.0 + 0.01 * rng.uniform(-1.0, 1.0, N), device="cuda")
+            qw = q_cold.clone()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            st, it, rr = ctx.bem_solve(pd2, qw, use_q_as_x0=True, tol=args.solve_tol, max_iter=max_it)
+            torch.cuda.synchronize()
+            ms_s = (time.perf_counter() - t0) * 1e3
+            solve["warm start, phi perturbed by 1% (unpreconditioned)"] = dict(ms=ms_s, iterations=it, relres=rr, tol=args.solve_tol,
+                                                                                status=bem.STATUS_NAMES[st], ms_per_iteration=ms_s / max(it, 1))
         ctx.bem_set_option("precond", 0)
         if not args.direct:
             ctx.bem_set_option("p2p_precision", 1 if f32 else 0)
 
     line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
                 higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64 (near-field pairs f32)" if f32 else "f64", data="synthetic",
-                config=dict(workload=workload_name(c), mode="direct" if args.direct else "fmm", p=p,
-                            p2p_precision="fp32 pairs, fp64 sums" if f32 else "fp64", n_nodes=N, n_triangles=T,
-                            n_sources=int(stats["n_sources"]), leaf_size=args.leaf_size or c["leaf_size"], eta=c["eta"],
-                            lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]), n_tgt_leaves=int(stats["n_tgt_leaves"]),
-                            parallelism="replicas only" if world > 1 else "1 gpu",
-                            launch="CUDA graph replay" if (stream.cuda_stream != 0 and not args.no_graph) else "kernel by kernel",
-                            l2="flushed between iterations (512 MB write)" if flush else "working set larger than L2",
-                            device_bytes=int(stats["device_bytes"])),
+                config=workload_config(c, args, p),
+                run=dict(mode="direct" if args.direct else "fmm", p2p_precision="fp32 pairs, fp64 sums" if f32 else "fp64",
+                         p_dipole=int(stats["p_dipole"]), lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]),
+                         n_tgt_leaves=int(stats["n_tgt_leaves"]),
+                         launch="CUDA graph replay" if (stream.cuda_stream != 0 and not args.no_graph) else "kernel by kernel",
+                         device_bytes=int(stats["device_bytes"]), options=args.opt),
                 e2e=dict(value=e2e, unit=UNIT, h2d_bytes_per_step=(8 if cloud else 16) * N, d2h_bytes_per_step=8 * N),
                 gpu_launches=int(stats["kernel_launches_per_apply"]) * args.steps,
                 clocks=clocks, roofline=roof, cpu_baseline=cpu, parity_rel_l2_vs_oracle=parity,
@@ -477,6 +532,8 @@ def main():
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="any bem_set_option key (repeatable), set before bem_setup")
     ap.add_argument("--solve-iters", type=int, default=-1, help="also run bem_solve with this max_iter (0: skip; -1: 30, or 400 = to convergence on config 5)")
     ap.add_argument("--solve-tol", type=float, default=1e-6)
+    ap.add_argument("--solve-check-rows", type=int, default=400,
+                    help="rows on which the ORACLE recomputes the residual of the first bem_solve (three oracle products; 0: skip)")
     ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU time budget of one oracle sample")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -76,6 +76,8 @@ enum {
     BEM_S_M2L_FLOP,        /* executed flop of the M2L tiles of one product (graded truncation: 4 (4 KE)^2 per pair) */
     BEM_S_M2L_ROW_BYTES,   /* bytes of translated rows the per-target sums read in one product                     */
     BEM_S_P_DIPOLE,        /* truncation number of the products that carry dipoles (option "dipole_degrees")                 */
+    BEM_S_P2P_PAIRS_EXECUTED, /* point pairs the near-field kernel executes: BEM_S_P2P_PAIRS are the useful ones, the source list
+                               of a target leaf is padded to whole rounds of 128 sources                               */
     BEM_S_COUNT
 };
 

@@ -704,6 +704,7 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
         s[BEM_S_N_SRC_LEAVES] = c->sb.nbox[c->sb.lmax];
         s[BEM_S_N_TGT_LEAVES] = c->tb.nbox[c->tb.lmax];
         s[BEM_S_P2P_PAIRS] = (double)c->p2p_pairs;
+        s[BEM_S_P2P_PAIRS_EXECUTED] = (double)c->p2p_pairs_exec;
         s[BEM_S_M2L_PAIRS] = (double)c->m2l_pairs;
         const FmmLayout &Lf = c->lay[c->n_lay - 1];           // the layout of a full product (q and phi)
         s[BEM_S_M2L_FLOP] = Lf.m2l_flop;
@@ -712,7 +713,7 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
         s[BEM_S_N_SRC_BOXES] = c->sb.total();
         s[BEM_S_N_TGT_BOXES] = c->tb.total();
     } else {
-        s[BEM_S_P2P_PAIRS] = (double)c->N * (double)c->ns;
+        s[BEM_S_P2P_PAIRS] = s[BEM_S_P2P_PAIRS_EXECUTED] = (double)c->N * (double)c->ns;
     }
     for (int k = 0; k < n && k < BEM_S_COUNT; ++k) out[k] = s[k];
     return BEM_OK;

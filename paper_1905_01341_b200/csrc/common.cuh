@@ -250,6 +250,7 @@ struct bem_ctx {
     std::vector<bem::Stage> m2l;    // 2 .. lmax: L_own(l) = sum of the M2L rows of the level
     std::vector<bem::Stage> l2l;    // 3 .. lmax: L(l) = L_own(l) + L2L L(l-1)
     int64_t m2l_pairs = 0, p2p_pairs = 0;
+    int64_t p2p_pairs_exec = 0;     // pairs the near-field kernel executes: source lists padded to rounds of 128 (tree.cu)
 
     // partial sums of the point engine, combined by the SpMV kernel
     bem::dvec<double> ypart;        // [nsplit * N]  (FMM mode: slot 0 = far field (L2P), slot 1 = near field (P2P))

@@ -196,6 +196,20 @@ __global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
     if (xcount) { xcount[t] = xc; if (xp) atomicAdd(xpairs, xp); }
 }
 
+// pairs the near-field kernel EXECUTES: it pads the concatenated source list of a target leaf (neighbours + direct far
+// boxes) to whole rounds of `round` sources (p2p.cu), so a leaf costs nt x ceil(S / round) x round pairs
+__global__ void executed_pairs(const int32_t *tbegin, const int32_t *nbr, const int32_t *xptr, const int32_t *xsrc,
+                               const int32_t *sbegin, int ntl, int round, unsigned long long *out)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntl) return;
+    long long S = 0;
+    for (int k = 0; k < 27; ++k) { const int b = nbr[(int64_t)t * 27 + k]; if (b >= 0) S += sbegin[b + 1] - sbegin[b]; }
+    if (xptr) for (int k = xptr[t]; k < xptr[t + 1]; ++k) { const int b = xsrc[k]; S += sbegin[b + 1] - sbegin[b]; }
+    const long long nt = tbegin[t + 1] - tbegin[t];
+    atomicAdd(out, (unsigned long long)(nt * ((S + round - 1) / round) * round));
+}
+
 // L2L: one pair per target box: its parent's local expansion through the matrix of its octant
 __global__ void l2l_pairs(const uint64_t *tkey, const int32_t *tparent, int nt, int tbase_parent, int32_t *src, int32_t *mat, int32_t *ptr)
 {
@@ -352,6 +366,14 @@ void build_lists(bem_ctx *c)
         c->m2l_pairs += total;
         st.scratch_off = max_pairs;                           // regions of the levels one after the other
         max_pairs += total;
+    }
+    {
+        pc.zero(s);
+        executed_pairs<<<cdiv(ntl, 128), 128, 0, s>>>(tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, sb.begin.get(), ntl, 128, pc.get());
+        KERNEL_CHECK();
+        unsigned long long ex = 0;
+        d2h_sync(&ex, pc.get(), sizeof ex, s);
+        c->p2p_pairs_exec = (int64_t)ex;
     }
     // M2M stages: parents on level l = lmax-1 .. 2
     c->m2m.clear();
