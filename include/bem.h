@@ -138,9 +138,13 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   the diagonal rule M_ii = -1/2 - sum_{j!=i} M_ij
  *                   (default); 1 = c_i = 1/2 literally (Eq. 15)
  *   "gmres_restart" 0 = no restart up to max_iter (default), else restart length
- *   "reduce_ctas"   bem_apply sums the translated M2L rows per target on a side stream while the near field runs;
- *                   that pass is a persistent grid of this many CTAs per SM (1..32; 0 = chosen in bem_setup from
- *                   the pair counts so that it ends just before the near field does; default).  Tuning only.
+ *   "overlap"       0 (default) = every kernel of a product on the context's stream; 1 = the per-target sums of the
+ *                   translated M2L rows (HBM-bound) run on a side stream beside the near field (FP64-bound).  Round 1
+ *                   measured a gain (25.6 -> 24.5 ms on config 5); with the graded M2L rows of round 2 the sums are
+ *                   short, and the CTAs they hold cost the near-field kernel more than the overlap wins (config 5:
+ *                   22.6 ms on one stream, 22.6-24.4 ms with the side stream).  Results are bit-identical.
+ *   "reduce_ctas"   with overlap = 1: the sums are a persistent grid of this many CTAs per SM (1..32; 0 = chosen
+ *                   from the pair counts so that it ends just before the near field does).  Tuning only.
  *   "m2l_rows16"    M2L tiles at p = 11, 12: 1 = 4 warps x 16 rows per CTA (default), 0 = 8 warps x 8 rows.
  *                   A tuning switch: both compute the same tiles.  May be changed between products.
  *   "precond"       bem_solve: 0 = unpreconditioned GMRES, as in the paper (default); 1 = right

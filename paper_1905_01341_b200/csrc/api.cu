@@ -188,7 +188,7 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
         launch_p2m(c);
         mark(c, BEM_T_P2M);
         for (int l = lmax - 1; l >= 2; --l) launch_stage(c, c->m2m[l], BEM_T_M2M, BEM_T_M2M);
-        if (c->timing || !c->side) {
+        if (c->timing || !c->side || !c->overlap) {
             // one stream, class by class (option "timing": the per-class event times add up to the total)
             for (int l = 2; l <= lmax; ++l) launch_stage(c, c->m2l[l], BEM_T_M2L, BEM_T_L2L_REDUCE);
             for (int l = 3; l <= lmax; ++l) launch_stage(c, c->l2l[l], BEM_T_L2L_REDUCE, BEM_T_L2L_REDUCE);
@@ -621,6 +621,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "m2l_order_radius")) { if (!(value >= 0 && value < 1.0)) return BEM_ERR_INVALID_ARG; c->m2l_order_radius = value; c->ready = false; }
     else if (!strcmp(key, "m2l_order_extra")) { if (v < -8 || v > 8) return BEM_ERR_INVALID_ARG; c->m2l_order_extra = v; c->ready = false; }
     else if (!strcmp(key, "dipole_degrees")) { if (v < -1 || v > 16) return BEM_ERR_INVALID_ARG; c->dipole_degrees = v; c->ready = false; }
+    else if (!strcmp(key, "overlap")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->overlap = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
     return BEM_OK;
