@@ -384,7 +384,8 @@ def run_gpu(args):
 
     # the paper's "single precision on GPU" option for A^(sparse) X, measured beside the fp64 default
     mixed = None
-    if not args.direct and not f32:
+    adaptive = any(o.replace(" ", "") == "tree=1" for o in args.opt)            # fp32 pairs need leaves of one size (uniform tree)
+    if not args.direct and not f32 and not adaptive:
         ctx.bem_set_option("p2p_precision", 1)
         for _ in range(3):
             ctx.bem_apply(qd, pd, yd)
@@ -438,7 +439,7 @@ def run_gpu(args):
     if max_it > 0 and not cloud:
         solve = {}
         runs = [("unpreconditioned (paper)", 0, 0), ("diagonal S_ii (option precond)", 1, 0)]
-        if not args.direct and not f32:
+        if not args.direct and not f32 and not adaptive:
             runs.append(("diagonal S_ii, fp32 pairs (options precond, p2p_precision)", 1, 1))
         for name, pre, prec in runs:
             ctx.bem_set_option("precond", pre)

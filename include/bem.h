@@ -152,7 +152,28 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   the L_ii of Eq. 21).  The stopping rule (true relative residual of S q = b) is unchanged.
  *                   Not in the paper: it equilibrates bubbles of different size (S_ii ~ mesh size).  May be
  *                   changed between solves.
- *   "lmax"          0 = choose the octree depth from leaf_size (default), else force it
+ *   "lmax"          0 = choose the octree depth from leaf_size (default), else force it (adaptive tree: cap it)
+ *   "tree"          0 = uniform depth l_max with empty boxes skipped -- the paper's tree (default);
+ *                   1 = adaptive octree: a box is subdivided iff it holds more than leaf_size sources or lies above
+ *                   the depth the uniform rule gives for that leaf_size (so the adaptive tree only REFINES the boxes
+ *                   that are denser than the mean; "tree_min_level" lowers that floor, >= 2), a box exists iff its
+ *                   parent is subdivided, leaves sit on several levels.  Far field between existing boxes of equal
+ *                   level (V lists); a target leaf sums directly the sources of the same-level boxes that touch it
+ *                   and of the coarser source leaves that touch its ancestors (the U, W and X lists of the adaptive
+ *                   FMM, W and X taken directly: exact).  Same tolerances; p2p_precision = 1 is refused (its fp32
+ *                   positions need leaves of one size).  Measured: on the bubble clusters of BASELINE.json the two
+ *                   trees are within 2% of each other; on a strongly clustered point cloud the adaptive tree needs
+ *                   19x fewer point pairs.
+ *   "tree_min_level" adaptive tree: boxes above this level are always subdivided (0 = the uniform depth; >= 2)
+ *   "dipole_degrees" products that carry dipoles (phi != NULL) are truncated to p + this many degrees; -1 (default) =
+ *                   3 below p = 12 and 0 from 12 on (measured: S - D then meets relative L2 1e-5 at the stated p of
+ *                   every BASELINE config; a dipole is one derivative of the monopole expansion and loses 3-4
+ *                   degrees of accuracy at equal truncation); 0 = one truncation for everything, the paper's
+ *                   convention.  Products without dipoles (every GMRES iteration) always use p.
+ *   "m2l_order_radius", "m2l_order_extra"  graded truncation of the M2L translations: the offset o (in box edges) uses
+ *                   the degrees < p_o = ceil(p ln k(2) / ln k(|o|)) + extra, k(d) = a / (d - a), a = radius (default
+ *                   0.5, extra 1: error against the oracle unchanged within 7% on every config, executed M2L work
+ *                   x0.54 at p = 12); radius 0 = every translation uses all p degrees.
  *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply
  *   "gemm_path"     batched translations (M2M, M2L, L2L): 0 = FP64 tensor-core tiles (DMMA; p <= 16,
  *                   default -- measured faster), 1 = plain FP64 FMA tiles (any p).

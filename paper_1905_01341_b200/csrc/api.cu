@@ -19,6 +19,9 @@ void build_empty_correction(bem_ctx *c);
 void boxset_sort(BoxSet &bs, const double *xyz, int64_t n, const double cube_min[3], double cube_side, int counts[22], cudaStream_t s);
 void boxset_build(BoxSet &bs, int lmax, const int counts[22], cudaStream_t s);
 void build_lists(bem_ctx *c);
+// adaptive.cu
+int adaptive_source_flags(bem_ctx *c, bool *want_deeper);
+void build_adaptive(bem_ctx *c);
 // translate.cu
 void build_matrices(bem_ctx *c, FmmLayout &L);
 void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce);
@@ -176,7 +179,10 @@ void apply_device(bem_ctx *c, const double *q, const double *phi, double *y)
 {
     c->ev_n = 0;
     if (c->mode == 0) activate_layout(c, (phi && c->n_lay > 1) ? 1 : 0);      // products with dipoles carry more degrees (option dipole_degrees)
-    if (c->mode == 0 && c->p2p_precision == 1) ensure_p2p_f32(c);
+    if (c->mode == 0 && c->p2p_precision == 1) {
+        if (c->adaptive) throw Error(BEM_ERR_INVALID_ARG, "p2p_precision = 1 needs the uniform tree (option tree = 0): its fp32 positions are relative to leaves of one size");
+        ensure_p2p_f32(c);
+    }
     mark(c, -1);
     launch_lift(c, q, phi);
     mark(c, BEM_T_LIFT);
@@ -347,7 +353,28 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         int lmax = 2;
         while (lmax < MAX_LEVEL && (double)c->ns / (double)cs[lmax] > (double)leaf_size) ++lmax;
         if (c->force_lmax >= 2) lmax = std::min(c->force_lmax, MAX_LEVEL);
-        boxset_build(c->sb, lmax, cs, s);
+        if (c->adaptive) {
+            // adaptive tree: build the source boxes down to a probe depth (option lmax caps it), flag what exists under the
+            // rule "subdivide a box that holds more than leaf_size sources", and keep the levels that hold an existing box
+            c->ad.lmin = c->tree_min_level >= 2 ? std::min(c->tree_min_level, lmax) : lmax;
+            if (c->force_lmax >= 2) c->ad.lmin = std::min(c->ad.lmin, lmax);
+            int lprobe = c->force_lmax >= 2 ? lmax : std::min(MAX_LEVEL, lmax + 3);
+            int deep = 2;
+            for (;;) {                                            // deepen the probe while the rule still wants to subdivide
+                bool more = false;
+                boxset_build(c->sb, lprobe, cs, s);
+                deep = adaptive_source_flags(c, &more);
+                if (!more || c->force_lmax >= 2 || lprobe >= MAX_LEVEL) break;
+                lprobe = std::min(MAX_LEVEL, lprobe + 3);
+            }
+            if (deep < lprobe) { boxset_build(c->sb, deep, cs, s); adaptive_source_flags(c, nullptr); }
+            lmax = deep;
+            for (int l = lmax + 1; l <= MAX_LEVEL; ++l) {
+                c->sb.bkey[l].free(); c->sb.child[l].free(); c->sb.parent[l].free(); c->sb.nbox[l] = 0;
+                c->ad.s_ex[l].free(); c->ad.s_sub[l].free(); c->ad.s_pbeg[l].free();
+            }
+            c->sb.child[lmax].free();
+        } else boxset_build(c->sb, lmax, cs, s);
         boxset_build(c->tb, lmax, ct, s);
         build_sources(c, c->sb.perm.get());
         c->tgt_pos.alloc(3 * N);
@@ -367,7 +394,8 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
             const double w = 800.0 * (double)c->nre * (double)c->nre / 6400.0;
             c->direct_max_eff = c->direct_max >= 0 ? c->direct_max : (int64_t)w;
         }
-        build_lists(c);
+        if (c->adaptive) build_adaptive(c);
+        else build_lists(c);
         for (int i = 0; i < c->n_lay; ++i) layout_stats(c, c->lay[i]);
         activate_layout(c, 0);
         c->nsplit = 2;                                  // far field (L2P) and near field (P2P) partial sums
@@ -391,7 +419,7 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
 
     if (c->quadrature == 0 || c->quadrature == 3) build_correction(c);
     else build_empty_correction(c);
-    if (c->mode == 0 && c->p2p_precision == 1) ensure_p2p_f32(c);
+    if (c->mode == 0 && c->p2p_precision == 1 && !c->adaptive) ensure_p2p_f32(c);
     c->ready = true;
     if (c->quadrature >= 2) {                               // point cloud, evaluator: no free term, no solve
         CUDA_TRY(cudaStreamSynchronize(s));
@@ -614,13 +642,15 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
         c->p2p_precision = v;
         // the fp32 source records are built HERE (or at the end of bem_setup), never inside a product: a product may run
         // inside a stream capture of the caller, where an allocation is not allowed
-        if (v == 1 && c->ready && c->mode == 0) return guarded(c, [&]() { ensure_p2p_f32(c); CUDA_TRY(cudaStreamSynchronize(c->stream)); });
+        if (v == 1 && c->ready && c->mode == 0 && !c->adaptive) return guarded(c, [&]() { ensure_p2p_f32(c); CUDA_TRY(cudaStreamSynchronize(c->stream)); });
     }
     else if (!strcmp(key, "direct_pairs")) { if (value < -1 || value > 1e9) return BEM_ERR_INVALID_ARG; c->direct_max = (int64_t)value; c->ready = false; }
     else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
     else if (!strcmp(key, "m2l_order_radius")) { if (!(value >= 0 && value < 1.0)) return BEM_ERR_INVALID_ARG; c->m2l_order_radius = value; c->ready = false; }
     else if (!strcmp(key, "m2l_order_extra")) { if (v < -8 || v > 8) return BEM_ERR_INVALID_ARG; c->m2l_order_extra = v; c->ready = false; }
     else if (!strcmp(key, "dipole_degrees")) { if (v < -1 || v > 16) return BEM_ERR_INVALID_ARG; c->dipole_degrees = v; c->ready = false; }
+    else if (!strcmp(key, "tree_min_level")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->tree_min_level = v; c->ready = false; }
+    else if (!strcmp(key, "tree")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->adaptive = v; c->ready = false; }
     else if (!strcmp(key, "overlap")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->overlap = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }
     else { c->err = std::string("unknown option: ") + key; return BEM_ERR_INVALID_ARG; }
@@ -702,8 +732,8 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
     s[BEM_S_KERNEL_LAUNCHES_PER_APPLY] = c->launches_per_apply;
     if (c->mode == 0) {
         s[BEM_S_LMAX] = c->sb.lmax;
-        s[BEM_S_N_SRC_LEAVES] = c->sb.nbox[c->sb.lmax];
-        s[BEM_S_N_TGT_LEAVES] = c->tb.nbox[c->tb.lmax];
+        s[BEM_S_N_SRC_LEAVES] = c->adaptive ? c->ad.n_src_leaves : c->sb.nbox[c->sb.lmax];
+        s[BEM_S_N_TGT_LEAVES] = c->adaptive ? c->ad.n_tleaf : c->tb.nbox[c->tb.lmax];
         s[BEM_S_P2P_PAIRS] = (double)c->p2p_pairs;
         s[BEM_S_P2P_PAIRS_EXECUTED] = (double)c->p2p_pairs_exec;
         s[BEM_S_M2L_PAIRS] = (double)c->m2l_pairs;

@@ -122,6 +122,13 @@ struct BoxSet {                     // the non-empty boxes of one point set on l
     int total() const { return base[lmax + 1]; }
 };
 
+// existence / subdivision flags of the boxes an interaction-list kernel looks at (adaptive tree; all null: uniform tree)
+struct AdaptiveFlags {
+    const uint8_t *t_ex = nullptr, *t_sub = nullptr;                 // target boxes of the level
+    const uint8_t *s_sub = nullptr;                                   // source boxes of the level
+    const uint8_t *s_ex_parent = nullptr, *s_sub_parent = nullptr;    // source boxes of the parent level
+};
+
 // One batched-translation stage: out[tgt] = sum over the target's pairs of T[mat] * in[src]
 // executed as (tiles of a dense GEMM per matrix) -> scratch rows in target-major order -> fixed-order row sums.
 struct Tile { int32_t mat, row0, nrows, flags; };     // flags: bit 0 input rows are local expansions, bit 1 M2L (azimuth split)
@@ -136,14 +143,36 @@ struct Stage {
     int out_base = 0;               // global index of the first target box
     bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
     bool accumulate = false;        // the reduce pass adds to the output instead of overwriting it (L2L)
+    bool keep_empty = false;        // the reduce pass leaves the output of a target with no pair alone (adaptive M2M: leaves)
     dvec<int32_t> src_sorted;       // [npairs] global input box of scratch row r (matrix-sorted order)
     dvec<int32_t> krow;             // [npairs] target-major index k of the pair in tile row r: its scratch row (the rows of a target are
                                     // contiguous in scratch, so the row sums stream them; the tiles scatter whole 8 nst-byte rows)
     dvec<int32_t> mat_t;            // [npairs] matrix id of pair k (target-major order): the reduce pass rotates back by its azimuth
     dvec<int32_t> ptr;              // [ntgt+1] CSR of pairs per target (target-major)
+    dvec<int32_t> tgt_list;         // adaptive tree: the targets the reduce pass visits (existing boxes; M2M: subdivided parents)
+    int n_list = -1;                // -1: every target
     dvec<Tile> tiles;
     int ntiles = 0;
     int ntiles_split = 0;           // the first ntiles_split tiles are M2L tiles (matrix ids < MAT_L2L come first)
+};
+
+// Adaptive octree (option "tree" = 1, adaptive.cu): flags and tables on top of the two BoxSets
+struct Adaptive {
+    dvec<uint8_t> s_ex[MAX_LEVEL + 1], s_sub[MAX_LEVEL + 1];   // source boxes of a level: exists (parent subdivided), subdivided
+    dvec<uint8_t> t_ex[MAX_LEVEL + 1], t_sub[MAX_LEVEL + 1];   // target boxes
+    dvec<int32_t> s_pbeg[MAX_LEVEL + 1], t_pbeg[MAX_LEVEL + 1]; // [nbox + 1] first point of every box of a level
+    dvec<int32_t> sleaf[MAX_LEVEL + 1];                         // source leaves of a level (box indices): P2M
+    int n_sleaf[MAX_LEVEL + 1] = {0};
+    int lmin = 2;                                                 // boxes above this level are always subdivided
+    int n_src_leaves = 0;
+    dvec<uint64_t> tkey_all;                                    // [target boxes] key and level by global box id: L2P
+    dvec<uint8_t> tlev_all;
+    dvec<int32_t> pt_gbox;                                      // [N] global box id of the leaf of every target point
+    dvec<int32_t> tleaf_begin, tleaf_gbox;                      // target leaves in point order: first point, global box id
+    int n_tleaf = 0;
+    dvec<int32_t> near_ptr;                                     // [n_tleaf + 1] CSR of the direct source ranges of a target leaf
+    dvec<int2> near_rng;                                        // (first source, count)
+    dvec<int32_t> x_ptr[MAX_LEVEL + 1], x_src[MAX_LEVEL + 1];   // far pairs of two sparse leaves, summed directly (per level)
 };
 
 // Everything bem_setup builds that depends on the truncation number.  A context holds one layout for the products without
@@ -226,6 +255,9 @@ struct bem_ctx {
 
     // octree + lists (FMM mode)
     bem::BoxSet sb, tb;
+    int tree_min_level = 0;         // option "tree_min_level": 0 = the depth of the uniform rule, else the level (>= 2)
+    int adaptive = 0;               // option "tree": 0 = uniform depth (the paper's), 1 = adaptive (adaptive.cu)
+    bem::Adaptive ad;
     bem::dvec<int32_t> nbr;         // [n_tgt_leaves * 27] source leaves adjacent to a target leaf, -1 padded
     bem::dvec<int32_t> xdir_ptr;    // [n_tgt_leaves + 1] CSR of the leaf-level far pairs that are summed directly (option direct_pairs)
     bem::dvec<int32_t> xdir_src;    // [xdir_pairs] their source leaves

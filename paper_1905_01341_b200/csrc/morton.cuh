@@ -43,4 +43,12 @@ __host__ __device__ __forceinline__ uint32_t cell21(double u)
     return (uint32_t)v;
 }
 
+// index of key k in the ascending array keys[0..n), or -1
+__device__ __forceinline__ int find_box(const uint64_t *keys, int n, uint64_t k)
+{
+    int lo = 0, hi = n;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (keys[mid] < k) lo = mid + 1; else hi = mid; }
+    return (lo < n && keys[lo] == k) ? lo : -1;
+}
+
 }  // namespace bem

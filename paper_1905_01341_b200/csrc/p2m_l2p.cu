@@ -64,7 +64,7 @@ constexpr int P2M_TBL = 64 * 33;
 
 template <int P, bool DIP>
 __global__ void __launch_bounds__(P2M_WARPS * 32, P2M_MINB)
-p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf,
+p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, const int32_t *__restrict__ list, int nleaf,
              double cmx, double cmy, double cmz, double h,
              const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nst, double *__restrict__ Mout,
              int *__restrict__ counter)
@@ -79,6 +79,7 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
     if (lane == 0) leaf = atomicAdd(counter, 1);
     leaf = __shfl_sync(0xffffffffu, leaf, 0);
     if (leaf >= nleaf) return;
+    if (list) leaf = list[leaf];                                  // adaptive tree: the leaves of this level are a subset of its boxes
     uint32_t ix, iy, iz;
     morton_decode(skey[leaf], &ix, &iy, &iz);
     const double cx = cmx + (ix + 0.5) * h, cy = cmy + (iy + 0.5) * h, cz = cmz + (iz + 0.5) * h;
@@ -172,11 +173,12 @@ p2m_kernel_t(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ sk
     }
 }
 
+// level / nleaf / list / sbegin: the leaves of one level (uniform tree: all boxes of level lmax, list = null)
 template <int P>
-static void p2m_launch(bem_ctx *c)
+static void p2m_launch(bem_ctx *c, int lmax, int nleaf, const int32_t *list, const int32_t *sbegin)
 {
     const BoxSet &sb = c->sb;
-    const int lmax = sb.lmax, nleaf = sb.nbox[lmax];
+    if (nleaf == 0) return;
     const double h = c->cube_side / (double)(1 << lmax);
     const size_t smem = (size_t)P2M_WARPS * P2M_TBL * sizeof(double);
     static std::vector<char> attr_done;
@@ -188,24 +190,31 @@ static void p2m_launch(bem_ctx *c)
     CUDA_TRY(cudaMemsetAsync(c->p2p_counter.get() + 2, 0, sizeof(int), c->stream));
     const int grid = std::max(1, std::min(cdiv(nleaf, P2M_WARPS), P2M_MINB * c->n_sm));     // the CTAs that fit an SM (registers, shared memory)
     kern<<<grid, P2M_WARPS * 32, smem, c->stream>>>(
-        sb.begin.get(), sb.bkey[lmax].get(), nleaf, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
+        sbegin, sb.bkey[lmax].get(), list, nleaf, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
         c->src_pos.get(), c->src_str.get(), c->p, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst, c->p2p_counter.get() + 2);
     KERNEL_CHECK();
 }
 
-void launch_p2m_generic(bem_ctx *c);   // translate.cu
+void launch_p2m_generic(bem_ctx *c, int level, int nleaf, const int32_t *list, const int32_t *sbegin);   // translate.cu
+
+static void launch_p2m_level(bem_ctx *c, int level, int nleaf, const int32_t *list, const int32_t *sbegin)
+{
+    const int p = c->p;
+    if (p <= 4) p2m_launch<4>(c, level, nleaf, list, sbegin);
+    else if (p <= 6) p2m_launch<6>(c, level, nleaf, list, sbegin);
+    else if (p <= 8) p2m_launch<8>(c, level, nleaf, list, sbegin);
+    else if (p <= 10) p2m_launch<10>(c, level, nleaf, list, sbegin);
+    else if (p <= 12) p2m_launch<12>(c, level, nleaf, list, sbegin);
+    else if (p <= 14) p2m_launch<14>(c, level, nleaf, list, sbegin);
+    else if (p <= 16) p2m_launch<16>(c, level, nleaf, list, sbegin);
+    else launch_p2m_generic(c, level, nleaf, list, sbegin);
+}
 
 void launch_p2m(bem_ctx *c)
 {
-    const int p = c->p;
-    if (p <= 4) p2m_launch<4>(c);
-    else if (p <= 6) p2m_launch<6>(c);
-    else if (p <= 8) p2m_launch<8>(c);
-    else if (p <= 10) p2m_launch<10>(c);
-    else if (p <= 12) p2m_launch<12>(c);
-    else if (p <= 14) p2m_launch<14>(c);
-    else if (p <= 16) p2m_launch<16>(c);
-    else launch_p2m_generic(c);
+    if (!c->adaptive) { launch_p2m_level(c, c->sb.lmax, c->sb.nbox[c->sb.lmax], nullptr, c->sb.begin.get()); return; }
+    for (int l = 2; l <= c->sb.lmax; ++l)                         // adaptive tree: the source leaves of every level
+        launch_p2m_level(c, l, c->ad.n_sleaf[l], c->ad.sleaf[l].get(), c->ad.s_pbeg[l].get());
 }
 
 // ------------------------------------------------------------------ L2P
@@ -213,11 +222,13 @@ void launch_p2m(bem_ctx *c)
 template <int P>
 __global__ void __launch_bounds__(128)
 l2p_kernel_t(const double *__restrict__ tgt, int64_t nt, const int32_t *__restrict__ leaf_of, const uint64_t *__restrict__ tkey,
-             double cmx, double cmy, double cmz, double h, int p, int nst, const double *__restrict__ Lleaf, double *__restrict__ y)
+             const uint8_t *__restrict__ lev_all, double cmx, double cmy, double cmz, double h, int p, int nst,
+             const double *__restrict__ Lleaf, double *__restrict__ y)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nt) return;
     const int leaf = leaf_of[t];
+    if (lev_all) h = ldexp(h, -(int)lev_all[leaf]);              // adaptive tree: leaf_of / tkey / Lleaf are indexed by the global box id; h = cube side
     uint32_t ix, iy, iz;
     morton_decode(tkey[leaf], &ix, &iy, &iz);
     const double ih = 1.0 / h;
@@ -251,7 +262,12 @@ static void l2p_launch(bem_ctx *c, const int32_t *leaf_of)
     const BoxSet &tb = c->tb;
     const int lmax = tb.lmax;
     const double h = c->cube_side / (double)(1 << lmax);
-    l2p_kernel_t<P><<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, leaf_of, tb.bkey[lmax].get(),
+    if (c->adaptive)
+        l2p_kernel_t<P><<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->ad.pt_gbox.get(), c->ad.tkey_all.get(), c->ad.tlev_all.get(),
+                                                                c->cube_min[0], c->cube_min[1], c->cube_min[2], c->cube_side, c->p, c->nst,
+                                                                c->Lexp.get(), c->ypart.get());
+    else
+    l2p_kernel_t<P><<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, leaf_of, tb.bkey[lmax].get(), nullptr,
                                                             c->cube_min[0], c->cube_min[1], c->cube_min[2], h, c->p, c->nst,
                                                             c->Lexp.get() + (size_t)tb.base[lmax] * c->nst, c->ypart.get());
     KERNEL_CHECK();

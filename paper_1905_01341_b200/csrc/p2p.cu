@@ -183,7 +183,10 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
     const int leaf = blockIdx.x;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int t0 = tbegin[leaf], nt = tbegin[leaf + 1] - t0;
-    if (warp == 0) build_segments(lane, leaf, nbr, xptr, xsrc, sbegin, seg_s0, seg_pre, &seg_n, [](int, int) {});
+    if (warp == 0) {
+        if (nbr) build_segments(lane, leaf, nbr, xptr, xsrc, sbegin, seg_s0, seg_pre, &seg_n, [](int, int) {});
+        else build_segments_csr(lane, leaf, xptr, reinterpret_cast<const int2 *>(xsrc), seg_s0, seg_pre, &seg_n);   // adaptive tree
+    }
     __syncthreads();
     const int S = seg_pre[SEG_MAX];
     const int rounds = (S + P2P_THREADS - 1) / P2P_THREADS;
@@ -289,7 +292,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
 
 void launch_p2p_leaves(bem_ctx *c)
 {
-    const int nleaf = c->tb.nbox[c->tb.lmax];
+    const int nleaf = c->adaptive ? c->ad.n_tleaf : c->tb.nbox[c->tb.lmax];
     static std::vector<char> attr_done;
     if (first_use_on_device(attr_done, c->device)) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
@@ -298,8 +301,13 @@ void launch_p2p_leaves(bem_ctx *c)
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
     }
     const bool self = c->quadrature != 0;                       // V1 (j = i) and point clouds may have r = 0; G3 cannot
-#define BEM_LEAF(D, S) p2p_leaf_kernel<D, S><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), c->tb.begin.get(), c->nbr.get(), c->xdir_ptr.p, \
-                           c->xdir_src.p, c->sb.begin.get(), c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N)
+    // adaptive tree: target leaves in point order (ad.tleaf_begin), source ranges from the CSR (ad.near_ptr, ad.near_rng), nbr = null
+    const int32_t *tbeg = c->adaptive ? c->ad.tleaf_begin.get() : c->tb.begin.get();
+    const int32_t *nbr = c->adaptive ? nullptr : c->nbr.get();
+    const int32_t *xp = c->adaptive ? c->ad.near_ptr.get() : c->xdir_ptr.p;
+    const int32_t *xs = c->adaptive ? reinterpret_cast<const int32_t *>(c->ad.near_rng.get()) : c->xdir_src.p;
+#define BEM_LEAF(D, S) p2p_leaf_kernel<D, S><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), tbeg, nbr, xp, \
+                           xs, c->sb.begin.get(), c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N)
     if (c->has_dipole) { if (self) BEM_LEAF(true, true); else BEM_LEAF(true, false); }
     else { if (self) BEM_LEAF(false, true); else BEM_LEAF(false, false); }
 #undef BEM_LEAF

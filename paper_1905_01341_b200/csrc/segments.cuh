@@ -9,7 +9,7 @@
 
 namespace bem {
 
-constexpr int SEG_MAX = 224;          // 27 + 189 segments, rounded up to a multiple of 32
+constexpr int SEG_MAX = 256;          // 27 + 189 segments (uniform tree), rounded up; the longest CSR row an adaptive tree may have
 
 // called by warp 0 of the CTA; per_segment(k, b) is called by the lane that owns segment k (b = source leaf or -1)
 template <class F>
@@ -31,6 +31,27 @@ __device__ __forceinline__ void build_segments(int lane, int leaf, const int32_t
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
         if (e < SEG_MAX) { seg_s0[e] = s0; seg_pre[e + 1] = run + inc; per_segment(e, b); }
+        run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) { seg_pre[0] = 0; *seg_n = nseg; }
+    for (int e = ((nseg + 31) & ~31) + lane; e < SEG_MAX; e += 32) seg_pre[e + 1] = run;
+}
+
+// adaptive tree (adaptive.cu): the source list of a target leaf is a CSR row of (first source, count) ranges -- the boxes of
+// its own level that touch it, the coarser source leaves that touch its ancestors, and the far leaves summed directly
+__device__ __forceinline__ void build_segments_csr(int lane, int leaf, const int32_t *__restrict__ near_ptr, const int2 *__restrict__ near_rng,
+                                                   int *seg_s0, int *seg_pre, int *seg_n)
+{
+    const int x0 = near_ptr[leaf], nseg = min(near_ptr[leaf + 1] - x0, SEG_MAX);     // bem_setup refuses longer rows
+    int run = 0;
+    for (int base = 0; base < nseg; base += 32) {
+        const int e = base + lane;
+        int2 r = make_int2(0, 0);
+        if (e < nseg) r = near_rng[x0 + e];
+        int inc = r.y;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += v; }
+        if (e < SEG_MAX) { seg_s0[e] = r.x; seg_pre[e + 1] = run + inc; }
         run += __shfl_sync(0xffffffffu, inc, 31);
     }
     if (lane == 0) { seg_pre[0] = 0; *seg_n = nseg; }

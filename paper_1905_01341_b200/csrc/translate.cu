@@ -617,17 +617,20 @@ constexpr int RED_CHUNK = 192;     // pairs of a target staged at a time (an M2L
 __global__ void __launch_bounds__(160)
 translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t, const int32_t *__restrict__ mat_ne,
                  const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-                 int nre, int accumulate, int ntgt, double *__restrict__ out)
+                 int nre, int accumulate, int ntgt, const int32_t *__restrict__ list, double *__restrict__ out)
 {
+    // accumulate: 0 = overwrite (an empty list writes zeros), 1 = add to the output, 2 = overwrite but leave the output of an
+    // empty list alone (adaptive tree: a parent without children is a leaf whose multipoles P2M wrote).
     // A row of a graded (truncated) translation holds the leading mat_ne[matrix] dofs only; the rest of the scratch row was
     // never written.  (matrix id | dofs << 16) of the target's pairs is staged in shared memory so that the row loads do
     // not wait for a global load of their predicate.
     __shared__ int s_mt[RED_CHUNK];
     const int nst = 2 * nre;
-    for (int t = blockIdx.x; t < ntgt; t += gridDim.x) {            // grid < ntgt: a persistent pass (see launch_stage_reduce)
+    for (int ti = blockIdx.x; ti < ntgt; ti += gridDim.x) {         // grid < ntgt: a persistent pass (see launch_stage_reduce)
+        const int t = list ? list[ti] : ti;                            // adaptive tree: only the boxes that exist are visited
         const int b = ptr[t], e = ptr[t + 1];
         double *o = out + (size_t)t * nst;
-        if (b == e && !accumulate)
+        if (b == e && accumulate == 0)
             for (int cc = threadIdx.x; cc < nst; cc += blockDim.x) o[cc] = 0.0;
         for (int k0 = b; k0 < e; k0 += RED_CHUNK) {                 // one round for every list the library builds
             const int n = min(RED_CHUNK, e - k0);
@@ -655,7 +658,7 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
                         }
                     }
                 }
-                if (accumulate || k0 > b) { sr += o[cc]; si += o[cc + nre]; }
+                if (accumulate == 1 || k0 > b) { sr += o[cc]; si += o[cc + nre]; }
                 o[cc] = sr;
                 o[cc + nre] = si;
             }
@@ -694,13 +697,15 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
 {
     if (st.ntgt == 0) return;
     double *out = (st.out_is_local ? c->Lexp.get() : c->Mexp.get()) + (size_t)st.out_base * c->nst;
-    const int grid = ctas_per_sm > 0 ? std::min(st.ntgt, c->n_sm * ctas_per_sm) : st.ntgt;
+    const int nvisit = st.n_list >= 0 ? st.n_list : st.ntgt;
+    if (nvisit == 0) return;
+    const int grid = ctas_per_sm > 0 ? std::min(nvisit, c->n_sm * ctas_per_sm) : nvisit;
     static std::vector<char> attr_done;
     if (first_use_on_device(attr_done, c->device))                     // same carve-out as the pair kernels it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
         st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
-        c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : 0, st.ntgt, out);
+        c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : (st.keep_empty ? 2 : 0), nvisit, st.n_list >= 0 ? st.tgt_list.get() : nullptr, out);
     KERNEL_CHECK();
 }
 
@@ -723,14 +728,15 @@ void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce)
 constexpr int P2M_WARPS_G = 4;
 
 __global__ void __launch_bounds__(P2M_WARPS_G * 32)
-p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, int nleaf, int level,
+p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey, const int32_t *__restrict__ list, int nleaf, int level,
            double cmx, double cmy, double cmz, double h,
            const double4 *__restrict__ spos, const double4 *__restrict__ sstr, int p, int nre, int nst, double *__restrict__ Mout)
 {
     extern __shared__ double sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int leaf = blockIdx.x * P2M_WARPS_G + warp;
+    int leaf = blockIdx.x * P2M_WARPS_G + warp;
     if (leaf >= nleaf) return;
+    if (list) leaf = list[leaf];
     double *tbl = sm + (size_t)warp * (2 * p - 1) * 33;            // [2l+1 values][33]
     uint32_t ix, iy, iz;
     morton_decode(skey[leaf], &ix, &iy, &iz);
@@ -794,15 +800,15 @@ p2m_kernel(const int32_t *__restrict__ sbegin, const uint64_t *__restrict__ skey
     }
 }
 
-void launch_p2m_generic(bem_ctx *c)
+void launch_p2m_generic(bem_ctx *c, int lmax, int nleaf, const int32_t *list, const int32_t *sbegin)
 {
     const BoxSet &sb = c->sb;
-    const int lmax = sb.lmax, nleaf = sb.nbox[lmax];
+    if (nleaf == 0) return;
     const double h = c->cube_side / (double)(1 << lmax);
     const size_t smem = (size_t)P2M_WARPS_G * (2 * c->p - 1) * 33 * sizeof(double);
     if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(p2m_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     p2m_kernel<<<cdiv(nleaf, P2M_WARPS_G), P2M_WARPS_G * 32, smem, c->stream>>>(
-        sb.begin.get(), sb.bkey[lmax].get(), nleaf, lmax, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
+        sbegin, sb.bkey[lmax].get(), list, nleaf, lmax, c->cube_min[0], c->cube_min[1], c->cube_min[2], h,
         c->src_pos.get(), c->src_str.get(), c->p, c->nre, c->nst, c->Mexp.get() + (size_t)sb.base[lmax] * c->nst);
     KERNEL_CHECK();
 }
@@ -812,11 +818,13 @@ void launch_p2m_generic(bem_ctx *c)
 // One thread per target; threads of a warp mostly share the leaf, so coefficient loads are broadcasts.
 __global__ void __launch_bounds__(128)
 l2p_kernel(const double *__restrict__ tgt, int64_t nt, const int32_t *__restrict__ leaf_of, const uint64_t *__restrict__ tkey,
-           double cmx, double cmy, double cmz, double h, int p, int nre, int nst, const double *__restrict__ Lleaf, double *__restrict__ y)
+           const uint8_t *__restrict__ lev_all, double cmx, double cmy, double cmz, double h, int p, int nre, int nst,
+           const double *__restrict__ Lleaf, double *__restrict__ y)
 {
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nt) return;
     const int leaf = leaf_of[t];
+    if (lev_all) h = ldexp(h, -(int)lev_all[leaf]);               // adaptive tree: global box ids, h = cube side
     uint32_t ix, iy, iz;
     morton_decode(tkey[leaf], &ix, &iy, &iz);
     const double ih = 1.0 / h;
@@ -854,7 +862,12 @@ void launch_l2p_generic(bem_ctx *c, const int32_t *leaf_of)
     const BoxSet &tb = c->tb;
     const int lmax = tb.lmax;
     const double h = c->cube_side / (double)(1 << lmax);
-    l2p_kernel<<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, leaf_of, tb.bkey[lmax].get(),
+    if (c->adaptive)
+        l2p_kernel<<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, c->ad.pt_gbox.get(), c->ad.tkey_all.get(), c->ad.tlev_all.get(),
+                                                           c->cube_min[0], c->cube_min[1], c->cube_min[2], c->cube_side, c->p, c->nre, c->nst,
+                                                           c->Lexp.get(), c->ypart.get());
+    else
+    l2p_kernel<<<cdiv(c->N, 128), 128, 0, c->stream>>>(c->tgt_pos.get(), c->N, leaf_of, tb.bkey[lmax].get(), nullptr,
                                                        c->cube_min[0], c->cube_min[1], c->cube_min[2], h, c->p, c->nre, c->nst,
                                                        c->Lexp.get() + (size_t)tb.base[lmax] * c->nst, c->ypart.get());
     KERNEL_CHECK();

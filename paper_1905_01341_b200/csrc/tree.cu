@@ -6,6 +6,7 @@
 // bit-interleaving followed by a sorting algorithm)".
 #include "common.cuh"
 #include "morton.cuh"
+#include "lists.cuh"
 
 namespace bem {
 
@@ -114,13 +115,6 @@ void boxset_build(BoxSet &bs, int lmax, const int counts[22], cudaStream_t s)
 }
 
 // ------------------------------------------------------------------ lists
-__device__ __forceinline__ int find_box(const uint64_t *keys, int n, uint64_t k)
-{
-    int lo = 0, hi = n;
-    while (lo < hi) { const int mid = (lo + hi) >> 1; if (keys[mid] < k) lo = mid + 1; else hi = mid; }
-    return (lo < n && keys[lo] == k) ? lo : -1;
-}
-
 // source leaves adjacent to (or equal to) each target leaf, in fixed (dz, dy, dx) order, -1 padded
 __global__ void neighbour_lists(const uint64_t *tkey, int ntb, const uint64_t *skey, int nsb, int level, int32_t *nbr,
                                 const int32_t *tbegin, const int32_t *sbegin, unsigned long long *pair_count)
@@ -142,58 +136,6 @@ __global__ void neighbour_lists(const uint64_t *tkey, int ntb, const uint64_t *s
             }
     for (int k = cnt; k < 27; ++k) nbr[(int64_t)t * 27 + k] = -1;
     atomicAdd(pair_count, ns * (unsigned long long)(tbegin[t + 1] - tbegin[t]));
-}
-
-// Interaction (V) list of target box t at `level`: source boxes that are children of the
-// parent's neighbours and not adjacent to t.
-// count pass (src == nullptr) or fill pass.
-__global__ void interaction_lists(const uint64_t *tkey, int ntb, int level,
-                                  const uint64_t *skey_parent, int nsb_parent, const int32_t *schild_parent,
-                                  const uint64_t *skey, const int32_t *tparent, int sbase, int tbase_parent,
-                                  int32_t *count, const int32_t *ptr, int32_t *src, int32_t *mat,
-                                  const int32_t *tbegin, const int32_t *sbegin, int64_t direct_max,
-                                  int32_t *xcount, const int32_t *xptr, int32_t *xsrc, unsigned long long *xpairs)
-{
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ntb) return;
-    uint32_t ix, iy, iz;
-    morton_decode(tkey[t], &ix, &iy, &iz);
-    const int px = ix >> 1, py = iy >> 1, pz = iz >> 1;
-    const int lim = 1 << (level - 1);
-    int cnt = 0;
-    int w = ptr ? ptr[t] : 0;
-    // leaf level, direct_max > 0: a pair whose boxes hold nt x ns <= direct_max point pairs costs less summed directly
-    // than translated (one M2L = 4 nre^2 flop whatever the boxes hold): it goes to the near field (list xsrc) instead
-    const int64_t ntp = direct_max > 0 ? tbegin[t + 1] - tbegin[t] : 0;
-    int xc = 0, xw = xptr ? xptr[t] : 0;
-    unsigned long long xp = 0;
-    for (int dz = -1; dz <= 1; ++dz)
-        for (int dy = -1; dy <= 1; ++dy)
-            for (int dx = -1; dx <= 1; ++dx) {
-                const int x = px + dx, y = py + dy, z = pz + dz;
-                if (x < 0 || y < 0 || z < 0 || x >= lim || y >= lim || z >= lim) continue;
-                const int pb = find_box(skey_parent, nsb_parent, morton_encode(x, y, z));
-                if (pb < 0) continue;
-                for (int c = schild_parent[pb]; c < schild_parent[pb + 1]; ++c) {
-                    uint32_t cx, cy, cz;
-                    morton_decode(skey[c], &cx, &cy, &cz);
-                    const int ox = (int)ix - (int)cx, oy = (int)iy - (int)cy, oz = (int)iz - (int)cz;   // target - source
-                    if (max(max(abs(ox), abs(oy)), abs(oz)) < 2) continue;                           // adjacent: near field
-                    if (direct_max > 0) {
-                        const int64_t nsp = sbegin[c + 1] - sbegin[c];
-                        if (ntp * nsp <= direct_max) {
-                            if (xsrc) xsrc[xw++] = c;
-                            ++xc;
-                            xp += (unsigned long long)(ntp * nsp);
-                            continue;
-                        }
-                    }
-                    if (src) { src[w] = sbase + c; mat[w] = MAT_M2L + (ox + 3) + 7 * (oy + 3) + 49 * (oz + 3); ++w; }
-                    ++cnt;
-                }
-            }
-    if (count) count[t] = cnt;
-    if (xcount) { xcount[t] = xc; if (xp) atomicAdd(xpairs, xp); }
 }
 
 // pairs the near-field kernel EXECUTES: it pads the concatenated source list of a target leaf (neighbours + direct far
@@ -249,7 +191,7 @@ constexpr int GEMM_TM = 64;   // rows per GEMM tile (translate.cu uses the same 
 
 
 // from target-major (src, mat) pairs to a Stage: rows sorted by matrix, tiles, inverse positions
-static void finish_stage(bem_ctx *c, Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cudaStream_t s)
+void finish_stage(bem_ctx *c, Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat, cudaStream_t s)
 {
     const int64_t n = st.npairs;
     st.src_sorted.alloc(n);
@@ -337,7 +279,7 @@ void build_lists(bem_ctx *c)
         interaction_lists<<<cdiv(nt, 128), 128, 0, s>>>(tb.bkey[l].get(), nt, l, sb.bkey[l - 1].get(), sb.nbox[l - 1], sb.child[l - 1].get(),
                                                         sb.bkey[l].get(), l > 2 ? tb.parent[l].get() : nullptr, sb.base[l],
                                                         l > 2 ? tb.base[l - 1] : 0, cnt.get(), nullptr, nullptr, nullptr,
-                                                        tb.begin.get(), sb.begin.get(), dmax, dmax > 0 ? xcnt.get() : nullptr, nullptr, nullptr, pc.get());
+                                                        tb.begin.get(), sb.begin.get(), dmax, dmax > 0 ? xcnt.get() : nullptr, nullptr, nullptr, pc.get(), AdaptiveFlags());
         KERNEL_CHECK();
         if (dmax > 0) {
             scan_exclusive_i32(xcnt.get(), c->xdir_ptr.get(), nt, s);
@@ -360,7 +302,7 @@ void build_lists(bem_ctx *c)
                                                         sb.bkey[l].get(), l > 2 ? tb.parent[l].get() : nullptr, sb.base[l],
                                                         l > 2 ? tb.base[l - 1] : 0, nullptr, st.ptr.get(), src.get(), mat.get(),
                                                         tb.begin.get(), sb.begin.get(), dmax, nullptr, dmax > 0 ? c->xdir_ptr.get() : nullptr,
-                                                        dmax > 0 ? c->xdir_src.get() : nullptr, pc.get());
+                                                        dmax > 0 ? c->xdir_src.get() : nullptr, pc.get(), AdaptiveFlags());
         KERNEL_CHECK();
         finish_stage(c, st, src, mat, s);
         c->m2l_pairs += total;

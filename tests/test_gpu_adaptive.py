@@ -1,0 +1,121 @@
+"""The adaptive octree (option tree = 1, reading R9 stage 2; csrc/adaptive.cu) against the CPU oracle at
+the tolerances of the uniform tree, through the C-ABI.  `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import bem_inputs as bi
+from bem_inputs.configs import make_config, sample_rows
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _rel(a, b):
+    return np.linalg.norm(a - b) / np.linalg.norm(b)
+
+
+def _bem():
+    import paper_1905_01341_b200 as bem
+    return bem
+
+
+def _run(c, rows, q="q", phi="phi", p=None, leaf=None, **opts):
+    ctx = _bem().bem_create(c["V"], c["F"], c.get("bubble_id"))
+    ctx.bem_set_option("tree", 1)
+    for k, v in opts.items():
+        ctx.bem_set_option(k, v)
+    ctx.bem_setup(p or c["p"], leaf or c["leaf_size"], c["eta"])
+    N = c["V"].shape[0]
+    y, y2 = np.full(N, np.nan), np.full(N, np.nan)
+    qq, pp = (None if q is None else c[q]), (None if phi is None else c[phi])
+    ctx.bem_apply(qq, pp, y)
+    ctx.bem_apply(qq, pp, y2)
+    st = ctx.bem_get_stats()
+    ctx.bem_destroy()
+    assert np.isfinite(y).all() and np.array_equal(y, y2)                     # bit-reproducible
+    return y, st
+
+
+@pytest.mark.parametrize("n,nb", [(1, None), (2, None), (3, None), (4, 60), (5, 150)])
+def test_adaptive_tree_meets_the_fmm_tolerances(n, nb):
+    """North_star tolerance at the stated p (S - D <= 1e-5) and Table 1's for the single layer, on every config (4 and 5
+    shrunken), with leaves on several levels; <= 1e-8 at p = 24 on configs 1-2."""
+    c = make_config(n) if nb is None else make_config(n, n_bubbles=nb)
+    N = c["V"].shape[0]
+    rows = np.arange(N, dtype=np.int64) if N < 3000 else sample_rows(n, N, 1000)
+    yo = oracle.g3_apply(c["V"], c["F"], c["q"], c["phi"], eta=c["eta"], rows=rows)
+    yoS = oracle.g3_apply(c["V"], c["F"], c["q"], None, eta=c["eta"], rows=rows)
+    y, st = _run(c, rows)
+    yS, _ = _run(c, rows, phi=None)
+    eB, eS = _rel(y[rows], yo), _rel(yS[rows], yoS)
+    print(f"cfg{n} adaptive p={c['p']}: S {eS:.2e}, S-D {eB:.2e}; lmax {st['lmax']:.0f}, leaves {st['n_src_leaves']:.0f} / {st['n_tgt_leaves']:.0f}, "
+          f"m2l pairs {st['m2l_pairs']:.0f}, point pairs {st['p2p_pairs']:.3e} ({st['p2p_pairs_executed']:.3e} executed)")
+    table1 = {8: 1e-5, 10: 2.2e-6, 12: 5e-7}
+    assert st["m2l_pairs"] > 0 and eB <= 1e-5 and eS <= 3.0 * table1[c["p"]]
+    if n <= 2:
+        yh, _ = _run(c, rows, p=24)
+        assert _rel(yh[rows], yo) <= 1e-8
+
+
+def test_adaptive_tree_depth_controls_and_quadratures():
+    """leaf_size 1 .. huge, a capped depth (option lmax), a lower minimum level (leaves on MANY levels), direct_pairs off /
+    all, and the paper's V1 quadrature (coincident source and target) all give the same product up to truncation."""
+    c = make_config(1)
+    N = c["V"].shape[0]
+    rows = np.arange(N, dtype=np.int64)
+    yo = oracle.g3_apply(c["V"], c["F"], c["q"], c["phi"], eta=c["eta"])
+    for opts in (dict(leaf=1), dict(leaf=8), dict(leaf=100000), dict(leaf=16, lmax=3), dict(leaf=8, tree_min_level=2),
+                 dict(leaf=24, tree_min_level=2, direct_pairs=0), dict(leaf=24, tree_min_level=2, direct_pairs=10 ** 9)):
+        leaf = opts.pop("leaf")
+        y, st = _run(c, rows, p=12, leaf=leaf, **opts)
+        e = _rel(y, yo)
+        print(f"leaf {leaf} {opts}: {e:.2e}, lmax {st['lmax']:.0f}, tgt leaves {st['n_tgt_leaves']:.0f}")
+        assert e <= 3e-5                                      # the bound of test_fmm_leaf_size_one_and_huge (uniform tree, p = 12)
+    yv = oracle.v1_apply(c["V"], c["F"], c["q"], c["phi"])
+    y, _ = _run(c, rows, p=12, leaf=8, quadrature=1, tree_min_level=2)
+    assert _rel(y, yv) <= 3e-5
+
+
+def test_adaptive_tree_on_a_strongly_non_uniform_cloud():
+    """Where the adaptive tree is for: 90% of the points in a ball of 1% of the cube's edge.  The uniform rule stops at the
+    depth the MEAN population gives and leaves the ball in a handful of boxes; the adaptive tree keeps refining there.
+    Both meet the tolerance; the adaptive one does it with a fraction of the point pairs."""
+    rng = np.random.default_rng(77)
+    n = 60000
+    dense = 0.5 + 0.005 * rng.normal(size=(int(0.9 * n), 3))
+    pts = np.vstack([dense, rng.uniform(0, 1, size=(n - dense.shape[0], 3))])
+    m = rng.uniform(-1, 1, size=n)
+    rows = np.sort(rng.choice(n, 300, replace=False))
+    yo = oracle.monopole_sum(pts, m, pts[rows])
+    res = {}
+    for tree in (0, 1):
+        ctx = _bem().bem_create_points(pts, pts)
+        ctx.bem_set_option("tree", tree)
+        ctx.bem_setup(12, 64, 2.5)
+        y = np.full(n, np.nan)
+        ctx.bem_apply(m, None, y)
+        st = ctx.bem_get_stats()
+        ctx.bem_destroy()
+        res[tree] = (_rel(y[rows], yo), st["p2p_pairs"], st["lmax"])
+        print(f"tree {tree}: error {res[tree][0]:.2e}, point pairs {st['p2p_pairs']:.3e}, lmax {st['lmax']:.0f}, m2l pairs {st['m2l_pairs']:.0f}")
+    assert res[0][0] <= 1e-5 and res[1][0] <= 1e-5
+    assert res[1][1] < 0.2 * res[0][1] and res[1][2] > res[0][2]
+
+
+def test_adaptive_tree_evaluator_and_refusals():
+    bem = _bem()
+    V, F = bi.icosphere(3)
+    rng = np.random.default_rng(5)
+    q, ph = rng.normal(size=V.shape[0]), rng.normal(size=V.shape[0])
+    X = V[rng.choice(V.shape[0], 1500)] * rng.uniform(1.05, 2.5, size=(1500, 1))
+    mesh = bem.bem_create(V, F, None)
+    ev = bem.bem_create_evaluator(mesh, X)
+    ev.bem_set_option("tree", 1)
+    ev.bem_setup(12, 32, 2.5)
+    u = np.full(X.shape[0], np.nan)
+    ev.bem_apply(q, ph, u)
+    assert _rel(u, oracle.g3_evaluate(V, F, q, ph, X, eta=2.5)) <= 1e-5
+    ev.bem_set_option("p2p_precision", 1)                      # fp32 pairs need leaves of one size
+    with pytest.raises(bem.BemError):
+        ev.bem_apply(q, ph, u)
+    ev.bem_destroy(); mesh.bem_destroy()
