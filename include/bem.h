@@ -172,7 +172,7 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   convention.  Products without dipoles (every GMRES iteration) always use p.
  *   "m2l_order_radius", "m2l_order_extra"  graded truncation of the M2L translations: the offset o (in box edges) uses
  *                   the degrees < p_o = ceil(p ln k(2) / ln k(|o|)) + extra, k(d) = a / (d - a), a = radius (default
- *                   0.5, extra 1: error against the oracle unchanged within 7% on every config, executed M2L work
+ *                   0.5, extra 1: error against the direct sum unchanged within 7% on every config, executed M2L work
  *                   x0.54 at p = 12); radius 0 = every translation uses all p degrees.
  *   "timing"        1 = record per-kernel-class CUDA-event timings in bem_apply
  *   "gemm_path"     batched translations (M2M, M2L, L2L): 0 = FP64 tensor-core tiles (DMMA; p <= 16,
