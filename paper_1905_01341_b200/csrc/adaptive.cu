@@ -442,7 +442,6 @@ void build_adaptive(bem_ctx *c)
         st.scratch_off = 0;
         max_pairs = std::max<int64_t>(max_pairs, total);
     }
-    c->scratch.alloc((size_t)max_pairs * c->lay[c->n_lay - 1].nst);
 
     // direct source ranges of the target leaves
     for (int l = 0; l <= lmax; ++l) { L.x_ptr[l] = ad.x_ptr[l].p; L.x_src[l] = ad.x_src[l].p; }

@@ -24,6 +24,7 @@ int adaptive_source_flags(bem_ctx *c, bool *want_deeper);
 void build_adaptive(bem_ctx *c);
 // translate.cu
 void build_matrices(bem_ctx *c, FmmLayout &L);
+void pack_scratch(bem_ctx *c);
 void launch_stage(bem_ctx *c, const Stage &st, int cls_gemm, int cls_reduce);
 void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stream);
 void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int ctas_per_sm);
@@ -133,7 +134,7 @@ void activate_layout(bem_ctx *c, int i)
     c->lay_active = i;
     c->p = L.p; c->pl = L.pl; c->nre = L.nre; c->nst = L.nst;
     c->mats.p = L.mats.get(); c->rot.p = L.rot.get(); c->kinfo.p = L.kinfo.get();
-    c->mat_ne.p = L.mat_ne.get(); c->mat_cls.p = L.mat_cls.get();
+    c->mat_ne.p = L.mat_ne.get(); c->mat_cls.p = L.mat_cls.get(); c->mat_w.p = L.mat_w.get();
     c->m2l_row_bytes = L.m2l_row_bytes;
 }
 // executed work of the M2L tiles of one product with this layout (bem_get_stats), from the pairs per matrix
@@ -144,7 +145,7 @@ static void layout_stats(const bem_ctx *c, FmmLayout &L)
     for (int m = 0; m < MAT_L2L; ++m) {
         const double kr = dmma ? 4.0 * ke_of(L.pl - L.mat_cls_host[m]) : (double)L.nre;
         L.m2l_flop += c->m2l_hist[m] * 4.0 * kr * kr;
-        L.m2l_row_bytes += c->m2l_hist[m] * 16.0 * L.mat_ne_host[m];
+        L.m2l_row_bytes += c->m2l_hist[m] * 16.0 * L.mat_w_host[m];
     }
 }
 
@@ -396,6 +397,7 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
         }
         if (c->adaptive) build_adaptive(c);
         else build_lists(c);
+        pack_scratch(c);
         for (int i = 0; i < c->n_lay; ++i) layout_stats(c, c->lay[i]);
         activate_layout(c, 0);
         c->nsplit = 2;                                  // far field (L2P) and near field (P2P) partial sums

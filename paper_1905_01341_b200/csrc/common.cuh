@@ -138,7 +138,12 @@ __host__ __device__ constexpr int ke_of(int pp) { return pp < 2 ? 2 : 2 * ((pp *
 constexpr int TILES_ALL = 0, TILES_SPLIT = 1, TILES_DENSE = 2;
 struct Stage {
     int64_t npairs = 0;
-    int64_t scratch_off = 0;        // first scratch row of the stage (every M2L level has its own region; M2M stages alias row 0)
+    int64_t scratch_off = 0;        // order of the regions: pairs of the stages before this one (M2M / L2L stages alias region 0)
+    // packed scratch rows (translate.cu pack_scratch), per truncation layout: the row of pair k (target-major) holds the
+    // 2 W dofs its matrix class computes (W real parts, then W imaginary parts) at row_off[k] units of 16 doubles from the
+    // start of the stage's region, which starts region_units units into the scratch buffer
+    dvec<int32_t> row_off[2];
+    int64_t region_units[2] = {0, 0};
     int ntgt = 0;
     int out_base = 0;               // global index of the first target box
     bool out_is_local = false;      // output array: local (L) or multipole (M) expansions
@@ -185,6 +190,8 @@ struct FmmLayout {
     dvec<int32_t> kinfo;            // [nst] order m of every stored dof (0 for padding)
     dvec<int32_t> mat_ne;           // [N_MATS] leading dofs of either block that take part in the translation (graded truncation)
     dvec<int32_t> mat_cls;          // [N_MATS] truncation class of the M2L tiles of the matrix: min(M2L_NCLS - 1, pl - p_o)
+    dvec<int32_t> mat_w;            // [N_MATS] dofs of either block a translated row of the matrix stores: 4 ke_of(pl - class) (M2M / L2L: nre)
+    std::vector<int32_t> mat_w_host;
     std::vector<int32_t> mat_ne_host, mat_cls_host;
     double m2l_flop = 0;            // executed flop of the M2L tiles of one product: 4 (4 KE)^2 per pair, KE the k-steps of its class
     double m2l_row_bytes = 0;       // bytes of translated rows the sums read per product: 16 x dofs carried per pair
@@ -266,7 +273,7 @@ struct bem_ctx {
     int64_t direct_max_eff = 0;
     bem::dptr<double> mats;         // views of the active layout (FmmLayout)
     bem::dptr<double2> rot;
-    bem::dptr<int32_t> kinfo, mat_ne, mat_cls;
+    bem::dptr<int32_t> kinfo, mat_ne, mat_cls, mat_w;
     double m2l_hist[bem::MAT_L2L] = {0};   // M2L pairs per matrix over all levels (statistics of the layouts)
     double m2l_order_radius = 0.5;  // option "m2l_order_radius": cluster radius a (box edges) of the graded truncation, 0 = off
     int m2l_order_extra = 1;        // option "m2l_order_extra": degrees added to the graded order of every offset

@@ -93,6 +93,11 @@ void build_matrices(bem_ctx *c, FmmLayout &L)
     }
     L.mat_ne_host = ne;
     L.mat_cls_host = cls;
+    std::vector<int32_t> mw(N_MATS, L.nre);                          // dofs per block a translated row stores (a multiple of 8)
+    for (int m = 0; m < MAT_L2L; ++m) mw[m] = std::min(L.nre, 4 * ke_of(L.pl - cls[m]));
+    L.mat_w_host = mw;
+    L.mat_w.alloc(N_MATS);
+    CUDA_TRY(cudaMemcpyAsync(L.mat_w.get(), mw.data(), N_MATS * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     L.mat_ne.alloc(N_MATS);
     L.mat_cls.alloc(N_MATS);
     CUDA_TRY(cudaMemcpyAsync(L.mat_ne.get(), ne.data(), N_MATS * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
@@ -142,7 +147,8 @@ __global__ void __launch_bounds__(GEMM_THREADS)
 translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
                const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-               int nst, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+               int nst, const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, const int32_t *__restrict__ mat_w,
+               double *__restrict__ scratch)
 {
     __shared__ double As[GEMM_KC][GEMM_TM + 4];
     __shared__ double Bs[GEMM_KC][GEMM_TN];
@@ -204,10 +210,17 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
     for (int i = 0; i < 4; ++i) {
         const int r = ty * 4 + i;
         if (r >= tile.nrows) continue;
-        double *out = scratch + (size_t)krow[tile.row0 + r] * nst + n0;
+        // packed row: the W leading dofs of the real parts, then of the imaginary parts (W = nre for M2M / L2L)
+        double *out = scratch + (size_t)row_off[krow[tile.row0 + r]] * 16;
+        const int W = mat_w[tile.mat], nre = nst >> 1;
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (n0 + tx + 16 * j < nst) out[tx + 16 * j] = acc[i][j];
+        for (int j = 0; j < 4; ++j) {
+            const int col = n0 + tx + 16 * j;
+            if (col < nst) {
+                const int part = col >= nre, cc = col - part * nre;
+                if (cc < W) out[part * W + cc] = acc[i][j];
+            }
+        }
     }
 }
 
@@ -291,7 +304,7 @@ __global__ void __launch_bounds__(DM_THREADS)
 translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
                const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-               const int32_t *__restrict__ krow, double *__restrict__ scratch)
+               const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, double *__restrict__ scratch)
 {
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S] (dense tiles: [2][2 NRE][DM_S_DENSE])
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
@@ -350,7 +363,7 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
             a[2 * j + 1] = v.y;
         }
     }
-    double *orow = scratch + (size_t)(rvalid ? krow[tile.row0 + row] : 0) * NST + 2 * lk;
+    double *orow = scratch + (size_t)(rvalid ? row_off[krow[tile.row0 + row]] : 0) * 16 + 2 * lk;     // dense rows are full rows
 
     for (int ch = 0; ch < nchunks; ++ch) {
         double *cur = (ch & 1) ? Bs1 : Bs0;
@@ -383,7 +396,8 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
 template <int KSH, int KE>
 __device__ __forceinline__ void m2l_body8(const Tile &tile, const int32_t *__restrict__ src_sorted, const double *__restrict__ Mexp,
                                           const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-                                          const int32_t *__restrict__ krow, double *__restrict__ scratch, double *dm_smem, double2 *cs_k)
+                                          const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, double *__restrict__ scratch,
+                                          double *dm_smem, double2 *cs_k)
 {
     constexpr int NRE = 4 * KSH, NST = 2 * NRE;               // layout of the stored rows and matrices
     constexpr int KR = 4 * KE;                                 // dofs of either block that take part
@@ -411,7 +425,7 @@ __device__ __forceinline__ void m2l_body8(const Tile &tile, const int32_t *__res
     for (int k = threadIdx.x; k < KR; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
     const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
     const double2 *ap = reinterpret_cast<const double2 *>(Mexp + (size_t)(arow < 0 ? 0 : arow) * NST) + lk;
-    double *orow = scratch + (size_t)(rvalid ? krow[tile.row0 + row] : 0) * NST + 2 * lk;
+    double *orow = scratch + (size_t)(rvalid ? row_off[krow[tile.row0 + row]] : 0) * 16 + 2 * lk;   // packed row: 2 KR dofs
     double a[KE];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
@@ -431,7 +445,7 @@ __device__ __forceinline__ void m2l_body8(const Tile &tile, const int32_t *__res
             }
         }
         const int t0 = CW * cl, nt = min(CW, NTH - t0);
-        dm_chunk<KE, 0, KE, 0>(a, cur, nt, lr, lk, rvalid, orow + blk * NRE + 8 * t0);
+        dm_chunk<KE, 0, KE, 0>(a, cur, nt, lr, lk, rvalid, orow + blk * KR + 8 * t0);
     }
 }
 
@@ -442,18 +456,19 @@ template <int PL>
 __global__ void __launch_bounds__(DM_THREADS, (ke_of(PL) <= 20 ? 3 : 2))
 translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                      const double *__restrict__ Mexp, const double *__restrict__ mats, const int32_t *__restrict__ mat_cls,
-                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow,
+                     const int32_t *__restrict__ row_off, double *__restrict__ scratch)
 {
     constexpr int KSH = ke_of(PL);
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
     const Tile tile = tiles[blockIdx.x];
     switch (__ldg(mat_cls + tile.mat)) {                        // truncation class of the tile's matrix (CTA-uniform)
-    case 0: m2l_body8<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    case 1: m2l_body8<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    case 2: m2l_body8<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    case 3: m2l_body8<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    default: m2l_body8<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 0: m2l_body8<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    case 1: m2l_body8<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    case 2: m2l_body8<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    case 3: m2l_body8<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    default: m2l_body8<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
     }
 }
 
@@ -489,7 +504,8 @@ __device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KE], const doub
 template <int KSH, int KE>
 __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__restrict__ src_sorted, const double *__restrict__ Mexp,
                                            const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-                                           const int32_t *__restrict__ krow, double *__restrict__ scratch, double *dm_smem, double2 *cs_k)
+                                           const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, double *__restrict__ scratch,
+                                           double *dm_smem, double2 *cs_k)
 {
     constexpr int NRE = 4 * KSH, NST = 2 * NRE;
     constexpr int KR = 4 * KE;
@@ -518,8 +534,8 @@ __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__re
     const int ar0 = v0 ? src_sorted[tile.row0 + row0] : -1, ar1 = v1 ? src_sorted[tile.row0 + row1] : -1;
     const double2 *ap0 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar0 < 0 ? 0 : ar0) * NST) + lk;
     const double2 *ap1 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar1 < 0 ? 0 : ar1) * NST) + lk;
-    double *o0 = scratch + (size_t)(v0 ? krow[tile.row0 + row0] : 0) * NST + 2 * lk;
-    double *o1 = scratch + (size_t)(v1 ? krow[tile.row0 + row1] : 0) * NST + 2 * lk;
+    double *o0 = scratch + (size_t)(v0 ? row_off[krow[tile.row0 + row0]] : 0) * 16 + 2 * lk;      // packed rows: 2 KR dofs
+    double *o1 = scratch + (size_t)(v1 ? row_off[krow[tile.row0 + row1]] : 0) * 16 + 2 * lk;
     double a0[KE], a1[KE];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
@@ -544,7 +560,7 @@ __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__re
                 }
             }
         }
-        const int t0 = CW * cl, nt = min(CW, NTH - t0), oc = blk * NRE + 8 * t0;
+        const int t0 = CW * cl, nt = min(CW, NTH - t0), oc = blk * KR + 8 * t0;
         switch (nt) {
         case 5: dm16_chunk_nt<KE, 5>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
         case 4: dm16_chunk_nt<KE, 4>(a0, a1, cur, lr, lk, v0, v1, o0 + oc, o1 + oc); break;
@@ -559,18 +575,19 @@ template <int PL>
 __global__ void __launch_bounds__(DM16_THREADS, 3)
 translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                        const double *__restrict__ Mexp, const double *__restrict__ mats, const int32_t *__restrict__ mat_cls,
-                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow, double *__restrict__ scratch)
+                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow,
+                     const int32_t *__restrict__ row_off, double *__restrict__ scratch)
 {
     constexpr int KSH = ke_of(PL);
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];
     const Tile tile = tiles[blockIdx.x];
     switch (__ldg(mat_cls + tile.mat)) {
-    case 0: m2l_body16<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    case 1: m2l_body16<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    case 2: m2l_body16<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    case 3: m2l_body16<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
-    default: m2l_body16<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, scratch, dm_smem, cs_k); break;
+    case 0: m2l_body16<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    case 1: m2l_body16<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    case 2: m2l_body16<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    case 3: m2l_body16<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    default: m2l_body16<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
     }
 }
 
@@ -599,15 +616,17 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
     if (which != TILES_DENSE && st.ntiles_split > 0) {
         if (PL == 12 && c->m2l_rows16)                           // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
             translate_dmma_split16<(PL == 12 ? PL : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
-                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
+                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), st.row_off[c->lay_active].get(), scratch);
         else
             translate_dmma_split<PL><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                   c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
+                                                                                   c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(),
+                                                                                   st.row_off[c->lay_active].get(), scratch);
     }
     if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
         translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
                                                                                       c->Mexp.get(), c->Lexp.get(), c->mats.get(),
-                                                                                      c->kinfo.get(), c->rot.get(), st.krow.get(), scratch);
+                                                                                      c->kinfo.get(), c->rot.get(), st.krow.get(),
+                                                                                      st.row_off[c->lay_active].get(), scratch);
 }
 
 // out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[k][:]   (fixed order; a_k = azimuth of
@@ -616,7 +635,7 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
 constexpr int RED_CHUNK = 192;     // pairs of a target staged at a time (an M2L list holds at most 189)
 __global__ void __launch_bounds__(160)
 translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t, const int32_t *__restrict__ mat_ne,
-                 const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+                 const int32_t *__restrict__ mat_w, const int32_t *__restrict__ row_off, const double *__restrict__ scratch, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
                  int nre, int accumulate, int ntgt, const int32_t *__restrict__ list, double *__restrict__ out)
 {
     // accumulate: 0 = overwrite (an empty list writes zeros), 1 = add to the output, 2 = overwrite but leave the output of an
@@ -624,7 +643,7 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
     // A row of a graded (truncated) translation holds the leading mat_ne[matrix] dofs only; the rest of the scratch row was
     // never written.  (matrix id | dofs << 16) of the target's pairs is staged in shared memory so that the row loads do
     // not wait for a global load of their predicate.
-    __shared__ int s_mt[RED_CHUNK];
+    __shared__ int s_mt[RED_CHUNK + 8], s_off[RED_CHUNK + 8], s_w[RED_CHUNK + 8];   // matrix | dofs << 16, row offset (16 doubles), dofs per block stored
     const int nst = 2 * nre;
     for (int ti = blockIdx.x; ti < ntgt; ti += gridDim.x) {         // grid < ntgt: a persistent pass (see launch_stage_reduce)
         const int t = list ? list[ti] : ti;                            // adaptive tree: only the boxes that exist are visited
@@ -635,23 +654,30 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
         for (int k0 = b; k0 < e; k0 += RED_CHUNK) {                 // one round for every list the library builds
             const int n = min(RED_CHUNK, e - k0);
             __syncthreads();
-            for (int i = threadIdx.x; i < n; i += blockDim.x) { const int mt = mat_t[k0 + i]; s_mt[i] = mt | (__ldg(mat_ne + mt) << 16); }
+            for (int i = threadIdx.x; i < n; i += blockDim.x) {
+                const int mt = mat_t[k0 + i];
+                s_mt[i] = mt | (__ldg(mat_ne + mt) << 16);
+                s_off[i] = row_off[k0 + i];
+                s_w[i] = __ldg(mat_w + mt);
+            }
             __syncthreads();
             for (int cc = threadIdx.x; cc < nre; cc += blockDim.x) {
                 const int m = kinfo[cc];
-                const double *base = scratch + (size_t)k0 * nst + cc;
+                const double *base = scratch + cc;
                 double sr = 0.0, si = 0.0;
+                // (a branch-free version that issues the 16 loads of 8 rows before using the first, reading the rows that do
+                // not carry dof cc at a dummy offset, measured SLOWER: 3.77 against 2.84 ms on config 5)
                 if (m == 0) {
 #pragma unroll 8
                     for (int i = 0; i < n; ++i)
-                        if (cc < (s_mt[i] >> 16)) sr += base[(size_t)i * nst];
+                        if (cc < (s_mt[i] >> 16)) sr += base[(size_t)s_off[i] * 16];
                 } else {
 #pragma unroll 8
                     for (int i = 0; i < n; ++i) {
                         const int mt = s_mt[i];
                         if (cc < (mt >> 16)) {
-                            const double *row = base + (size_t)i * nst;
-                            double vr = row[0], vi = row[nre];
+                            const double *row = base + (size_t)s_off[i] * 16;
+                            double vr = row[0], vi = row[s_w[i]];
                             azimuth(__ldg(rot + (size_t)(mt & 0xffff) * ROT_M + m), vr, vi);
                             sr += vr;
                             si += vi;
@@ -666,18 +692,57 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
     }
 }
 
+// ------------------------------------------------------------------ packed scratch rows (setup)
+__global__ void row_units(const int32_t *mat_t, int64_t n, const int32_t *mat_w, int32_t *u)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) u[k] = mat_w[mat_t[k]] >> 3;                       // 2 W doubles = W / 8 units of 16 doubles
+}
+// Row offsets of every stage for every truncation layout, and the scratch buffer.  The M2L stages of all levels have their
+// own regions (their tiles are all issued before the first sum when option overlap = 1); M2M and L2L stages run when no
+// M2L row is alive and alias the start of the buffer.
+void pack_scratch(bem_ctx *c)
+{
+    cudaStream_t s = c->stream;
+    int64_t need = 1;
+    for (int i = 0; i < c->n_lay; ++i) {
+        const FmmLayout &L = c->lay[i];
+        int64_t region = 0, top = 0;
+        auto pack = [&](Stage &st, bool own_region) {
+            if (st.ntgt == 0 && st.npairs == 0) return;
+            const int64_t n = st.npairs;
+            st.row_off[i].alloc(n + 1);
+            dvec<int32_t> u;
+            u.alloc(n);
+            if (n > 0) { row_units<<<cdiv(n, 256), 256, 0, s>>>(st.mat_t.get(), n, L.mat_w.get(), u.get()); KERNEL_CHECK(); }
+            scan_exclusive_i32(u.get(), st.row_off[i].get(), n, s);
+            int total = 0;
+            d2h_sync(&total, st.row_off[i].get() + n, sizeof(int), s);
+            st.region_units[i] = own_region ? region : 0;
+            if (own_region) region += total;
+            top = std::max(top, (own_region ? region : (int64_t)total));
+        };
+        for (auto &st : c->m2l) pack(st, true);
+        for (auto &st : c->m2m) pack(st, false);
+        for (auto &st : c->l2l) pack(st, false);
+        need = std::max(need, top);
+    }
+    c->scratch.alloc((size_t)need * 16);
+}
+
 // the tiles of a stage (which = all, only the M2L tiles, only the dense M2M / L2L tiles) on `stream`
 void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stream)
 {
     const int first = which == TILES_DENSE ? st.ntiles_split : 0;
     const int last = which == TILES_SPLIT ? st.ntiles_split : st.ntiles;
     if (st.ntgt == 0 || last <= first) return;
-    double *scratch = c->scratch.get() + (size_t)st.scratch_off * c->nst;
+    double *scratch = c->scratch.get() + (size_t)st.region_units[c->lay_active] * 16;
     const int pl = c->pl;
     if (c->gemm_path == 1 || pl > 16) {                         // plain-FMA tiles: p > 16, or forced (option "gemm_path")
         dim3 grid(last - first, cdiv(c->nst, GEMM_TN));
         translate_gemm<<<grid, GEMM_THREADS, 0, stream>>>(st.tiles.get() + first, st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, st.krow.get(), scratch);
+                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, st.krow.get(),
+                                                          st.row_off[c->lay_active].get(), c->mat_w.get(), scratch);
     }
     else if (pl == 4) launch_dmma<4>(c, st, which, stream, scratch);     // layout degree -> ke_of(pl) = nre / 4 k-steps per block
     else if (pl == 6) launch_dmma<6>(c, st, which, stream, scratch);
@@ -704,7 +769,8 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
     if (first_use_on_device(attr_done, c->device))                     // same carve-out as the pair kernels it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
-        st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->scratch.get() + (size_t)st.scratch_off * c->nst,
+        st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->mat_w.get(), st.row_off[c->lay_active].get(),
+        c->scratch.get() + (size_t)st.region_units[c->lay_active] * 16,
         c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : (st.keep_empty ? 2 : 0), nvisit, st.n_list >= 0 ? st.tgt_list.get() : nullptr, out);
     KERNEL_CHECK();
 }

@@ -359,7 +359,6 @@ void build_lists(bem_ctx *c)
         st.scratch_off = 0;
         max_pairs = std::max<int64_t>(max_pairs, nt);
     }
-    c->scratch.alloc((size_t)max_pairs * c->lay[c->n_lay - 1].nst);            // rows of the widest layout
 }
 
 }  // namespace bem
