@@ -195,6 +195,10 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   captured into a CUDA graph the second time the same (q, phi, y) is asked for and replayed from then
  *                   on -- one launch instead of 20-40 on the launch-bound small meshes.  Any bem_set_option,
  *                   bem_set_stream or bem_setup drops the captured graphs.  0: always launch kernel by kernel.
+ *                   The cache is keyed on the raw (q, phi, y, stream) addresses and holds no reference to the buffers:
+ *                   a replay reads and writes whatever lives at those addresses, so freeing a buffer and asking for a
+ *                   product with a new buffer that landed on the same address is fine, but a freed buffer must not be
+ *                   passed again; set "graph" 0 if the caller's allocator makes that hard to guarantee.
  *   "p2p_ctas"      fp32 near field: CTAs per SM of its persistent grid while the row sums share the SMs
  *                   (1..16; 0 = 4, default).  Tuning only. */
 bem_status bem_set_option(bem_ctx *ctx, const char *key, double value);

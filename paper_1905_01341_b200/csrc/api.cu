@@ -124,7 +124,9 @@ __global__ void v1_diag(const double *V, const double *nrm, const double *y0, co
 static void init_layout(FmmLayout &L, int p)
 {
     L.p = p;
-    L.pl = p <= 16 ? std::max(4, 2 * ((p + 1) / 2)) : p;      // template buckets 4, 6, .., 16 of the P2M / L2P / DMMA kernels
+    // template buckets of the P2M / L2P / DMMA kernels: the even degrees 4 .. 16, and 11 and 13 (what p = 8 and 10 become
+    // with three more degrees for the dipoles)
+    L.pl = p > 16 ? p : (p == 11 || p == 13) ? p : std::max(4, 2 * ((p + 1) / 2));
     L.nre = lay_nre(L.pl);
     L.nst = lay_nst(L.pl);
 }

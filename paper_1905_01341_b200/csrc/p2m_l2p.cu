@@ -199,8 +199,10 @@ void launch_p2m_generic(bem_ctx *c, int level, int nleaf, const int32_t *list, c
 
 static void launch_p2m_level(bem_ctx *c, int level, int nleaf, const int32_t *list, const int32_t *sbegin)
 {
-    const int p = c->p;
-    if (p <= 4) p2m_launch<4>(c, level, nleaf, list, sbegin);
+    const int p = c->pl;                                          // the layout degree: the kernels store rows of its size
+    if (p == 11) p2m_launch<11>(c, level, nleaf, list, sbegin);
+    else if (p == 13) p2m_launch<13>(c, level, nleaf, list, sbegin);
+    else if (p <= 4) p2m_launch<4>(c, level, nleaf, list, sbegin);
     else if (p <= 6) p2m_launch<6>(c, level, nleaf, list, sbegin);
     else if (p <= 8) p2m_launch<8>(c, level, nleaf, list, sbegin);
     else if (p <= 10) p2m_launch<10>(c, level, nleaf, list, sbegin);
@@ -277,8 +279,10 @@ void launch_l2p_generic(bem_ctx *c, const int32_t *leaf_of);   // translate.cu
 
 void launch_l2p(bem_ctx *c, const int32_t *leaf_of)
 {
-    const int p = c->p;
-    if (p <= 4) l2p_launch<4>(c, leaf_of);
+    const int p = c->pl;
+    if (p == 11) l2p_launch<11>(c, leaf_of);
+    else if (p == 13) l2p_launch<13>(c, leaf_of);
+    else if (p <= 4) l2p_launch<4>(c, leaf_of);
     else if (p <= 6) l2p_launch<6>(c, leaf_of);
     else if (p <= 8) l2p_launch<8>(c, leaf_of);
     else if (p <= 10) l2p_launch<10>(c, leaf_of);

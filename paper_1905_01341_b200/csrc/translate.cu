@@ -748,6 +748,8 @@ void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stre
     else if (pl == 6) launch_dmma<6>(c, st, which, stream, scratch);
     else if (pl == 8) launch_dmma<8>(c, st, which, stream, scratch);
     else if (pl == 10) launch_dmma<10>(c, st, which, stream, scratch);
+    else if (pl == 11) launch_dmma<11>(c, st, which, stream, scratch);
+    else if (pl == 13) launch_dmma<13>(c, st, which, stream, scratch);
     else if (pl == 12) launch_dmma<12>(c, st, which, stream, scratch);
     else if (pl == 14) launch_dmma<14>(c, st, which, stream, scratch);
     else launch_dmma<16>(c, st, which, stream, scratch);
