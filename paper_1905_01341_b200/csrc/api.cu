@@ -377,7 +377,10 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
                 c->ad.s_ex[l].free(); c->ad.s_sub[l].free(); c->ad.s_pbeg[l].free();
             }
             c->sb.child[lmax].free();
-        } else boxset_build(c->sb, lmax, cs, s);
+        } else {
+            c->ad = Adaptive();                                   // a context that was adaptive before: drop its tables
+            boxset_build(c->sb, lmax, cs, s);
+        }
         boxset_build(c->tb, lmax, ct, s);
         build_sources(c, c->sb.perm.get());
         c->tgt_pos.alloc(3 * N);

@@ -119,3 +119,38 @@ def test_adaptive_tree_evaluator_and_refusals():
     with pytest.raises(bem.BemError):
         ev.bem_apply(q, ph, u)
     ev.bem_destroy(); mesh.bem_destroy()
+
+
+@pytest.mark.parametrize("tree", [0, 1])
+def test_side_stream_option_gives_the_same_bits(tree):
+    """Option overlap = 1 (the row sums of the M2L stages on a side stream beside the near field, round 1's default) against
+    the one-stream default, on device buffers, for both trees; and a context switched from the adaptive tree back to the
+    uniform one gives the uniform tree's bits."""
+    import torch
+    bem = _bem()
+    c = make_config(2)
+    qd, pd = torch.tensor(c["q"], device="cuda"), torch.tensor(c["phi"], device="cuda")
+    ctx = bem.bem_create(c["V"], c["F"], c["bubble_id"])
+    ctx.bem_set_option("tree", tree)
+    ctx.bem_setup(c["p"], c["leaf_size"], c["eta"])
+    ys = []
+    for ov in (0, 1, 0):
+        ctx.bem_set_option("overlap", ov)
+        yd = torch.empty_like(qd)
+        ctx.bem_apply(qd, pd, yd)
+        torch.cuda.synchronize()
+        ys.append(yd.cpu().numpy())
+    assert np.array_equal(ys[0], ys[1]) and np.array_equal(ys[0], ys[2])
+    if tree == 1:
+        ctx.bem_set_option("tree", 0)
+        ctx.bem_setup(c["p"], c["leaf_size"], c["eta"])
+        yd = torch.empty_like(qd)
+        ctx.bem_apply(qd, pd, yd)
+        ref = bem.bem_create(c["V"], c["F"], c["bubble_id"])
+        ref.bem_setup(c["p"], c["leaf_size"], c["eta"])
+        yr = torch.empty_like(qd)
+        ref.bem_apply(qd, pd, yr)
+        torch.cuda.synchronize()
+        assert np.array_equal(yd.cpu().numpy(), yr.cpu().numpy())
+        ref.bem_destroy()
+    ctx.bem_destroy()
