@@ -142,7 +142,10 @@ struct Stage {
     // packed scratch rows (translate.cu pack_scratch), per truncation layout: the row of pair k (target-major) holds the
     // 2 W dofs its matrix class computes (W real parts, then W imaginary parts) at row_off[k] units of 16 doubles from the
     // start of the stage's region, which starts region_units units into the scratch buffer
-    dvec<int32_t> row_off[2];
+    dvec<int32_t> row_off[2];       // [npairs + 1] by target-major pair index k (the row sums)
+    dvec<int32_t> orow[2];          // [npairs] the same offsets by tile row r: orow[r] = row_off[krow[r]] (the tile kernels: one load, not two)
+    dvec<uint8_t> tile_cls[2];      // [ntiles] truncation class of every tile's matrix (loaded beside the tile, not after it)
+    std::vector<int32_t> tile_mat_host;
     int64_t region_units[2] = {0, 0};
     int ntgt = 0;
     int out_base = 0;               // global index of the first target box

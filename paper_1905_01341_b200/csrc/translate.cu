@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(GEMM_THREADS)
 translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
                const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-               int nst, const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, const int32_t *__restrict__ mat_w,
+               int nst, const int32_t *__restrict__ orow_t, const int32_t *__restrict__ mat_w,
                double *__restrict__ scratch)
 {
     __shared__ double As[GEMM_KC][GEMM_TM + 4];
@@ -211,7 +211,7 @@ translate_gemm(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
         const int r = ty * 4 + i;
         if (r >= tile.nrows) continue;
         // packed row: the W leading dofs of the real parts, then of the imaginary parts (W = nre for M2M / L2L)
-        double *out = scratch + (size_t)row_off[krow[tile.row0 + r]] * 16;
+        double *out = scratch + (size_t)orow_t[tile.row0 + r] * 16;
         const int W = mat_w[tile.mat], nre = nst >> 1;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(DM_THREADS)
 translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
                const double *__restrict__ Mexp, const double *__restrict__ Lexp,
                const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-               const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, double *__restrict__ scratch)
+               const int32_t *__restrict__ orow_t, double *__restrict__ scratch)
 {
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S] (dense tiles: [2][2 NRE][DM_S_DENSE])
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
@@ -363,7 +363,7 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
             a[2 * j + 1] = v.y;
         }
     }
-    double *orow = scratch + (size_t)(rvalid ? row_off[krow[tile.row0 + row]] : 0) * 16 + 2 * lk;     // dense rows are full rows
+    double *orow = scratch + (size_t)(rvalid ? orow_t[tile.row0 + row] : 0) * 16 + 2 * lk;     // dense rows are full rows
 
     for (int ch = 0; ch < nchunks; ++ch) {
         double *cur = (ch & 1) ? Bs1 : Bs0;
@@ -396,7 +396,7 @@ translate_dmma(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_s
 template <int KSH, int KE>
 __device__ __forceinline__ void m2l_body8(const Tile &tile, const int32_t *__restrict__ src_sorted, const double *__restrict__ Mexp,
                                           const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-                                          const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, double *__restrict__ scratch,
+                                          const int32_t *__restrict__ orow_t, double *__restrict__ scratch,
                                           double *dm_smem, double2 *cs_k)
 {
     constexpr int NRE = 4 * KSH, NST = 2 * NRE;               // layout of the stored rows and matrices
@@ -425,7 +425,7 @@ __device__ __forceinline__ void m2l_body8(const Tile &tile, const int32_t *__res
     for (int k = threadIdx.x; k < KR; k += DM_THREADS) cs_k[k] = __ldg(rot + (size_t)tile.mat * ROT_M + __ldg(kinfo + k));
     const int arow = rvalid ? src_sorted[tile.row0 + row] : -1;
     const double2 *ap = reinterpret_cast<const double2 *>(Mexp + (size_t)(arow < 0 ? 0 : arow) * NST) + lk;
-    double *orow = scratch + (size_t)(rvalid ? row_off[krow[tile.row0 + row]] : 0) * 16 + 2 * lk;   // packed row: 2 KR dofs
+    double *orow = scratch + (size_t)(rvalid ? orow_t[tile.row0 + row] : 0) * 16 + 2 * lk;   // packed row: 2 KR dofs
     double a[KE];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
@@ -455,20 +455,20 @@ static_assert(M2L_NCLS_K == 5, "the switches below list the classes");
 template <int PL>
 __global__ void __launch_bounds__(DM_THREADS, (ke_of(PL) <= 20 ? 3 : 2))
 translate_dmma_split(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
-                     const double *__restrict__ Mexp, const double *__restrict__ mats, const int32_t *__restrict__ mat_cls,
-                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow,
-                     const int32_t *__restrict__ row_off, double *__restrict__ scratch)
+                     const double *__restrict__ Mexp, const double *__restrict__ mats, const uint8_t *__restrict__ mat_cls,
+                     const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ orow_t,
+                     double *__restrict__ scratch)
 {
     constexpr int KSH = ke_of(PL);
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];                          // (cos, sin)(m_k a) of every real-part dof k
     const Tile tile = tiles[blockIdx.x];
-    switch (__ldg(mat_cls + tile.mat)) {                        // truncation class of the tile's matrix (CTA-uniform)
-    case 0: m2l_body8<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    case 1: m2l_body8<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    case 2: m2l_body8<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    case 3: m2l_body8<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    default: m2l_body8<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    switch (mat_cls[blockIdx.x]) {                              // truncation class of the tile's matrix (CTA-uniform; per-tile table)
+    case 0: m2l_body8<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    case 1: m2l_body8<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    case 2: m2l_body8<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    case 3: m2l_body8<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    default: m2l_body8<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
     }
 }
 
@@ -504,7 +504,7 @@ __device__ __forceinline__ void dm16_chunk_nt(const double (&a0)[KE], const doub
 template <int KSH, int KE>
 __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__restrict__ src_sorted, const double *__restrict__ Mexp,
                                            const double *__restrict__ mats, const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
-                                           const int32_t *__restrict__ krow, const int32_t *__restrict__ row_off, double *__restrict__ scratch,
+                                           const int32_t *__restrict__ orow_t, double *__restrict__ scratch,
                                            double *dm_smem, double2 *cs_k)
 {
     constexpr int NRE = 4 * KSH, NST = 2 * NRE;
@@ -534,8 +534,8 @@ __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__re
     const int ar0 = v0 ? src_sorted[tile.row0 + row0] : -1, ar1 = v1 ? src_sorted[tile.row0 + row1] : -1;
     const double2 *ap0 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar0 < 0 ? 0 : ar0) * NST) + lk;
     const double2 *ap1 = reinterpret_cast<const double2 *>(Mexp + (size_t)(ar1 < 0 ? 0 : ar1) * NST) + lk;
-    double *o0 = scratch + (size_t)(v0 ? row_off[krow[tile.row0 + row0]] : 0) * 16 + 2 * lk;      // packed rows: 2 KR dofs
-    double *o1 = scratch + (size_t)(v1 ? row_off[krow[tile.row0 + row1]] : 0) * 16 + 2 * lk;
+    double *o0 = scratch + (size_t)(v0 ? orow_t[tile.row0 + row0] : 0) * 16 + 2 * lk;      // packed rows: 2 KR dofs
+    double *o1 = scratch + (size_t)(v1 ? orow_t[tile.row0 + row1] : 0) * 16 + 2 * lk;
     double a0[KE], a1[KE];
 
     for (int ch = 0; ch < 2 * CPB; ++ch) {
@@ -574,20 +574,20 @@ __device__ __forceinline__ void m2l_body16(const Tile &tile, const int32_t *__re
 template <int PL>
 __global__ void __launch_bounds__(DM16_THREADS, 3)
 translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict__ src_sorted,
-                       const double *__restrict__ Mexp, const double *__restrict__ mats, const int32_t *__restrict__ mat_cls,
-                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ krow,
-                     const int32_t *__restrict__ row_off, double *__restrict__ scratch)
+                       const double *__restrict__ Mexp, const double *__restrict__ mats, const uint8_t *__restrict__ mat_cls,
+                       const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot, const int32_t *__restrict__ orow_t,
+                     double *__restrict__ scratch)
 {
     constexpr int KSH = ke_of(PL);
     extern __shared__ __align__(16) double dm_smem[];          // [2][NRE][DM_S]
     __shared__ double2 cs_k[4 * KSH];
     const Tile tile = tiles[blockIdx.x];
-    switch (__ldg(mat_cls + tile.mat)) {
-    case 0: m2l_body16<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    case 1: m2l_body16<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    case 2: m2l_body16<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    case 3: m2l_body16<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
-    default: m2l_body16<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, krow, row_off, scratch, dm_smem, cs_k); break;
+    switch (mat_cls[blockIdx.x]) {
+    case 0: m2l_body16<KSH, ke_of(PL)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    case 1: m2l_body16<KSH, ke_of(PL - 1)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    case 2: m2l_body16<KSH, ke_of(PL - 2)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    case 3: m2l_body16<KSH, ke_of(PL - 3)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
+    default: m2l_body16<KSH, ke_of(PL - 4)>(tile, src_sorted, Mexp, mats, kinfo, rot, orow_t, scratch, dm_smem, cs_k); break;
     }
 }
 
@@ -616,17 +616,17 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
     if (which != TILES_DENSE && st.ntiles_split > 0) {
         if (PL == 12 && c->m2l_rows16)                           // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
             translate_dmma_split16<(PL == 12 ? PL : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
-                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(), st.row_off[c->lay_active].get(), scratch);
+                st.tiles.get(), st.src_sorted.get(), c->Mexp.get(), c->mats.get(), st.tile_cls[c->lay_active].get(), c->kinfo.get(), c->rot.get(), st.orow[c->lay_active].get(), scratch);
         else
             translate_dmma_split<PL><<<st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get(), st.src_sorted.get(), c->Mexp.get(),
-                                                                                   c->mats.get(), c->mat_cls.get(), c->kinfo.get(), c->rot.get(), st.krow.get(),
-                                                                                   st.row_off[c->lay_active].get(), scratch);
+                                                                                   c->mats.get(), st.tile_cls[c->lay_active].get(), c->kinfo.get(), c->rot.get(),
+                                                                                   st.orow[c->lay_active].get(), scratch);
     }
     if (which != TILES_SPLIT && st.ntiles > st.ntiles_split)
         translate_dmma<KSH><<<st.ntiles - st.ntiles_split, DM_THREADS, smem, stream>>>(st.tiles.get() + st.ntiles_split, st.src_sorted.get(),
                                                                                       c->Mexp.get(), c->Lexp.get(), c->mats.get(),
-                                                                                      c->kinfo.get(), c->rot.get(), st.krow.get(),
-                                                                                      st.row_off[c->lay_active].get(), scratch);
+                                                                                      c->kinfo.get(), c->rot.get(),
+                                                                                      st.orow[c->lay_active].get(), scratch);
 }
 
 // out[out_base + t][:] = sum_{k in ptr[t]..ptr[t+1]} e^{i m a_k} scratch[k][:]   (fixed order; a_k = azimuth of
@@ -693,6 +693,11 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
 }
 
 // ------------------------------------------------------------------ packed scratch rows (setup)
+__global__ void gather_i32(const int32_t *idx, const int32_t *v, int64_t n, int32_t *out)
+{
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r < n) out[r] = v[idx[r]];
+}
 __global__ void row_units(const int32_t *mat_t, int64_t n, const int32_t *mat_w, int32_t *u)
 {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -718,6 +723,15 @@ void pack_scratch(bem_ctx *c)
             scan_exclusive_i32(u.get(), st.row_off[i].get(), n, s);
             int total = 0;
             d2h_sync(&total, st.row_off[i].get() + n, sizeof(int), s);
+            st.orow[i].alloc(n);
+            if (n > 0) { gather_i32<<<cdiv(n, 256), 256, 0, s>>>(st.krow.get(), st.row_off[i].get(), n, st.orow[i].get()); KERNEL_CHECK(); }
+            std::vector<uint8_t> tc(st.tile_mat_host.size());
+            for (size_t t = 0; t < tc.size(); ++t) tc[t] = (uint8_t)L.mat_cls_host[st.tile_mat_host[t]];
+            st.tile_cls[i].alloc(tc.size());
+            if (!tc.empty()) {
+                CUDA_TRY(cudaMemcpyAsync(st.tile_cls[i].get(), tc.data(), tc.size(), cudaMemcpyHostToDevice, s));
+                CUDA_TRY(cudaStreamSynchronize(s));
+            }
             st.region_units[i] = own_region ? region : 0;
             if (own_region) region += total;
             top = std::max(top, (own_region ? region : (int64_t)total));
@@ -741,8 +755,8 @@ void launch_stage_gemm(bem_ctx *c, const Stage &st, int which, cudaStream_t stre
     if (c->gemm_path == 1 || pl > 16) {                         // plain-FMA tiles: p > 16, or forced (option "gemm_path")
         dim3 grid(last - first, cdiv(c->nst, GEMM_TN));
         translate_gemm<<<grid, GEMM_THREADS, 0, stream>>>(st.tiles.get() + first, st.src_sorted.get(), c->Mexp.get(), c->Lexp.get(),
-                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst, st.krow.get(),
-                                                          st.row_off[c->lay_active].get(), c->mat_w.get(), scratch);
+                                                          c->mats.get(), c->kinfo.get(), c->rot.get(), c->nst,
+                                                          st.orow[c->lay_active].get(), c->mat_w.get(), scratch);
     }
     else if (pl == 4) launch_dmma<4>(c, st, which, stream, scratch);     // layout degree -> ke_of(pl) = nre / 4 k-steps per block
     else if (pl == 6) launch_dmma<6>(c, st, which, stream, scratch);

@@ -227,6 +227,8 @@ void finish_stage(bem_ctx *c, Stage &st, dvec<int32_t> &src, dvec<int32_t> &mat,
         }
         row += h[m];
     }
+    st.tile_mat_host.clear();
+    for (const Tile &t : tiles) st.tile_mat_host.push_back(t.mat);
     st.mat_t = std::move(mat);
     st.ntiles = (int)tiles.size();
     st.ntiles_split = 0;
