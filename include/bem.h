@@ -143,6 +143,8 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   measured a gain (25.6 -> 24.5 ms on config 5); with the graded M2L rows of round 2 the sums are
  *                   short, and the CTAs they hold cost the near-field kernel more than the overlap wins (config 5:
  *                   22.6 ms on one stream, 22.6-24.4 ms with the side stream).  Results are bit-identical.
+ *   "reduce_stream" 1 (default) = the per-target sums of the translated rows stream the packed rows of a target through
+ *                   shared memory (cp.async, batches of 4 rows, two in flight); 0 = direct loads.  The same bits; tuning.
  *   "reduce_ctas"   with overlap = 1: the sums are a persistent grid of this many CTAs per SM (1..32; 0 = chosen
  *                   from the pair counts so that it ends just before the near field does).  Tuning only.
  *   "m2l_rows16"    M2L tiles at p = 11, 12: 1 = 4 warps x 16 rows per CTA (default), 0 = 8 warps x 8 rows.

@@ -228,6 +228,7 @@ struct bem_ctx {
     int quadrature = 0, mode = 0, free_term = 0, gmres_restart = 0, force_lmax = 0, timing = 0;
     int precond = 0;                // bem_solve: 0 = unpreconditioned (the paper), 1 = right diagonal scaling by S_ii
     int overlap = 0;                // option "overlap": 1 = the row sums of the M2L stages run on a side stream beside the near field, 0 = one stream (default: measured faster since round 2)
+    int reduce_stream = 1;          // option "reduce_stream": 1 = the row sums stream the packed rows through shared memory (cp.async), 0 = direct loads
     int reduce_ctas = 0;            // option "reduce_ctas": CTAs per SM of the persistent side-stream sums, 0 = from the cost model
     int n_sm = 148;
     int m2l_rows16 = 1;             // M2L tiles: 1 = 4 warps x 16 rows (B fragments feed two DMMAs), 0 = 8 warps x 8 rows

@@ -692,6 +692,81 @@ translate_reduce(const int32_t *__restrict__ ptr, const int32_t *__restrict__ ma
     }
 }
 
+// The same sums with the rows STREAMED through shared memory (option "reduce_stream", default): the packed rows of a target
+// are one contiguous byte range of the scratch (row offsets are a prefix sum in target-major order), so batches of
+// RS_ROWS rows are copied whole by cp.async, two batches in flight, while the previous batch is summed from shared memory --
+// the copies carry no predicate and no address arithmetic per dof, and many are in flight per thread.  Same order of the
+// additions as translate_reduce: the same bits.
+constexpr int RS_ROWS = 4;
+constexpr int RS_STAGES = 2;        // batches in flight.  Measured on config 5 (ms of the sums + L2L class; direct loads: 2.88): two stages, 128 threads, rows 2 / 4 / 8 / 16: 2.57 / 2.22 / 2.65 / 3.78; four stages x 4 rows: 2.86; two stages, 96 threads, rows 3 / 4: 2.21 / 2.15 -- what counts is how many CTAs an SM holds
+constexpr int RS_THREADS = 128;
+__global__ void __launch_bounds__(RS_THREADS)
+translate_reduce_stream(const int32_t *__restrict__ ptr, const int32_t *__restrict__ mat_t, const int32_t *__restrict__ mat_ne,
+                        const int32_t *__restrict__ mat_w, const int32_t *__restrict__ row_off, const double *__restrict__ scratch,
+                        const int32_t *__restrict__ kinfo, const double2 *__restrict__ rot,
+                        int nre, int accumulate, int ntgt, const int32_t *__restrict__ list, double *__restrict__ out)
+{
+    extern __shared__ __align__(16) double rs_buf[];                  // [RS_STAGES][RS_ROWS * nst]
+    __shared__ int s_mt[RED_CHUNK + 8], s_off[RED_CHUNK + 8], s_w[RED_CHUNK + 8];
+    const int nst = 2 * nre;
+    const int bufsz = RS_ROWS * nst;
+    for (int ti = blockIdx.x; ti < ntgt; ti += gridDim.x) {
+        const int t = list ? list[ti] : ti;
+        const int b = ptr[t], e = ptr[t + 1];
+        double *o = out + (size_t)t * nst;
+        if (b == e && accumulate == 0)
+            for (int cc = threadIdx.x; cc < nst; cc += blockDim.x) o[cc] = 0.0;
+        for (int k0 = b; k0 < e; k0 += RED_CHUNK) {
+            const int n = min(RED_CHUNK, e - k0);
+            __syncthreads();
+            for (int i = threadIdx.x; i <= n; i += blockDim.x) {
+                s_off[i] = row_off[k0 + i];                              // row_off has npairs + 1 entries
+                if (i < n) { const int mt = mat_t[k0 + i]; s_mt[i] = mt | (__ldg(mat_ne + mt) << 16); s_w[i] = __ldg(mat_w + mt); }
+            }
+            __syncthreads();
+            const int nb = (n + RS_ROWS - 1) / RS_ROWS;
+            auto issue = [&](int bi) {                                   // rows [bi RS_ROWS, ..) of the chunk: one contiguous range
+                const int i0 = bi * RS_ROWS, i1 = min(n, i0 + RS_ROWS);
+                const double *src = scratch + (size_t)s_off[i0] * 16;
+                const int pieces = (s_off[i1] - s_off[i0]) * 8;          // 16-byte pieces
+                double *dst = rs_buf + (bi % RS_STAGES) * bufsz;
+                for (int q = threadIdx.x; q < pieces; q += blockDim.x) cp_async16(dst + 2 * q, src + 2 * q);
+            };
+            double sr = 0.0, si = 0.0;                                   // blockDim >= nre: one dof per thread
+            const int cc = threadIdx.x;
+            const int m = cc < nre ? kinfo[cc] : 0;
+            for (int j = 0; j < RS_STAGES - 1; ++j) { if (j < nb) issue(j); cp_async_commit(); }
+            for (int bi = 0; bi < nb; ++bi) {
+                if (bi + RS_STAGES - 1 < nb) issue(bi + RS_STAGES - 1);  // into the buffer batch bi - 1 left (barrier below)
+                cp_async_commit();                                       // one group per iteration, empty at the tail
+                cp_async_wait<RS_STAGES - 1>();
+                __syncthreads();                                         // batch bi is in shared memory
+                if (cc < nre) {
+                    const int i0 = bi * RS_ROWS, i1 = min(n, i0 + RS_ROWS);
+                    const double *buf = rs_buf + (bi % RS_STAGES) * bufsz;
+                    const int base = s_off[i0];
+                    for (int i = i0; i < i1; ++i) {
+                        const int mt = s_mt[i];
+                        if (cc < (mt >> 16)) {
+                            const double *row = buf + (s_off[i] - base) * 16;
+                            double vr = row[cc], vi = row[s_w[i] + cc];
+                            if (m != 0) { azimuth(__ldg(rot + (size_t)(mt & 0xffff) * ROT_M + m), vr, vi); si += vi; }
+                            sr += vr;
+                        }
+                    }
+                }
+                __syncthreads();                                         // everyone left batch bi before it is overwritten
+            }
+            if (cc < nre) {
+                if (accumulate == 1 || k0 > b) { sr += o[cc]; si += o[cc + nre]; }
+                o[cc] = sr;
+                o[cc + nre] = si;
+            }
+        }
+    }
+}
+
+
 // ------------------------------------------------------------------ packed scratch rows (setup)
 __global__ void gather_i32(const int32_t *idx, const int32_t *v, int64_t n, int32_t *out)
 {
@@ -784,6 +859,18 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
     static std::vector<char> attr_done;
     if (first_use_on_device(attr_done, c->device))                     // same carve-out as the pair kernels it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+    if (c->reduce_stream && c->nre <= RS_THREADS) {                    // rows streamed through shared memory (cp.async)
+        const size_t smem = (size_t)RS_STAGES * RS_ROWS * c->nst * sizeof(double);
+        static std::vector<char> attr2_done;
+        if (first_use_on_device(attr2_done, c->device))
+            CUDA_TRY(cudaFuncSetAttribute(translate_reduce_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_STAGES * RS_ROWS * 2 * RS_THREADS * (int)sizeof(double)));
+        translate_reduce_stream<<<grid, std::max(64, ((c->nre + 31) / 32) * 32), smem, stream>>>(
+            st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->mat_w.get(), st.row_off[c->lay_active].get(),
+            c->scratch.get() + (size_t)st.region_units[c->lay_active] * 16,
+            c->kinfo.get(), c->rot.get(), c->nre, st.accumulate ? 1 : (st.keep_empty ? 2 : 0), nvisit, st.n_list >= 0 ? st.tgt_list.get() : nullptr, out);
+        KERNEL_CHECK();
+        return;
+    }
     translate_reduce<<<grid, std::min(160, ((c->nre + 31) / 32) * 32), 0, stream>>>(
         st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->mat_w.get(), st.row_off[c->lay_active].get(),
         c->scratch.get() + (size_t)st.region_units[c->lay_active] * 16,
