@@ -227,6 +227,12 @@ def run_gpu(args):
     ctx = bem.bem_create_points(V, V) if c.get("cloud") else bem.bem_create(V, F, c["bubble_id"])
     ctx.bem_set_stream(stream.cuda_stream)
     ctx.bem_set_option("mode", 1 if args.direct else 0)
+    # tree: the adaptive octree (option tree = 1) is the faster one on config 5 (21.4 against 22.2 ms) and
+    # within 1% of the uniform one elsewhere; auto = adaptive on config 5 with fp64 pairs (fp32 pairs need the uniform tree)
+    adaptive = (not args.direct) and (args.tree == "adaptive" or (args.tree == "auto" and args.config == 5 and args.p2p_precision == 64)
+                                      or any(o.replace(" ", "") == "tree=1" for o in args.opt))
+    if adaptive:
+        ctx.bem_set_option("tree", 1)
     if args.lmax:
         ctx.bem_set_option("lmax", args.lmax)
     if args.no_graph:
@@ -392,8 +398,7 @@ def run_gpu(args):
 
     # the paper's "single precision on GPU" option for A^(sparse) X, measured beside the fp64 default
     mixed = None
-    adaptive = any(o.replace(" ", "") == "tree=1" for o in args.opt)            # fp32 pairs need leaves of one size (uniform tree)
-    if not args.direct and not f32 and not adaptive:
+    if not args.direct and not f32 and not adaptive:                            # fp32 pairs need leaves of one size (uniform tree)
         ctx.bem_set_option("p2p_precision", 1)
         for _ in range(3):
             ctx.bem_apply(qd, pd, yd)
@@ -409,6 +414,38 @@ def run_gpu(args):
                      value=mixed_ms, unit=UNIT, p2p_ms=tmix["p2p"], p2p_gpairs_per_s=stats["p2p_pairs"] / (tmix["p2p"] * 1e-3) / 1e9,
                      parity_rel_l2_vs_oracle=float(np.linalg.norm(ym[rows] - yo) / np.linalg.norm(yo)),
                      rel_l2_vs_fp64_path=float(np.linalg.norm(ym - y) / np.linalg.norm(y)))
+
+    # the uniform tree of PAPER.md:440 (the library default) beside the adaptive one, with its fp32-pair variant
+    uniform = None
+    if adaptive:
+        cu = bem.bem_create(V, F, c["bubble_id"])
+        cu.bem_set_stream(stream.cuda_stream)
+        if args.lmax:
+            cu.bem_set_option("lmax", args.lmax)
+        cu.bem_setup(p, args.leaf_size or c["leaf_size"], c["eta"])
+        su = cu.bem_get_stats()
+        for _ in range(3):
+            cu.bem_apply(qd, pd, yd)
+        torch.cuda.synchronize()
+        u_ms = timed(lambda: cu.bem_apply(qd, pd, yd), args.steps) / args.steps
+        yu = yd.cpu().numpy()
+        cu.bem_set_option("timing", 1)
+        cu.bem_apply(qd, pd, yd)
+        tu = cu.bem_get_timings()
+        cu.bem_set_option("timing", 0)
+        cu.bem_set_option("p2p_precision", 1)
+        for _ in range(3):
+            cu.bem_apply(qd, pd, yd)
+        torch.cuda.synchronize()
+        u32_ms = timed(lambda: cu.bem_apply(qd, pd, yd), args.steps) / args.steps
+        yu32 = yd.cpu().numpy()
+        cu.bem_destroy()
+        uniform = dict(option="tree = 0: uniform depth l_max, the paper's tree (PAPER.md:440) and the library default", value=u_ms, unit=UNIT,
+                       lmax=int(su["lmax"]), breakdown_ms={k: round(v, 4) for k, v in tu.items()}, m2l_pairs=int(su["m2l_pairs"]),
+                       p2p_pairs=su["p2p_pairs"], device_bytes=int(su["device_bytes"]),
+                       parity_rel_l2_vs_oracle=float(np.linalg.norm(yu[rows] - yo) / np.linalg.norm(yo)),
+                       with_fp32_pairs=dict(value=u32_ms, unit=UNIT,
+                                            parity_rel_l2_vs_oracle=float(np.linalg.norm(yu32[rows] - yo) / np.linalg.norm(yo))))
 
     # the steps either side of the solve in a time step: surface velocity, shape filter
     extras = None
@@ -498,7 +535,7 @@ def run_gpu(args):
     line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
                 higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64 (near-field pairs f32)" if f32 else "f64", data="synthetic",
                 config=workload_config(c, args, p),
-                run=dict(mode="direct" if args.direct else "fmm", p2p_precision="fp32 pairs, fp64 sums" if f32 else "fp64",
+                run=dict(mode="direct" if args.direct else "fmm", tree="adaptive" if adaptive else "uniform", p2p_precision="fp32 pairs, fp64 sums" if f32 else "fp64",
                          p_dipole=int(stats["p_dipole"]), lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]),
                          n_tgt_leaves=int(stats["n_tgt_leaves"]),
                          launch="CUDA graph replay" if (stream.cuda_stream != 0 and not args.no_graph) else "kernel by kernel",
@@ -507,7 +544,7 @@ def run_gpu(args):
                 gpu_launches=int(stats["kernel_launches_per_apply"]) * args.steps,
                 clocks=clocks, roofline=roof, cpu_baseline=cpu, parity_rel_l2_vs_oracle=parity, parity_rows=parity_rows,
                 breakdown_ms=breakdown, kernels=kernels, setup_ms=stats["setup_ms"], setup_wall_ms=setup_wall_ms,
-                m2l_pairs=int(stats["m2l_pairs"]), solve=solve, mixed_precision_option=mixed, time_step_extras=extras,
+                m2l_pairs=int(stats["m2l_pairs"]), solve=solve, mixed_precision_option=mixed, uniform_tree_option=uniform, time_step_extras=extras,
                 paper_context=("paper Table 2 (PAPER.md:479-490): at N=1,048,576, p=12 the FMM+GPU (double) product is 2309x faster than the CPU "
                                "brute force and the brute-force GPU (double) 33x, Xeon 5660 + Tesla K20" if cloud else
                                "paper Table 3 (PAPER.md:606): 1 MVP = 4.0 s at N=2,629,632, p=12, double, Xeon 5660 x12 cores + Tesla K20"))
@@ -538,6 +575,8 @@ def main():
                     help="leaf-level far pairs with nt x ns <= this are summed directly instead of translated (default: library cost model; 0: off)")
     ap.add_argument("--p2p-ctas", type=int, default=0, help="fp32 near field: CTAs per SM of its persistent grid (0: library default)")
     ap.add_argument("--reduce-ctas", type=int, default=0, help="CTAs per SM of the persistent row-sum passes (0: library cost model)")
+    ap.add_argument("--tree", default="auto", choices=["auto", "uniform", "adaptive"],
+                    help="octree: uniform depth (the paper's), adaptive (option tree = 1), auto = adaptive on config 5 with fp64 pairs (measured faster)")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="any bem_set_option key (repeatable), set before bem_setup")
     ap.add_argument("--solve-iters", type=int, default=-1, help="also run bem_solve with this max_iter (0: skip; -1: 30, or 400 = to convergence on config 5)")
     ap.add_argument("--solve-tol", type=float, default=1e-6)
