@@ -19,7 +19,7 @@ CONFIG_PARAMS = {
     2: dict(p=10, leaf_size=64, eta=2.5),
     3: dict(p=10, leaf_size=64, eta=2.5),
     4: dict(p=10, leaf_size=96, eta=2.5),
-    5: dict(p=12, leaf_size=350, eta=2.5),     # uniform tree: l_max 6 for any leaf_size in 171..678; adaptive tree: measured optimum
+    5: dict(p=12, leaf_size=256, eta=2.5),
 }
 
 

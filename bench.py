@@ -59,6 +59,23 @@ def workload_name(c):
     return c["name"]
 
 
+def use_adaptive_tree(args):
+    """The adaptive octree (option tree = 1) is the faster one on config 5 (21.4 against 22.2 ms) and within
+    1% of the uniform one elsewhere: auto = adaptive on config 5 with fp64 pairs (fp32 pairs need the uniform tree)."""
+    if args.direct:
+        return False
+    return (args.tree == "adaptive" or (args.tree == "auto" and args.config == 5 and args.p2p_precision == 64)
+            or any(o.replace(" ", "") == "tree=1" for o in args.opt))
+
+
+def bench_leaf_size(args, c):
+    """leaf_size of the run: the config's, or 350 for the adaptive tree on config 5 (measured optimum; the uniform tree of
+    config 5 has l_max = 6 for any leaf_size between 171 and 678)."""
+    if args.leaf_size:
+        return int(args.leaf_size)
+    return 350 if (args.config == 5 and use_adaptive_tree(args)) else int(c["leaf_size"])
+
+
 def workload_config(c, args, p):
     """The keys that name the workload -- the SAME dict in the b200 arm and in the reference arm (the CPU oracle computes
     the same discretised operator on the same inputs); what only the GPU run knows (tree depth, launch mode, device bytes)
@@ -66,7 +83,7 @@ def workload_config(c, args, p):
     N, T = int(c["V"].shape[0]), int(c["F"].shape[0])
     cloud = bool(c.get("cloud"))
     return dict(workload=workload_name(c), operator="y = S[q] - D[phi] (G3 quadrature + near correction)" if not cloud else "monopole sum",
-                p=int(p), n_nodes=N, n_triangles=T, n_sources=(N if cloud else 3 * T), leaf_size=int(args.leaf_size or c["leaf_size"]),
+                p=int(p), n_nodes=N, n_triangles=T, n_sources=(N if cloud else 3 * T), leaf_size=bench_leaf_size(args, c),
                 eta=c["eta"], parallelism="replicas only" if args.gpus > 1 else "1 gpu",
                 l2="working set larger than L2" if N >= 100000 else "flushed between iterations (512 MB write)")
 
@@ -227,10 +244,7 @@ def run_gpu(args):
     ctx = bem.bem_create_points(V, V) if c.get("cloud") else bem.bem_create(V, F, c["bubble_id"])
     ctx.bem_set_stream(stream.cuda_stream)
     ctx.bem_set_option("mode", 1 if args.direct else 0)
-    # tree: the adaptive octree (option tree = 1) is the faster one on config 5 (21.4 against 22.2 ms) and
-    # within 1% of the uniform one elsewhere; auto = adaptive on config 5 with fp64 pairs (fp32 pairs need the uniform tree)
-    adaptive = (not args.direct) and (args.tree == "adaptive" or (args.tree == "auto" and args.config == 5 and args.p2p_precision == 64)
-                                      or any(o.replace(" ", "") == "tree=1" for o in args.opt))
+    adaptive = use_adaptive_tree(args)
     if adaptive:
         ctx.bem_set_option("tree", 1)
     if args.lmax:
@@ -248,7 +262,7 @@ def run_gpu(args):
     for kv in args.opt:
         k, v = kv.split("=")
         ctx.bem_set_option(k, float(v))
-    ctx.bem_setup(p, args.leaf_size or c["leaf_size"], c["eta"])
+    ctx.bem_setup(p, bench_leaf_size(args, c), c["eta"])
     torch.cuda.synchronize()
     setup_wall_ms = (time.perf_counter() - t0) * 1e3
     stats = ctx.bem_get_stats()
@@ -422,7 +436,7 @@ def run_gpu(args):
         cu.bem_set_stream(stream.cuda_stream)
         if args.lmax:
             cu.bem_set_option("lmax", args.lmax)
-        cu.bem_setup(p, args.leaf_size or c["leaf_size"], c["eta"])
+        cu.bem_setup(p, args.leaf_size or c["leaf_size"], c["eta"])          # the config's own leaf_size
         su = cu.bem_get_stats()
         for _ in range(3):
             cu.bem_apply(qd, pd, yd)
