@@ -154,3 +154,78 @@ def test_side_stream_option_gives_the_same_bits(tree):
         assert np.array_equal(yd.cpu().numpy(), yr.cpu().numpy())
         ref.bem_destroy()
     ctx.bem_destroy()
+
+
+def test_adaptive_tree_full_size_config5_as_bench_times_it():
+    """BASELINE.json config 5 at full size in the configuration bench.py times by default (tree = 1, leaf_size 350,
+    device-resident q, phi, y) on the 2000 seeded rows of the north_star; bit-identical repeat; GMRES takes one more
+    step through it (products without phi) and reduces the residual."""
+    import torch
+    bem = _bem()
+    c = make_config(5)
+    N = c["V"].shape[0]
+    rows = sample_rows(5, N, 2000)
+    yo = oracle.g3_apply(c["V"], c["F"], c["q"], c["phi"], eta=c["eta"], rows=rows)
+    ctx = bem.bem_create(c["V"], c["F"], c["bubble_id"])
+    ctx.bem_set_option("tree", 1)
+    ctx.bem_setup(c["p"], 350, c["eta"])
+    qd, pd = torch.tensor(c["q"], device="cuda"), torch.tensor(c["phi"], device="cuda")
+    yd = torch.empty_like(qd)
+    ctx.bem_apply(qd, pd, yd)
+    y1 = yd.cpu().numpy()
+    ctx.bem_apply(qd, pd, yd)
+    assert np.array_equal(y1, yd.cpu().numpy())
+    st = ctx.bem_get_stats()
+    e = _rel(y1[rows], yo)
+    print(f"cfg5 full size, adaptive: S-D on 2000 rows {e:.2e}; lmax {st['lmax']:.0f}, target leaves {st['n_tgt_leaves']:.0f}, "
+          f"m2l pairs {st['m2l_pairs']:.0f}, point pairs {st['p2p_pairs']:.3e}")
+    assert st["lmax"] > 6 and e <= 1e-5
+    qs = torch.zeros_like(qd)
+    status, it, rr = ctx.bem_solve(pd, qs, tol=1e-6, max_iter=3)
+    assert it == 3 and rr < 1.0 and status == bem.BEM_ERR_NOT_CONVERGED      # unpreconditioned GMRES starts slowly here (0.93 after 3 steps)
+    ctx.bem_destroy()
+
+
+def test_degenerate_inputs_both_trees():
+    """The smallest closed mesh (a tetrahedron: 4 vertices), one target, one source, all sources in one point's
+    neighbourhood and coincident source/target clouds -- both trees, FMM and direct, against the oracle."""
+    bem = _bem()
+    V = np.array([[1.0, 1.0, 1.0], [1.0, -1.0, -1.0], [-1.0, 1.0, -1.0], [-1.0, -1.0, 1.0]])
+    F = np.array([[0, 1, 2], [0, 3, 1], [0, 2, 3], [1, 3, 2]], dtype=np.int32)
+    if np.dot(np.cross(V[1] - V[0], V[2] - V[0]), V[0] + V[1] + V[2]) < 0:
+        F = F[:, [0, 2, 1]].copy()                           # outward orientation
+    q, ph = np.array([1.0, -2.0, 0.5, 3.0]), np.array([0.3, 0.1, -0.7, 1.1])
+    yo = oracle.g3_apply(V, F, q, ph, eta=2.5)
+    for tree in (0, 1):
+        for mode in (0, 1):
+            ctx = bem.bem_create(V, F, None)
+            ctx.bem_set_option("tree", tree); ctx.bem_set_option("mode", mode)
+            ctx.bem_setup(6, 1, 2.5)
+            y = np.full(4, np.nan)
+            ctx.bem_apply(q, ph, y)
+            ctx.bem_destroy()
+            assert _rel(y, yo) <= (1e-12 if mode else 1e-4), (tree, mode, _rel(y, yo))
+    rng = np.random.default_rng(9)
+    src = rng.uniform(0, 1, size=(500, 3))
+    m = rng.normal(size=500)
+    for tgt in (np.array([[0.5, 0.5, 0.5]]), np.array([[5.0, -3.0, 2.0]]), src[:1].copy()):
+        yo = oracle.monopole_sum(src, m, tgt)
+        for tree in (0, 1):
+            ctx = bem.bem_create_points(src, tgt)
+            ctx.bem_set_option("tree", tree)
+            ctx.bem_setup(12, 16, 2.5)
+            y = np.full(1, np.nan)
+            ctx.bem_apply(m, None, y)
+            ctx.bem_destroy()
+            assert abs(y[0] - yo[0]) <= 1e-5 * abs(yo[0]), (tree, tgt, y, yo)
+    one = np.array([[0.25, 0.5, 0.75]])
+    tg = rng.uniform(0, 1, size=(300, 3))
+    yo = oracle.point_sum(one, np.array([2.0]), np.array([[0.1, -0.2, 0.3]]), tg)
+    for tree in (0, 1):
+        ctx = bem.bem_create_points(one, tg)
+        ctx.bem_set_option("tree", tree)
+        ctx.bem_setup(16, 8, 2.5)
+        y = np.full(300, np.nan)
+        ctx.bem_apply(np.array([2.0]), np.array([[0.1, -0.2, 0.3]]), y)
+        ctx.bem_destroy()
+        assert _rel(y, yo) <= 1e-6, (tree, _rel(y, yo))
