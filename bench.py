@@ -338,6 +338,9 @@ def run_gpu(args):
     # FP64 pipe: 148 SMs x 64 lanes x 1.965 GHz = 18.6 T instr/s; an FMA counts 2 flop, so the flop peak is 37.2 TFLOP/s.
     # P2P: 17 FP64 instructions per pair (9 DFMA + 5 DMUL + 3 DADD = 26 flop; SASS count).
     P2P_INSTR, P2P_FLOP = 17.0, 26.0
+    if not args.direct and not any(o.replace(" ", "") == "p2p_exact=1" for o in args.opt):
+        # FMM mode: ONE Newton step after the hardware seed (option p2p_exact = 0): 8 DFMA + 5 DMUL + 3 DADD per pair
+        P2P_INSTR, P2P_FLOP = 16.0, 24.0
     slot_peak = FP64_NOMINAL_GFLOPS / 2e3                      # T instr/s
     f32 = args.p2p_precision == 32 and not args.direct
     if f32:
@@ -354,7 +357,7 @@ def run_gpu(args):
                           tflops=stats["p2p_pairs"] * P2P_FLOP / p2p_s / 1e12 if p2p_s > 0 else None,
                           fp64_slot_frac=stats["p2p_pairs"] * P2P_INSTR / p2p_s / 1e12 / slot_peak if p2p_s > 0 else None,
                           note=("12 FP32 instr (18 flop) + 1 MUFU.RSQ per pair; fp64_slot_frac here = share of the FP32 pipes' issue slots (nominal 37.2 T instr/s)"
-                                if f32 else "17 FP64 instr / 26 flop per pair; slot_frac = share of the FP64 pipe's issue slots (nominal 18.6 T instr/s)"))
+                                if f32 else "%d FP64 instr / %d flop per pair; slot_frac = share of the FP64 pipe's issue slots (nominal 18.6 T instr/s)" % (P2P_INSTR, P2P_FLOP)))
     if not args.direct:
         m2l_s = tm["m2l"] * 1e-3
         exec_flop = stats["m2l_flop"]                             # two blocks of (4 KE)^2 MACs per pair, KE = k-steps of the pair's truncation class
@@ -387,7 +390,7 @@ def run_gpu(args):
         roof = dict(kernel="p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", bound="alu", achieved=k["tflops"],
                     peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", frac=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
                     fp64_slot_frac=k["fp64_slot_frac"], traffic=ncu_traffic("p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", args.config),
-                    algorithmic="26 flop (17 FP64 instructions) per pair x %d pairs" % stats["p2p_pairs"], ms=tm["p2p"],
+                    algorithmic="%d flop (%d FP64 instructions) per pair x %d pairs" % (P2P_FLOP, P2P_INSTR, stats["p2p_pairs"]), ms=tm["p2p"],
                     share_of_step=tm["p2p"] / tm["total"], **common)
     else:
         k = kernels["m2l"]

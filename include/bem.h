@@ -187,6 +187,11 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   in fp64 in a fixed order.  The far field, the correction matrix and the direct-sum mode stay
  *                   fp64.  Error floor ~1e-7 (monopoles) .. 1e-6 (dipoles on surfaces) relative L2: at the
  *                   configs' p (<= 12) the product's error is unchanged.  May be changed between products.
+ *   "p2p_exact"     near field of the FMM mode, fp64 pairs: 0 (default) = 1/r by the hardware seed and ONE Newton step (relative
+ *                   error of a pair <= 4e-13, one-sided: four decades below the truncation error of the far field; 16
+ *                   FP64 instructions per pair), 1 = the third-order step of the direct-sum mode (1 ulp; 17 instructions).
+ *                   The direct-sum mode always uses the third-order step (its tolerance is 1e-12).  May be changed
+ *                   between products.
  *   "direct_pairs"  leaf-level far-field (M2L) pairs whose boxes hold nt targets and ns sources with nt x ns <= this
  *                   value are summed directly in the near-field kernel instead of being translated: a translation
  *                   costs 4 nre^2 flop whatever the boxes hold, and on surface meshes a third of the leaf-level pairs

@@ -658,6 +658,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
     else if (!strcmp(key, "dipole_degrees")) { if (v < -1 || v > 16) return BEM_ERR_INVALID_ARG; c->dipole_degrees = v; c->ready = false; }
     else if (!strcmp(key, "tree_min_level")) { if (v != 0 && (v < 2 || v > MAX_LEVEL)) return BEM_ERR_INVALID_ARG; c->tree_min_level = v; c->ready = false; }
     else if (!strcmp(key, "tree")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->adaptive = v; c->ready = false; }
+    else if (!strcmp(key, "p2p_exact")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->p2p_exact = v; }
     else if (!strcmp(key, "reduce_stream")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->reduce_stream = v; }
     else if (!strcmp(key, "overlap")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->overlap = v; }
     else if (!strcmp(key, "gemm_path")) { if (v != 0 && v != 1) return BEM_ERR_INVALID_ARG; c->gemm_path = v; }

@@ -233,6 +233,7 @@ struct bem_ctx {
     int n_sm = 148;
     int m2l_rows16 = 1;             // M2L tiles: 1 = 4 warps x 16 rows (B fragments feed two DMMAs), 0 = 8 warps x 8 rows
     int gemm_path = 0;              // translations: 0 = FP64 tensor path (DMMA) where p <= 16, 1 = plain-FMA tiles
+    int p2p_exact = 0;              // option "p2p_exact": 1 = the FMM near field refines 1/r to the last bit as direct mode does (17 FP64 instr per pair)
     int p2p_precision = 0;          // near field: 0 = fp64 pairs (default), 1 = fp32 pair arithmetic, fp64 accumulation (p2p_f32.cu)
     int p2p_ctas = 0;               // fp32 near field: CTAs per SM of its persistent grid beside the row sums, 0 = default (4)
 

@@ -68,13 +68,18 @@ void launch_lift(bem_ctx *c, const double *q, const double *phi)
 // 5 e^3/16 ~ 2.5 d^3 < 1e-19 -- 5 FP64 instructions instead of the two Newton steps and the
 // slow-path branch of the library rsqrt (P2P).
 // SELF = false: the caller guarantees x > 0 (G3: a Gauss point never coincides with a vertex) and the test is left out
-template <bool SELF>
+// ORD = 3: that step (direct-sum mode: 1e-12 against the oracle).  ORD = 2: the Newton step y1 = y0 (1 + e/2), which drops
+// 3 e^2/8: MUFU.RSQ64H reads the high word of x only, so e is up to ~2e-6 and the dropped term a one-sided <= 4e-13 -- too
+// much for the 1e-12 of direct mode, far below the truncation error of the FMM (1e-6 .. 1e-9), whose near field therefore
+// runs 16 instead of 17 FP64 instructions per pair (option "p2p_exact" = 1 keeps ORD = 3 there too).
+template <bool SELF, int ORD = 3>
 __device__ __forceinline__ double rsqrt_pos(double x)
 {
     double y0;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
     if (SELF) y0 = __double2hiint(x) > 0 ? y0 : 0.0;   // x >= 0 here; x == 0 (and subnormal x) -> 0, an integer test off the FP64 pipe
     const double e = fma(-x, y0 * y0, 1.0);
+    if (ORD == 2) return fma(y0 * e, 0.5, y0);
     const double pe = fma(0.375, e, 0.5) * e;
     return fma(y0, pe, y0);
 }
@@ -82,12 +87,12 @@ __device__ __forceinline__ double rsqrt_pos(double x)
 // one (target, source) interaction; r2 == 0 (V1: source j = target i; "i != j") adds nothing
 // acc += that interaction (the last multiply and the accumulation are one FMA)
 // DIP = false: monopole sources only (phi == NULL, every product of a GMRES iteration): 12 FP64 instructions instead of 17
-template <bool DIP, bool SELF>
+template <bool DIP, bool SELF, int ORD = 3>
 __device__ __forceinline__ double pair_acc(double acc, double tx, double ty, double tz, const double4 &sp, const double4 &ss)
 {
     const double dx = tx - sp.x, dy = ty - sp.y, dz = tz - sp.z;
     const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    const double inv = rsqrt_pos<SELF>(r2);
+    const double inv = rsqrt_pos<SELF, ORD>(r2);
     if (!DIP) return fma(inv, ss.x, acc);
     const double dd = fma(ss.y, dx, fma(ss.z, dy, ss.w * dz));
     // m/r - (d.dx)/r^3 = inv * (m - dd * inv^2)
@@ -170,7 +175,7 @@ __device__ __forceinline__ void lds_point(unsigned addr, double &x, double &y, d
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%3];\n\tld.shared.f64 %2, [%3+16];" : "=d"(x), "=d"(y), "=d"(z) : "r"(addr));
 }
 
-template <bool DIP, bool SELF>
+template <bool DIP, bool SELF, int ORD>
 __global__ void __launch_bounds__(P2P_THREADS, 5)
 p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbegin, const int32_t *__restrict__ nbr,
                 const int32_t *__restrict__ xptr, const int32_t *__restrict__ xsrc,
@@ -232,7 +237,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                     for (int t = tb; t < tb + 8; ++t) {
                         double Tx, Ty, Tz;
                         lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                        acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
+                        acc[t] = pair_acc<DIP, SELF, ORD>(acc[t], Tx, Ty, Tz, p, q);
                     }
                 } else if (tb < ntc) {                                  // the last 1..7 targets: 4 + singles
                     if (tb + 4 <= ntc) {
@@ -240,14 +245,14 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                         for (int t = tb; t < tb + 4; ++t) {
                             double Tx, Ty, Tz;
                             lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                            acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
+                            acc[t] = pair_acc<DIP, SELF, ORD>(acc[t], Tx, Ty, Tz, p, q);
                         }
 #pragma unroll
                         for (int t = tb + 4; t < tb + 7; ++t) {
                             if (t < ntc) {
                                 double Tx, Ty, Tz;
                                 lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                                acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
+                                acc[t] = pair_acc<DIP, SELF, ORD>(acc[t], Tx, Ty, Tz, p, q);
                             }
                         }
                     } else {
@@ -256,7 +261,7 @@ p2p_leaf_kernel(const double *__restrict__ tgt, const int32_t *__restrict__ tbeg
                             if (t < ntc) {
                                 double Tx, Ty, Tz;
                                 lds_point(tg_base + 32u * t, Tx, Ty, Tz);
-                                acc[t] = pair_acc<DIP, SELF>(acc[t], Tx, Ty, Tz, p, q);
+                                acc[t] = pair_acc<DIP, SELF, ORD>(acc[t], Tx, Ty, Tz, p, q);
                             }
                         }
                     }
@@ -295,10 +300,10 @@ void launch_p2p_leaves(bem_ctx *c)
     const int nleaf = c->adaptive ? c->ad.n_tleaf : c->tb.nbox[c->tb.lmax];
     static std::vector<char> attr_done;
     if (first_use_on_device(attr_done, c->device)) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
-        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+#define BEM_CARVE(D, S) CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<D, S, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT)); \
+                        CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<D, S, 3>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT))
+        BEM_CARVE(true, true); BEM_CARVE(true, false); BEM_CARVE(false, true); BEM_CARVE(false, false);
+#undef BEM_CARVE
     }
     const bool self = c->quadrature != 0;                       // V1 (j = i) and point clouds may have r = 0; G3 cannot
     // adaptive tree: target leaves in point order (ad.tleaf_begin), source ranges from the CSR (ad.near_ptr, ad.near_rng), nbr = null
@@ -306,11 +311,13 @@ void launch_p2p_leaves(bem_ctx *c)
     const int32_t *nbr = c->adaptive ? nullptr : c->nbr.get();
     const int32_t *xp = c->adaptive ? c->ad.near_ptr.get() : c->xdir_ptr.p;
     const int32_t *xs = c->adaptive ? reinterpret_cast<const int32_t *>(c->ad.near_rng.get()) : c->xdir_src.p;
-#define BEM_LEAF(D, S) p2p_leaf_kernel<D, S><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), tbeg, nbr, xp, \
+#define BEM_LEAF_O(D, S, O) p2p_leaf_kernel<D, S, O><<<nleaf, P2P_THREADS, 0, c->stream>>>(c->tgt_pos.get(), tbeg, nbr, xp, \
                            xs, c->sb.begin.get(), c->src_pos.get(), c->src_str.get(), c->ypart.get() + c->N)
+#define BEM_LEAF(D, S) do { if (c->p2p_exact) BEM_LEAF_O(D, S, 3); else BEM_LEAF_O(D, S, 2); } while (0)
     if (c->has_dipole) { if (self) BEM_LEAF(true, true); else BEM_LEAF(true, false); }
     else { if (self) BEM_LEAF(false, true); else BEM_LEAF(false, false); }
 #undef BEM_LEAF
+#undef BEM_LEAF_O
     KERNEL_CHECK();
 }
 
