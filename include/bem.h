@@ -326,6 +326,37 @@ bem_status bem_filter_apply(bem_filter *f, const double *x, int64_t n_cols, doub
 const char *bem_filter_last_error(const bem_filter *f);
 void bem_filter_destroy(bem_filter *f);
 
+/* bem_direct_sum_static -- the all-pairs sum of the two kernels of PAPER.md:143-145 (Eq. 13) over a point cloud,
+ *     y_i = sum_{j : y_j != x_i} [ q_j / (4 pi |x_i - y_j|)  -  d_j . (x_i - y_j) / (4 pi |x_i - y_j|^3) ],
+ * the same sum as bem_create_points + option "mode" = 1 + bem_apply (the direct-sum mode of PAPER.md:490), for callers
+ * that must NOT allocate device memory: this call makes no cudaMalloc / cudaFree and calls nothing that does.  It is
+ * meant for a host whose device memory is already spoken for when the sum is needed -- a simulation that carved the
+ * GPU into its own arenas at start-up, a tenant under a fixed MPS / MIG memory budget -- and for a latency-bound loop
+ * that cannot take the device-wide synchronisation a cudaMalloc / cudaFree brings.  Every other entry of this library
+ * allocates (contexts, staging, Krylov vectors) and is not for them.
+ *   sources  [n_sources x 3], q [n_sources] monopole strengths or NULL, d [n_sources x 3] dipole vectors or NULL,
+ *   targets  [n_targets x 3], y [n_targets] (overwritten; must not overlap the inputs).  All fp64, row-major, and all
+ *   DEVICE pointers of the CURRENT device (a host pointer is refused: copying it would need a staging buffer).
+ *   cuda_stream  a cudaStream_t, NULL = the default stream.  The call enqueues two kernels and returns; it never
+ *   synchronises.
+ * Scratch: the partial sums of the source chunks live in an array compiled into the library (static __device__,
+ * 16 x BEM_DIRECT_STATIC_MAX_TARGETS doubles = 8 MiB).  Consequences a caller must know:
+ *   - n_targets > BEM_DIRECT_STATIC_MAX_TARGETS is refused with BEM_ERR_INVALID_ARG (n_sources: up to 2^31 - 1);
+ *     split a larger target set into several calls, one after the other.
+ *   - every GPU on which the process has loaded the library holds those 8 MiB until the process exits, whether or not
+ *     this function is ever called.
+ *   - all calls on a device share the one array.  Nothing in it has to start at zero (each call overwrites every slot
+ *     it reads), but two calls whose kernels overlap on the GPU -- different streams, different host threads -- race
+ *     on it and return garbage: keep the calls of one device on one stream, or order them with events.
+ *   - the FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current) and keeps it; make that first call during start-up, before any stream capture begins.
+ * Errors: BEM_ERR_INVALID_ARG (sizes, NULL or host pointers, buffers of another device), BEM_ERR_CUDA; the text is
+ * returned by bem_direct_sum_static_last_error() (per host thread). */
+#define BEM_DIRECT_STATIC_MAX_TARGETS 65536
+bem_status bem_direct_sum_static(const double *sources, int64_t n_sources, const double *q, const double *d,
+                                 const double *targets, int64_t n_targets, double *y, void *cuda_stream);
+const char *bem_direct_sum_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

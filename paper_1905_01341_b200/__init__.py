@@ -31,7 +31,9 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
 # every symbol include/bem.h declares
 EXPORTS = ["bem_create", "bem_create_points", "bem_create_evaluator", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
            "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy",
-           "bem_surface_velocity", "bem_surface_curvature", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy"]
+           "bem_surface_velocity", "bem_surface_curvature", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy",
+           "bem_direct_sum_static", "bem_direct_sum_static_last_error"]
+DIRECT_STATIC_MAX_TARGETS = 65536      # BEM_DIRECT_STATIC_MAX_TARGETS of include/bem.h
 
 
 class BemError(RuntimeError):
@@ -78,8 +80,12 @@ def load_library() -> ctypes.CDLL:
     lib.bem_filter_last_error.restype = ctypes.c_char_p
     lib.bem_filter_destroy.argtypes = [vp]
     lib.bem_filter_destroy.restype = None
+    lib.bem_direct_sum_static.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp]
+    lib.bem_direct_sum_static_last_error.argtypes = []
+    lib.bem_direct_sum_static_last_error.restype = ctypes.c_char_p
     for name in EXPORTS:
-        if name not in ("bem_last_error", "bem_destroy", "bem_filter_last_error", "bem_filter_destroy"):
+        if name not in ("bem_last_error", "bem_destroy", "bem_filter_last_error", "bem_filter_destroy",
+                        "bem_direct_sum_static_last_error"):
             getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -269,3 +275,31 @@ class BemFilter:
 
 def bem_filter_create(theta, phi, p_f: int) -> BemFilter:
     return BemFilter(theta, phi, p_f)
+
+
+def bem_direct_sum_static(sources, q, d, targets, y, stream_handle: int = 0):
+    """y_i = sum_j [ q_j / (4 pi r) - d_j . (x_i - y_j) / (4 pi r^3) ] over a point cloud (Eq. 13) through
+    the one entry of the library that allocates no device memory -- for a caller whose GPU is already full of its own
+    arenas, who runs under a fixed memory budget, or who cannot take the device-wide stall of a cudaMalloc in its loop.
+    Its scratch is an 8 MiB array compiled into the library, shared by every call on a device: at most
+    DIRECT_STATIC_MAX_TARGETS targets per call, and calls that overlap on the GPU race (one stream, or events).
+
+    sources [ns x 3], q [ns] or None, d [ns x 3] or None, targets [nt x 3], y [nt]: contiguous float64 CUDA tensors of
+    the current device (host arrays are refused by the library: copying them would need a buffer).  Enqueued on
+    `stream_handle` (0 = default stream), never synchronised.  The first call on a device looks up the scratch
+    address; make it at start-up, outside any stream capture."""
+    lib = load_library()
+    for name, a in (("sources", sources), ("targets", targets)):
+        if a.dim() != 2 or a.shape[1] != 3:
+            raise ValueError(f"{name} must be [n, 3]")
+    ns, nt = sources.shape[0], targets.shape[0]
+    if q is not None and q.numel() != ns:
+        raise ValueError("q must be [n_sources]")
+    if d is not None and tuple(d.shape) != (ns, 3):
+        raise ValueError("d must be [n_sources, 3]")
+    if y.numel() != nt:
+        raise ValueError("y must be [n_targets]")
+    st = lib.bem_direct_sum_static(_ptr(sources), ns, _ptr(q), _ptr(d), _ptr(targets), nt, _ptr(y), ctypes.c_void_p(stream_handle))
+    if st != BEM_OK:
+        raise BemError(st, lib.bem_direct_sum_static_last_error().decode())
+    return y

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libbem_b200.so")
-SOURCES = ["prims.cu", "mesh.cu", "nearfield.cu", "tree.cu", "adaptive.cu", "translate.cu", "p2m_l2p.cu", "p2p.cu", "p2p_f32.cu", "api.cu", "solve.cu", "surface.cu"]
+SOURCES = ["prims.cu", "mesh.cu", "nearfield.cu", "tree.cu", "adaptive.cu", "translate.cu", "p2m_l2p.cu", "p2p.cu", "p2p_f32.cu", "api.cu", "solve.cu", "surface.cu", "direct_static.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
