@@ -121,8 +121,11 @@ bem_status bem_create_points(const double *sources, int64_t n_sources, const dou
  * with the SAME discretisation as bem_apply on the mesh (G3: 3-point Gauss per flat triangle with P1 densities, plus the
  * exact flat-triangle integrals on the near set { k : |x_t - c_k| <= eta d_k } through a CSR correction matrix whose
  * columns are the mesh vertices), the same octree / FMM engine and the same options.
- *   mesh_ctx  a context made by bem_create (its mesh is read during bem_setup of the evaluator: it must be alive until
- *             then; it need not be set up itself).  The evaluator runs on the device and stream of mesh_ctx.
+ *   mesh_ctx  a context made by bem_create (it need not be set up itself).  Its mesh is read by every bem_setup of the
+ *             evaluator and by nothing else: it must be alive during those calls, and may be destroyed after the last
+ *             one -- bem_apply, bem_get_stats and bem_destroy of the evaluator do not touch it (a bem_setup after the
+ *             mesh context is gone is a use-after-free the library cannot detect).  The evaluator runs on the device
+ *             and stream of mesh_ctx.
  *   targets   [n_targets x 3] fp64 points, host or device, copied.  A target ON the surface is not allowed (use
  *             bem_apply for the vertices); a target closer to a triangle than ~1e-6 of its size loses accuracy.
  * Then: bem_setup(ev, p, leaf_size, near_radius); bem_apply(ev, q, phi, u) with q, phi [n_vertices of the MESH] and
@@ -221,6 +224,10 @@ bem_status bem_set_stream(bem_ctx *ctx, void *cuda_stream);
  * interaction lists, translation matrices, and the near-field correction CSR.
  *   p            truncation number: expansions hold degrees n = 0..p-1, p^2 real
  *                coefficients.  1 <= p <= 32.  Ignored in direct mode.
+ *                p is the truncation of the products WITHOUT dipoles (phi == NULL: S[q],
+ *                every iteration of bem_solve).  A product with phi != NULL runs at
+ *                p + 3 when p < 12 (option "dipole_degrees", default -1; 0 = the paper's
+ *                one truncation for both layers); BEM_S_P_DIPOLE reports the value used.
  *   leaf_size    the octree depth l_max is the smallest level >= 2 at which the mean
  *                population of non-empty source boxes is <= leaf_size (the paper's
  *                clustering parameter).  >= 1.

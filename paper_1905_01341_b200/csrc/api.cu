@@ -302,10 +302,15 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
     if (c->quadrature < 2) compute_geometry(c);
     if (c->quadrature == 3 && !c->parent->triA.p) {              // an evaluator uses the areas and normals of its parent's mesh
         CUDA_TRY(cudaSetDevice(c->parent->device));
-        const cudaStream_t ps = c->parent->stream;
-        c->parent->stream = s;
-        compute_geometry(c->parent);
-        c->parent->stream = ps;
+        struct StreamSwap {                                      // the parent's geometry is computed on the evaluator's stream;
+            bem_ctx *ctx; cudaStream_t saved;                    // its own stream comes back whatever compute_geometry throws
+            StreamSwap(bem_ctx *x, cudaStream_t t) : ctx(x), saved(x->stream) { x->stream = t; }
+            ~StreamSwap() { ctx->stream = saved; }
+        };
+        {
+            StreamSwap swap(c->parent, s);
+            compute_geometry(c->parent);
+        }
         CUDA_TRY(cudaStreamSynchronize(s));
     }
     const int64_t N = c->N;
@@ -611,12 +616,18 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
     if (!out) return BEM_ERR_INVALID_ARG;
     *out = nullptr;
     if (!mesh_ctx || !targets || n_targets < 1 || n_targets > 2000000000ll) return BEM_ERR_INVALID_ARG;
-    if (mesh_ctx->quadrature >= 2 || mesh_ctx->T == 0) { mesh_ctx->err = "bem_create_evaluator: the context holds no mesh"; return BEM_ERR_INVALID_ARG; }
+    if (mesh_ctx->quadrature >= 2 || mesh_ctx->T == 0) {
+        mesh_ctx->err = "bem_create_evaluator: the context holds no mesh";
+        g_create_error = mesh_ctx->err;                           // no context is returned: bem_last_error(NULL) is where a caller looks
+        return BEM_ERR_INVALID_ARG;
+    }
     bem_ctx *c = new (std::nothrow) bem_ctx();
     if (!c) return BEM_ERR_OOM;
     c->device = mesh_ctx->device;
     c->stream = mesh_ctx->stream;
     c->parent = mesh_ctx;
+    c->mesh_N = mesh_ctx->N;                                      // bem_apply sizes q and phi with these and never reads the parent
+    c->mesh_T = mesh_ctx->T;
     c->N = n_targets;
     c->T = 0;
     c->quadrature = 3;
@@ -693,7 +704,8 @@ bem_status bem_apply(bem_ctx *c, const double *q, const double *phi, double *y)
         // lengths: q, phi are per mesh vertex (an evaluator: of its parent's mesh); a point cloud takes one monopole and
         // one dipole VECTOR per source; y is per target
         const size_t bytes = c->N * sizeof(double);
-        const size_t nq = c->quadrature == 2 ? c->np : mesh_of(c)->N, nphi = c->quadrature == 2 ? 3 * c->np : mesh_of(c)->N;
+        const size_t nv = c->quadrature == 3 ? c->mesh_N : c->N;    // an evaluator's mesh context may be gone by now (bem.h)
+        const size_t nq = c->quadrature == 2 ? c->np : nv, nphi = c->quadrature == 2 ? 3 * c->np : nv;
         const size_t qbytes = nq * sizeof(double), pbytes = nphi * sizeof(double);
         const bool hq = !is_device_ptr(q), hp = !is_device_ptr(phi), hy = !is_device_ptr(y);
         const double *dq = q, *dp = phi;

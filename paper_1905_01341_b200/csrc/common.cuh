@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 #include <stdexcept>
@@ -77,8 +78,19 @@ inline void d2h_sync(void *dst, const void *src, size_t bytes, cudaStream_t s)
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
 // Function attributes (dynamic shared-memory opt-in, carve-out) are PER DEVICE, and contexts may live on several devices
-// and threads: every launch site keeps one flag per device and asks here, under a mutex, whether it is the first use.
-bool first_use_on_device(std::vector<char> &done, int device);
+// and threads: every launch site keeps one flag per device and sets its attributes through once_per_device.
+// The mutex is held WHILE the attributes are set: a second thread on the same device waits until the opt-in is in place and
+// cannot launch with more dynamic shared memory than the default allows.  A failed set-up leaves the flag clear.
+std::mutex &device_once_mutex();
+template <class F>
+inline void once_per_device(std::vector<char> &done, int device, F &&set_attributes)
+{
+    std::lock_guard<std::mutex> lock(device_once_mutex());
+    if ((int)done.size() <= device) done.resize(device + 1, 0);
+    if (done[device]) return;
+    set_attributes();
+    done[device] = 1;
+}
 }  // namespace bem
 struct bem_ctx;
 namespace bem {
@@ -218,6 +230,8 @@ struct bem_ctx {
     int64_t np = 0;
     bem_ctx *parent = nullptr;      // evaluator (quadrature == 3, bem_create_evaluator): the mesh context whose Gauss points are the
                                     // sources; V holds the evaluation points (N of them), densities are indexed by the parent's vertices
+                                    // Only bem_setup follows this pointer (the mesh may be destroyed after the last set-up):
+    int64_t mesh_N = 0, mesh_T = 0; // evaluator: vertex and triangle counts of the parent's mesh, copied at creation (what bem_apply needs)
 
     // vertex -> incident triangle corners, sorted by vertex (bem_surface_velocity; built at first use)
     bem::dvec<int32_t> vc_begin;    // [N+1]

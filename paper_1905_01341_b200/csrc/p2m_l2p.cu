@@ -182,10 +182,10 @@ static void p2m_launch(bem_ctx *c, int lmax, int nleaf, const int32_t *list, con
     const double h = c->cube_side / (double)(1 << lmax);
     const size_t smem = (size_t)P2M_WARPS * P2M_TBL * sizeof(double);
     static std::vector<char> attr_done;
-    if (first_use_on_device(attr_done, c->device)) {
+    once_per_device(attr_done, c->device, [&]() {
         CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         CUDA_TRY(cudaFuncSetAttribute(p2m_kernel_t<P, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    }
+    });
     auto kern = c->has_dipole ? p2m_kernel_t<P, true> : p2m_kernel_t<P, false>;
     CUDA_TRY(cudaMemsetAsync(c->p2p_counter.get() + 2, 0, sizeof(int), c->stream));
     const int grid = std::max(1, std::min(cdiv(nleaf, P2M_WARPS), P2M_MINB * c->n_sm));     // the CTAs that fit an SM (registers, shared memory)

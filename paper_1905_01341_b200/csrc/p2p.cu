@@ -299,12 +299,12 @@ void launch_p2p_leaves(bem_ctx *c)
 {
     const int nleaf = c->adaptive ? c->ad.n_tleaf : c->tb.nbox[c->tb.lmax];
     static std::vector<char> attr_done;
-    if (first_use_on_device(attr_done, c->device)) {                                                   // same carve-out as the row sums it runs beside (common.cuh)
+    once_per_device(attr_done, c->device, [&]() {                                                      // same carve-out as the row sums it runs beside (common.cuh)
 #define BEM_CARVE(D, S) CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<D, S, 2>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT)); \
                         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel<D, S, 3>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT))
         BEM_CARVE(true, true); BEM_CARVE(true, false); BEM_CARVE(false, true); BEM_CARVE(false, false);
 #undef BEM_CARVE
-    }
+    });
     const bool self = c->quadrature != 0;                       // V1 (j = i) and point clouds may have r = 0; G3 cannot
     // adaptive tree: target leaves in point order (ad.tleaf_begin), source ranges from the CSR (ad.near_ptr, ad.near_rng), nbr = null
     const int32_t *tbeg = c->adaptive ? c->ad.tleaf_begin.get() : c->tb.begin.get();

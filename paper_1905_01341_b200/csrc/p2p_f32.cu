@@ -273,13 +273,13 @@ void launch_p2p_leaves_f32(bem_ctx *c, cudaStream_t stream, int ctas_per_sm, int
     CUDA_TRY(cudaMemsetAsync(c->p2p_counter.get() + part, 0, sizeof(int), stream));
     const bool self = c->quadrature != 0;
     static std::vector<char> attr_done;
-    if (first_use_on_device(attr_done, c->device)) {
+    once_per_device(attr_done, c->device, [&]() {
         // same shared-memory carve-out as the row sums it runs beside (common.cuh): an SM only holds CTAs of one carve-out
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<true, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<true, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<false, true>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
         CUDA_TRY(cudaFuncSetAttribute(p2p_leaf_kernel_f32<false, false>, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
-    }
+    });
 #define BEM_F32_ARGS c->tgt_pos.get(), c->tb.begin.get(), c->tb.bkey[lmax].get(), c->nbr.get(), c->xdir_ptr.p, c->xdir_src.p, c->sb.begin.get(), \
                      c->sb.bkey[lmax].get(), c->src_pos_f.get(), c->src_str_f.get(), c->cube_min[0], c->cube_min[1], \
                      c->cube_min[2], h, leaf0, nleaf, c->p2p_counter.get() + part, c->ypart.get() + c->N

@@ -591,15 +591,11 @@ translate_dmma_split16(const Tile *__restrict__ tiles, const int32_t *__restrict
     }
 }
 
-// attributes of a kernel are per device: one flag per device, under a mutex (several contexts, several devices)
-bool first_use_on_device(std::vector<char> &done, int device)
+// attributes of a kernel are per device: one flag per device, set under this mutex (common.cuh once_per_device)
+std::mutex &device_once_mutex()
 {
     static std::mutex mu;
-    std::lock_guard<std::mutex> lock(mu);
-    if ((int)done.size() <= device) done.resize(device + 1, 0);
-    if (done[device]) return false;
-    done[device] = 1;
-    return true;
+    return mu;
 }
 
 template <int PL>
@@ -608,11 +604,11 @@ static void launch_dmma(bem_ctx *c, const Stage &st, int which, cudaStream_t str
     constexpr int KSH = ke_of(PL);
     const size_t smem = (size_t)2 * 4 * KSH * DM_S * sizeof(double);
     static std::vector<char> attr_done;
-    if (first_use_on_device(attr_done, c->device)) {
+    once_per_device(attr_done, c->device, [&]() {
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma<KSH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split<PL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (PL == 12) CUDA_TRY(cudaFuncSetAttribute(translate_dmma_split16<(PL == 12 ? PL : 4)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    }
+    });
     if (which != TILES_DENSE && st.ntiles_split > 0) {
         if (PL == 12 && c->m2l_rows16)                           // measured: pays at p = 11, 12 (cfg 5), not at p <= 10 (cfg 4)
             translate_dmma_split16<(PL == 12 ? PL : 4)><<<st.ntiles_split, DM16_THREADS, smem, stream>>>(
@@ -857,13 +853,15 @@ void launch_stage_reduce(bem_ctx *c, const Stage &st, cudaStream_t stream, int c
     if (nvisit == 0) return;
     const int grid = ctas_per_sm > 0 ? std::min(nvisit, c->n_sm * ctas_per_sm) : nvisit;
     static std::vector<char> attr_done;
-    if (first_use_on_device(attr_done, c->device))                     // same carve-out as the pair kernels it runs beside (common.cuh)
+    once_per_device(attr_done, c->device, [&]() {                       // same carve-out as the pair kernels it runs beside (common.cuh)
         CUDA_TRY(cudaFuncSetAttribute(translate_reduce, cudaFuncAttributePreferredSharedMemoryCarveout, CORUN_CARVEOUT));
+    });
     if (c->reduce_stream && c->nre <= RS_THREADS) {                    // rows streamed through shared memory (cp.async)
         const size_t smem = (size_t)RS_STAGES * RS_ROWS * c->nst * sizeof(double);
         static std::vector<char> attr2_done;
-        if (first_use_on_device(attr2_done, c->device))
+        once_per_device(attr2_done, c->device, [&]() {
             CUDA_TRY(cudaFuncSetAttribute(translate_reduce_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_STAGES * RS_ROWS * 2 * RS_THREADS * (int)sizeof(double)));
+        });
         translate_reduce_stream<<<grid, std::max(64, ((c->nre + 31) / 32) * 32), smem, stream>>>(
             st.ptr.get(), st.mat_t.get(), c->mat_ne.get(), c->mat_w.get(), st.row_off[c->lay_active].get(),
             c->scratch.get() + (size_t)st.region_units[c->lay_active] * 16,

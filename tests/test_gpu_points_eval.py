@@ -185,9 +185,37 @@ def test_evaluator_greens_representation_and_errors():
         ev.bem_set_option("quadrature", 1)
     with pytest.raises(bem.BemError):
         bem.bem_create_evaluator(ev, X)                      # an evaluator has no mesh of its own
-    assert "mesh" in bem.load_library().bem_last_error(None).decode() or True
+    assert "holds no mesh" in bem.load_library().bem_last_error(None).decode()
     ev.bem_destroy()
     mesh.bem_destroy()
+
+
+def test_evaluator_outlives_its_mesh_context():
+    """include/bem.h: the mesh context is read by bem_setup of the evaluator only.  Destroy it after the set-up, let another
+    context of another size take its place on the heap, and the evaluator's products (host buffers: their staging is sized
+    by the MESH's vertex count) must not change by a bit."""
+    bem = _bem()
+    V, F = bi.icosphere(3)
+    rng = np.random.default_rng(47)
+    X = _shell_points(V, rng, 1500)
+    q, phi = rng.normal(size=V.shape[0]), rng.normal(size=V.shape[0])
+    mesh = bem.bem_create(V, F, None)
+    ev = bem.bem_create_evaluator(mesh, X)
+    ev.bem_setup(10, 64, 2.5)
+    mesh.bem_destroy()
+    V2, F2 = bi.icosphere(2)
+    others = [bem.bem_create(V2 * (1 + k), F2, None) for k in range(4)]      # same-sized heap blocks, other N and T
+    u1 = np.full(X.shape[0], np.nan)
+    ev.bem_apply(q, phi, u1)
+    u2 = np.full(X.shape[0], np.nan)
+    ev.bem_apply(q, phi, u2)
+    st = ev.bem_get_stats()
+    assert st["n_targets"] == X.shape[0] and st["n_sources"] == 3 * F.shape[0]
+    assert np.array_equal(u1, u2)
+    assert _rel(u1, oracle.g3_evaluate(V, F, q, phi, X, eta=2.5)) <= 1e-5
+    ev.bem_destroy()
+    for o in others:
+        o.bem_destroy()
 
 
 def test_evaluator_on_a_cluster_sampled_points():
