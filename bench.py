@@ -10,7 +10,9 @@ on a seeded synthetic bubble cluster.  Default workload: config 5 of BASELINE.js
 
   value     ms per bem_apply with q, phi, y resident in HBM (CUDA events on the context's stream)
   e2e       the same call with HOST buffers: H2D of q and phi, D2H of y inside the timed region
-  roofline  the dominant kernel (M2L batched GEMM) against the FP64 peak
+  roofline  the dominant kernel (on config 5 the near-field pair kernel p2p_leaf_kernel, FP64 ALU bound) against the
+            DFMA loop measured in the same run; the other kernels with their own roofs under "kernels"
+  sweep     (default run only) configs 1-4 timed the same way: the metric is ms/apply VERSUS N nodes
   cpu_baseline  the CPU oracle, timed on a bounded sample of target rows of the same workload
 
 The path does not shard (BASELINE.json: one GPU, no collectives): --gpus N runs N independent
@@ -76,6 +78,22 @@ def bench_leaf_size(args, c):
     return 350 if (args.config == 5 and use_adaptive_tree(args)) else int(c["leaf_size"])
 
 
+def p_with_dipoles(args, p):
+    """The truncation a product WITH phi executes (include/bem.h option "dipole_degrees"; R5'): the stated p is the
+    truncation of the monopole (single-layer) products; dipole sources carry 3 more degrees below p = 12 unless the option
+    says otherwise.  Direct mode has no truncation.  run_gpu checks this against the library's own BEM_S_P_DIPOLE."""
+    if args.direct:
+        return int(p)
+    dd = None
+    for o in args.opt:
+        k, _, v = o.replace(" ", "").partition("=")
+        if k == "dipole_degrees":
+            dd = int(float(v))
+    if dd is None or dd < 0:
+        dd = 3 if p < 12 else 0
+    return int(min(32, p + dd))
+
+
 def workload_config(c, args, p):
     """The keys that name the workload -- the SAME dict in the b200 arm and in the reference arm (the CPU oracle computes
     the same discretised operator on the same inputs); what only the GPU run knows (tree depth, launch mode, device bytes)
@@ -83,7 +101,9 @@ def workload_config(c, args, p):
     N, T = int(c["V"].shape[0]), int(c["F"].shape[0])
     cloud = bool(c.get("cloud"))
     return dict(workload=workload_name(c), operator="y = S[q] - D[phi] (G3 quadrature + near correction)" if not cloud else "monopole sum",
-                p=int(p), n_nodes=N, n_triangles=T, n_sources=(N if cloud else 3 * T), leaf_size=bench_leaf_size(args, c),
+                p=int(p), p_executed_with_phi=(int(p) if cloud else p_with_dipoles(args, p)),
+                p_note="p = truncation of the products without dipoles (S[q], every GMRES iteration); S[q] - D[phi] runs at p_executed_with_phi",
+                n_nodes=N, n_triangles=T, n_sources=(N if cloud else 3 * T), leaf_size=bench_leaf_size(args, c),
                 eta=c["eta"], parallelism="replicas only" if args.gpus > 1 else "1 gpu",
                 l2="working set larger than L2" if N >= 100000 else "flushed between iterations (512 MB write)")
 
@@ -206,6 +226,60 @@ class ClockSampler:
         os.unlink(self.f.name)
         return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=float(max(mx)) if mx else None,
                     samples=len(sm), reasons=sorted(reasons))
+
+
+def run_sweep(args, bem, torch, stream):
+    """The other points of "ms/apply vs N nodes" (BASELINE.json metric): configs 1-4 with the library's defaults at each
+    config's own p and leaf_size, timed like the headline (device-resident value, end-to-end with host buffers) and checked
+    against the oracle on seeded rows (all rows on config 1).  A failure is recorded, it does not cost the headline."""
+    import oracle
+    out = []
+    fbuf = torch.empty(512 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")
+
+    def timed(fn, steps, flush):
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            if flush:
+                fbuf.fill_(1.0)
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        return sum(a.elapsed_time(b) for a, b in evs)
+
+    for k in (1, 2, 3, 4):
+        try:
+            c = make_config(k)
+            V, F = c["V"], c["F"]
+            N = V.shape[0]
+            ctx = bem.bem_create(V, F, c["bubble_id"])
+            ctx.bem_set_stream(stream.cuda_stream)
+            ctx.bem_setup(c["p"], c["leaf_size"], c["eta"])
+            st = ctx.bem_get_stats()
+            qd, pd = torch.tensor(c["q"], device="cuda"), torch.tensor(c["phi"], device="cuda")
+            yd = torch.empty_like(qd)
+            qh, ph = torch.tensor(c["q"]).pin_memory(), torch.tensor(c["phi"]).pin_memory()
+            yh = torch.empty(N, dtype=torch.float64).pin_memory()
+            n_it = max(3, min(args.steps, 10))
+            for _ in range(3):
+                ctx.bem_apply(qd, pd, yd)
+            flush = N < 100000
+            ms = timed(lambda: ctx.bem_apply(qd, pd, yd), n_it, flush) / n_it
+            for _ in range(2):
+                ctx.bem_apply(qh, ph, yh)
+            e2e = timed(lambda: ctx.bem_apply(qh, ph, yh), n_it, flush) / n_it
+            y = yd.cpu().numpy()
+            rows = sample_rows(c["cfg"], N, N if N < 3000 else args.sweep_rows)
+            yo = oracle.g3_apply(V, F, c["q"], c["phi"], eta=c["eta"], rows=rows)
+            out.append(dict(config=k, workload=c["name"], n_nodes=int(N), p=int(c["p"]), p_executed_with_phi=int(st["p_dipole"]),
+                            leaf_size=int(c["leaf_size"]), lmax=int(st["lmax"]), ms=ms, e2e_ms=e2e, steps=n_it,
+                            parity_rel_l2_vs_oracle=float(np.linalg.norm(y[rows] - yo) / np.linalg.norm(yo)), parity_rows=int(len(rows)),
+                            l2="flushed between iterations (512 MB write)" if flush else "working set larger than L2"))
+            ctx.bem_destroy()
+            del qd, pd, yd
+        except Exception as e:  # noqa: BLE001
+            out.append(dict(config=k, error=repr(e)[:300]))
+    return out
 
 
 def run_gpu(args):
@@ -353,6 +427,8 @@ def run_gpu(args):
     p2p_s = tm["p2p"] * 1e-3
     kernels["p2p"] = dict(ms=tm["p2p"], pairs=stats["p2p_pairs"], pairs_executed=stats["p2p_pairs_executed"],
                           executed_note="source lists are padded to rounds of 128: pairs / pairs_executed of the kernel's work is useful",
+                          pairs_wx=stats["p2p_pairs_wx"], wx_share=(stats["p2p_pairs_wx"] / stats["p2p_pairs"]) if stats["p2p_pairs"] else None,
+                          wx_note="adaptive tree: pairs of W-list and X-list ranges, which the library sums directly instead of M2P / P2L (0 on the uniform tree)",
                           gpairs_per_s=stats["p2p_pairs"] / p2p_s / 1e9 if p2p_s > 0 else None,
                           tflops=stats["p2p_pairs"] * P2P_FLOP / p2p_s / 1e12 if p2p_s > 0 else None,
                           fp64_slot_frac=stats["p2p_pairs"] * P2P_INSTR / p2p_s / 1e12 / slot_peak if p2p_s > 0 else None,
@@ -365,19 +441,45 @@ def run_gpu(args):
         kernels["m2l"] = dict(ms=tm["m2l"], pairs=stats["m2l_pairs"], executed_tflops=exec_flop / m2l_s / 1e12,
                               dense_equivalent_tflops=dense_flop / m2l_s / 1e12,
                               frac_of_measured_dmma_peak=exec_flop / m2l_s / 1e9 / dmma, frac_of_nominal_fp64_peak=exec_flop / m2l_s / 1e9 / FP64_NOMINAL_GFLOPS,
-                              note="executed = 4 nre^2 flop per pair on the FP64 tensor path (nre = %d); dense-equivalent = 2 p^4" % int(nre))
+                              note="executed = the graded-truncation count the library reports (BEM_S_M2L_FLOP): per pair two blocks of (4 KE)^2 "
+                                   "multiply-adds, KE = k-steps of the pair's truncation class (full order: 4 nre^2 flop, nre = %d); dense-equivalent = 2 p^4" % int(nre))
         red_bytes = stats["m2l_row_bytes"]
         kernels["reduce"] = dict(ms=tm["l2l_reduce"], gbs=red_bytes / (tm["l2l_reduce"] * 1e-3) / 1e9,
                                  frac_hbm=red_bytes / (tm["l2l_reduce"] * 1e-3) / 1e9 / hbm_peak, bytes=red_bytes,
-                                 note="reads one translated row (8 nst bytes) per pair; L2L rows not counted")
-        p2m_bytes = 64.0 * stats["n_sources"] + 8.0 * stats["exp_stride"] * stats["n_src_leaves"]
-        kernels["p2m"] = dict(ms=tm["p2m"], gbs=p2m_bytes / (tm["p2m"] * 1e-3) / 1e9, msources_per_s=stats["n_sources"] / (tm["p2m"] * 1e-3) / 1e6)
+                                 note="bytes = the packed translated rows the sums read (BEM_S_M2L_ROW_BYTES: 16 bytes x the dofs each pair's "
+                                      "truncation class carries); the L2L tiles and sums run in the same timing class and their rows are not counted")
+        # P2M is FP64-ALU bound: FP64 SASS instructions of p2m_kernel_t<P, DIP> per (lane, source) -- static count of
+        # DFMA + DMUL + DADD in the kernel (cuobjdump -sass); the 32-entry row sums execute 4x their static 8, so it is a lower bound
+        P2M_FP64 = {(8, 0): 323, (8, 1): 617, (10, 0): 499, (10, 1): 967, (12, 0): 690, (12, 1): 1372, (14, 0): 930, (14, 1): 1866,
+                    (16, 0): 1207, (16, 1): 2450}
+        p_run = int(stats["p_dipole"]) if pd is not None else int(p)
+        key = (max(8, p_run + (p_run & 1)), 0 if pd is None else 1)
+        ins = P2M_FP64.get(key)
+        p2m_s = tm["p2m"] * 1e-3
+        kernels["p2m"] = dict(ms=tm["p2m"], msources_per_s=stats["n_sources"] / p2m_s / 1e6, bound="alu",
+                              fp64_instr_per_source=ins,
+                              fp64_slot_frac_lower_bound=(stats["n_sources"] * ins / p2m_s / 1e12 / (FP64_NOMINAL_GFLOPS / 2e3)) if ins else None,
+                              note="FP64 instructions per source: static SASS count of p2m_kernel_t<%d, %s>; slots against the nominal 18.6 T instr/s; "
+                                   "idle lanes of ragged leaves not counted" % (key[0], "dipoles" if key[1] else "monopoles"))
+        # tree passes that only move data (north_star: "achieved HBM GB/s for SpMV and tree passes, each against the B200 peak");
+        # algorithmic bytes per unit as stated in DESIGN.md section 8
+        nst = stats["exp_stride"]
+        tree = dict(
+            lift=(80.0 * stats["n_sources"], "80 B per source (weights 32, vertex ids 16, strengths written 32); the densities (16 N B) stay in L2 and are not counted"),
+            m2m=(8.0 * nst * (stats["m2m_pairs"] + stats["m2m_parents"]), "one child expansion read per (child, parent) translation, one parent expansion written (8 nst B each)"),
+            l2p=(32.0 * N + 8.0 * nst * stats["n_tgt_leaves"], "24 B position + 8 B result per target, one local expansion (8 nst B) per target leaf"))
+        for name, (nbytes, what) in tree.items():
+            t_s = tm[name] * 1e-3
+            if t_s > 0:
+                kernels[name] = dict(ms=tm[name], bytes=nbytes, gbs=nbytes / t_s / 1e9, frac_hbm=nbytes / t_s / 1e9 / hbm_peak, note=what)
+        kernels["l2l"] = dict(note="runs inside the 'reduce' timing class (L2L tiles + sums follow the M2L sums of each level): no separate figure")
     spmv_bytes = 20.0 * stats["csr_nnz"] + 32.0 * N
     kernels["spmv"] = dict(ms=tm["spmv"], gbs=spmv_bytes / (tm["spmv"] * 1e-3) / 1e9, frac_hbm=spmv_bytes / (tm["spmv"] * 1e-3) / 1e9 / hbm_peak,
                            hbm_peak_gbs=hbm_peak, hbm_peak_source=hbm_src, bytes=spmv_bytes)
-    common = dict(peak_source="derived: 148 SMs x 64 FP64 lanes/clk x 2 flop x 1.965 GHz (MEASURED_PEAKS.json has no FP64 entry); "
-                              "measured in this run: DFMA loop %.1f, DMMA loop %.1f TFLOP/s" % (dfma / 1e3, dmma / 1e3),
-                  measured_dfma_tflops=dfma / 1e3, measured_dmma_tflops=dmma / 1e3)
+    common = dict(peak_source="measured in this run: register-resident DFMA loop (bem_fp64_peak) %.1f TFLOP/s, DMMA loop %.1f TFLOP/s; "
+                              "MEASURED_PEAKS.json has no FP64 entry; derived nominal for context: 148 SMs x 64 FP64 lanes/clk x 2 flop x 1.965 GHz = %.1f"
+                              % (dfma / 1e3, dmma / 1e3, FP64_NOMINAL_GFLOPS / 1e3),
+                  measured_dfma_tflops=dfma / 1e3, measured_dmma_tflops=dmma / 1e3, derived_nominal_tflops=FP64_NOMINAL_GFLOPS / 1e3)
     if f32 and tm["p2p"] >= tm["m2l"]:
         k = kernels["p2p"]
         peak32 = 2.0 * FP64_NOMINAL_GFLOPS / 1e3
@@ -387,9 +489,14 @@ def run_gpu(args):
                     peak_source="derived: 148 SMs x 128 FP32 lanes/clk x 2 flop x 1.965 GHz")
     elif args.direct or tm["p2p"] >= tm["m2l"]:
         k = kernels["p2p"]
+        # two conventions, both printed: "flop" counts an FMA as 2 and a DMUL / DADD as 1 (so a kernel of 8 FMA + 8 others
+        # cannot pass 0.75); "slots" counts FP64 instructions against the pipe's issue rate and is what ncu's
+        # sm__pipe_fp64_cycles_active measures.  frac is the flop convention against the MEASURED DFMA loop.
         roof = dict(kernel="p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", bound="alu", achieved=k["tflops"],
-                    peak=FP64_NOMINAL_GFLOPS / 1e3, unit="TFLOP/s", frac=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
-                    fp64_slot_frac=k["fp64_slot_frac"], traffic=ncu_traffic("p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", args.config),
+                    peak=dfma / 1e3, unit="TFLOP/s", frac=k["tflops"] / (dfma / 1e3), frac_convention="flop / measured DFMA-loop flop rate",
+                    frac_of_derived_nominal=k["tflops"] / (FP64_NOMINAL_GFLOPS / 1e3),
+                    fp64_slot_frac=k["fp64_slot_frac"], fp64_slot_frac_of_measured=k["fp64_slot_frac"] * FP64_NOMINAL_GFLOPS / dfma,
+                    traffic=ncu_traffic("p2p_direct_kernel" if args.direct else "p2p_leaf_kernel", args.config),
                     algorithmic="%d flop (%d FP64 instructions) per pair x %d pairs" % (P2P_FLOP, P2P_INSTR, stats["p2p_pairs"]), ms=tm["p2p"],
                     share_of_step=tm["p2p"] / tm["total"], **common)
     else:
@@ -459,7 +566,8 @@ def run_gpu(args):
         cu.bem_destroy()
         uniform = dict(option="tree = 0: uniform depth l_max, the paper's tree (PAPER.md:440) and the library default", value=u_ms, unit=UNIT,
                        lmax=int(su["lmax"]), breakdown_ms={k: round(v, 4) for k, v in tu.items()}, m2l_pairs=int(su["m2l_pairs"]),
-                       p2p_pairs=su["p2p_pairs"], device_bytes=int(su["device_bytes"]),
+                       p2p_pairs=su["p2p_pairs"], device_bytes=int(su["device_bytes"] - stats["device_bytes"]),
+                       device_bytes_note="BEM_S_DEVICE_BYTES counts every live context of the process: the headline context's bytes are subtracted",
                        parity_rel_l2_vs_oracle=float(np.linalg.norm(yu[rows] - yo) / np.linalg.norm(yo)),
                        with_fp32_pairs=dict(value=u32_ms, unit=UNIT,
                                             parity_rel_l2_vs_oracle=float(np.linalg.norm(yu32[rows] - yo) / np.linalg.norm(yo))))
@@ -549,9 +657,14 @@ def run_gpu(args):
         if not args.direct:
             ctx.bem_set_option("p2p_precision", 1 if f32 else 0)
 
+    cfg_d = workload_config(c, args, p)
+    if not cloud and not args.direct:
+        cfg_d["p_executed_with_phi"] = int(stats["p_dipole"])         # the library's own word (equals the rule of p_with_dipoles)
+    sweep = run_sweep(args, bem, torch, stream) if (args.sweep and args.config == 5 and world == 1 and not args.direct) else None
+
     line = dict(metric=METRIC, value=ms, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms,
                 higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64 (near-field pairs f32)" if f32 else "f64", data="synthetic",
-                config=workload_config(c, args, p),
+                config=cfg_d, sweep=sweep,
                 run=dict(mode="direct" if args.direct else "fmm", tree="adaptive" if adaptive else "uniform", p2p_precision="fp32 pairs, fp64 sums" if f32 else "fp64",
                          p_dipole=int(stats["p_dipole"]), lmax=int(stats["lmax"]), n_src_leaves=int(stats["n_src_leaves"]),
                          n_tgt_leaves=int(stats["n_tgt_leaves"]),
@@ -601,6 +714,9 @@ def main():
     ap.add_argument("--solve-check-rows", type=int, default=400,
                     help="rows on which the ORACLE recomputes the residual of the first bem_solve (three oracle products; 0: skip)")
     ap.add_argument("--ref-seconds", type=float, default=12.0, help="CPU time budget of one oracle sample")
+    ap.add_argument("--no-sweep", dest="sweep", action="store_false",
+                    help="skip the configs 1-4 points that the default config-5 run appends (\"ms/apply vs N nodes\")")
+    ap.add_argument("--sweep-rows", type=int, default=500, help="seeded oracle rows of each sweep point (all rows below 3000 nodes)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

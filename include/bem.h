@@ -71,13 +71,20 @@ enum {
 enum {
     BEM_S_N_TARGETS = 0, BEM_S_N_SOURCES, BEM_S_LMAX, BEM_S_N_SRC_LEAVES, BEM_S_N_TGT_LEAVES,
     BEM_S_P2P_PAIRS, BEM_S_M2L_PAIRS, BEM_S_CSR_NNZ, BEM_S_NEAR_TRIANGLES, BEM_S_SETUP_MS,
-    BEM_S_N_SRC_BOXES, BEM_S_N_TGT_BOXES, BEM_S_DEVICE_BYTES, BEM_S_EXP_STRIDE,
+    BEM_S_N_SRC_BOXES, BEM_S_N_TGT_BOXES,
+    BEM_S_DEVICE_BYTES,    /* live device bytes of ALL contexts and filters of the process (one atomic counter), not of ctx alone */
+    BEM_S_EXP_STRIDE,
     BEM_S_KERNEL_LAUNCHES_PER_APPLY,
     BEM_S_M2L_FLOP,        /* executed flop of the M2L tiles of one product (graded truncation: 4 (4 KE)^2 per pair) */
     BEM_S_M2L_ROW_BYTES,   /* bytes of translated rows the per-target sums read in one product                     */
     BEM_S_P_DIPOLE,        /* truncation number of the products that carry dipoles (option "dipole_degrees")                 */
     BEM_S_P2P_PAIRS_EXECUTED, /* point pairs the near-field kernel executes: BEM_S_P2P_PAIRS are the useful ones, the source list
                                of a target leaf is padded to whole rounds of 128 sources                               */
+    BEM_S_P2P_PAIRS_WX,    /* adaptive tree: the point pairs of BEM_S_P2P_PAIRS that belong to W-list ranges (children, not touching the
+                            * target leaf, of a subdivided same-level neighbour) and X-list ranges (coarser source leaves that touch an
+                            * ancestor but not the leaf): the library sums them directly; an FMM with M2P / P2L would expand them   */
+    BEM_S_M2M_PAIRS,       /* (child, parent) translations of one upward pass                                               */
+    BEM_S_M2M_PARENTS,     /* parent boxes written by the upward pass                                                        */
     BEM_S_COUNT
 };
 

@@ -26,7 +26,7 @@ STATUS_NAMES = ["BEM_OK", "BEM_ERR_INVALID_ARG", "BEM_ERR_BAD_MESH", "BEM_ERR_NO
 TIMING_NAMES = ["lift", "p2m", "m2m", "m2l", "l2l_reduce", "l2p", "p2p", "spmv", "total"]
 STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", "p2p_pairs", "m2l_pairs", "csr_nnz",
               "near_triangles", "setup_ms", "n_src_boxes", "n_tgt_boxes", "device_bytes", "exp_stride",
-              "kernel_launches_per_apply", "m2l_flop", "m2l_row_bytes", "p_dipole", "p2p_pairs_executed"]
+              "kernel_launches_per_apply", "m2l_flop", "m2l_row_bytes", "p_dipole", "p2p_pairs_executed", "p2p_pairs_wx", "m2m_pairs", "m2m_parents"]
 
 # every symbol include/bem.h declares
 EXPORTS = ["bem_create", "bem_create_points", "bem_create_evaluator", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",

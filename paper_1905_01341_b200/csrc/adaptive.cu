@@ -143,7 +143,8 @@ __global__ void all_box_tables(const uint64_t *tkey, int n, int base, int level,
 // direct source ranges of every target leaf (count pass: rng == nullptr).  Order: the coarser levels first, then the own
 // level, then the far leaves summed directly -- a fixed order, so the sums are bit-reproducible.
 __global__ void near_lists(const int32_t *tleaf_gbox, const int32_t *tleaf_begin, int nleaf, LevelTables L,
-                           int32_t *count, const int32_t *ptr, int2 *rng, unsigned long long *pairs, unsigned long long *pairs_exec)
+                           int32_t *count, const int32_t *ptr, int2 *rng, unsigned long long *pairs, unsigned long long *pairs_exec,
+                           unsigned long long *pairs_wx)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= nleaf) return;
@@ -156,6 +157,7 @@ __global__ void near_lists(const int32_t *tleaf_gbox, const int32_t *tleaf_begin
     int cnt = 0;
     int w = ptr ? ptr[i] : 0;
     long long S = 0;
+    long long SX = 0;       // statistics (BEM_S_P2P_PAIRS_WX): sources of the ranges an FMM with M2P / P2L would not sum directly
     for (int l = 2; l <= lt; ++l) {
         const int sh = lt - l;
         const int ax = (int)(ix >> sh), ay = (int)(iy >> sh), az = (int)(iz >> sh);     // the ancestor of level l
@@ -172,6 +174,24 @@ __global__ void near_lists(const int32_t *tleaf_gbox, const int32_t *tleaf_begin
                     if (rng) rng[w++] = make_int2(s0, n);
                     ++cnt;
                     S += n;
+                    if (!count) continue;
+                    if (l < lt) {
+                        // X list: a coarser source leaf next to the ancestor that does not touch the leaf itself (P2L would serve)
+                        const int lox = x << sh, loy = y << sh, loz = z << sh, ext = (1 << sh);
+                        const bool touch = (int)ix >= lox - 1 && (int)ix <= lox + ext && (int)iy >= loy - 1 && (int)iy <= loy + ext &&
+                                           (int)iz >= loz - 1 && (int)iz <= loz + ext;
+                        if (!touch) SX += n;
+                    } else if (L.s_sub[l][sbx]) {
+                        // W list: children of a subdivided neighbour that do not touch the leaf (M2P would serve)
+                        for (int ch = 0; ch < 8; ++ch) {
+                            const int cx = 2 * x + (ch & 1), cy = 2 * y + ((ch >> 1) & 1), cz = 2 * z + (ch >> 2);
+                            const int cb = find_box(L.skey[l + 1], L.nsb[l + 1], morton_encode(cx, cy, cz));
+                            if (cb < 0) continue;
+                            const bool touch = cx >= 2 * (int)ix - 1 && cx <= 2 * (int)ix + 2 && cy >= 2 * (int)iy - 1 && cy <= 2 * (int)iy + 2 &&
+                                               cz >= 2 * (int)iz - 1 && cz <= 2 * (int)iz + 2;
+                            if (!touch) SX += L.s_pbeg[l + 1][cb + 1] - L.s_pbeg[l + 1][cb];
+                        }
+                    }
                 }
     }
     if (L.x_ptr[lt]) {                                                                  // far leaves of the own level summed directly
@@ -188,6 +208,7 @@ __global__ void near_lists(const int32_t *tleaf_gbox, const int32_t *tleaf_begin
         const long long nt = tleaf_begin[i + 1] - tleaf_begin[i];
         atomicAdd(pairs, (unsigned long long)(nt * S));
         atomicAdd(pairs_exec, (unsigned long long)(nt * ((S + 127) / 128) * 128));
+        atomicAdd(pairs_wx, (unsigned long long)(nt * SX));
     }
 }
 
@@ -318,7 +339,7 @@ void build_adaptive(bem_ctx *c)
     }
 
     dvec<unsigned long long> pc;
-    pc.alloc(2);
+    pc.alloc(3);
     // M2L stages of the existing boxes, levels 2 .. lmax; far pairs between two sparse leaves go to the direct lists
     c->m2l.clear();
     c->m2l.resize(lmax + 1);
@@ -449,16 +470,17 @@ void build_adaptive(bem_ctx *c)
     cnt.alloc(ad.n_tleaf);
     pc.zero(s);
     near_lists<<<cdiv(ad.n_tleaf, 128), 128, 0, s>>>(ad.tleaf_gbox.get(), ad.tleaf_begin.get(), ad.n_tleaf, L, cnt.get(), nullptr, nullptr,
-                                                     pc.get(), pc.get() + 1);
+                                                     pc.get(), pc.get() + 1, pc.get() + 2);
     KERNEL_CHECK();
     ad.near_ptr.alloc(ad.n_tleaf + 1);
     scan_exclusive_i32(cnt.get(), ad.near_ptr.get(), ad.n_tleaf, s);
     int nseg = 0;
     d2h_sync(&nseg, ad.near_ptr.get() + ad.n_tleaf, sizeof(int), s);
-    unsigned long long hp[2];
+    unsigned long long hp[3];
     d2h_sync(hp, pc.get(), sizeof hp, s);
     c->p2p_pairs = (int64_t)hp[0];
     c->p2p_pairs_exec = (int64_t)hp[1];
+    c->p2p_pairs_wx = (int64_t)hp[2];
     dvec<int> mx;
     mx.alloc(1);
     mx.zero(s);
@@ -470,7 +492,7 @@ void build_adaptive(bem_ctx *c)
         throw Error(BEM_ERR_INVALID_ARG, "adaptive tree: a target leaf has more than 256 direct source ranges (raise leaf_size or lower direct_pairs)");
     ad.near_rng.alloc(nseg);
     near_lists<<<cdiv(ad.n_tleaf, 128), 128, 0, s>>>(ad.tleaf_gbox.get(), ad.tleaf_begin.get(), ad.n_tleaf, L, nullptr, ad.near_ptr.get(),
-                                                     ad.near_rng.get(), pc.get(), pc.get() + 1);
+                                                     ad.near_rng.get(), pc.get(), pc.get() + 1, pc.get() + 2);
     KERNEL_CHECK();
     CUDA_TRY(cudaStreamSynchronize(s));
 }

@@ -748,7 +748,7 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
     s[BEM_S_CSR_NNZ] = (double)c->nnz;
     s[BEM_S_NEAR_TRIANGLES] = (double)c->near_tris;
     s[BEM_S_SETUP_MS] = c->setup_ms;
-    s[BEM_S_DEVICE_BYTES] = (double)g_device_bytes;
+    s[BEM_S_DEVICE_BYTES] = (double)g_device_bytes.load();
     s[BEM_S_EXP_STRIDE] = c->lay[c->n_lay - 1].nst;
     s[BEM_S_KERNEL_LAUNCHES_PER_APPLY] = c->launches_per_apply;
     if (c->mode == 0) {
@@ -762,6 +762,11 @@ bem_status bem_get_stats(const bem_ctx *c, double *out, int n)
         s[BEM_S_M2L_FLOP] = Lf.m2l_flop;
         s[BEM_S_M2L_ROW_BYTES] = Lf.m2l_row_bytes;
         s[BEM_S_P_DIPOLE] = Lf.p;
+        s[BEM_S_P2P_PAIRS_WX] = c->adaptive ? (double)c->p2p_pairs_wx : 0.0;
+        for (const bem::Stage &st : c->m2m) {
+            s[BEM_S_M2M_PAIRS] += (double)st.npairs;
+            if (st.npairs > 0) s[BEM_S_M2M_PARENTS] += (double)(st.n_list >= 0 ? st.n_list : st.ntgt);
+        }
         s[BEM_S_N_SRC_BOXES] = c->sb.total();
         s[BEM_S_N_TGT_BOXES] = c->tb.total();
     } else {

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <cstdio>
+#include <atomic>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -29,7 +30,7 @@ inline void cuda_check(cudaError_t e, const char *what, const char *file, int li
 #define CUDA_TRY(x) ::bem::cuda_check((x), #x, __FILE__, __LINE__)
 #define KERNEL_CHECK() ::bem::cuda_check(cudaGetLastError(), "kernel launch", __FILE__, __LINE__)
 
-extern size_t g_device_bytes;      // running total of live device allocations (stats only)
+extern std::atomic<size_t> g_device_bytes;   // running total of the live device allocations of ALL contexts of the process (stats only)
 
 // Owning device array.
 template <class T>
@@ -309,6 +310,7 @@ struct bem_ctx {
     std::vector<bem::Stage> m2l;    // 2 .. lmax: L_own(l) = sum of the M2L rows of the level
     std::vector<bem::Stage> l2l;    // 3 .. lmax: L(l) = L_own(l) + L2L L(l-1)
     int64_t m2l_pairs = 0, p2p_pairs = 0;
+    int64_t p2p_pairs_wx = 0;       // adaptive tree: the part of p2p_pairs that comes from W-list and X-list ranges (summed directly here)
     int64_t p2p_pairs_exec = 0;     // pairs the near-field kernel executes: source lists padded to rounds of 128 (tree.cu)
 
     // partial sums of the point engine, combined by the SpMV kernel

@@ -6,7 +6,7 @@
 
 namespace bem {
 
-size_t g_device_bytes = 0;
+std::atomic<size_t> g_device_bytes{0};
 
 // ------------------------------------------------------------------ scan
 constexpr int SCAN_THREADS = 256;

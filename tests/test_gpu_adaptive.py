@@ -96,10 +96,14 @@ def test_adaptive_tree_on_a_strongly_non_uniform_cloud():
         ctx.bem_apply(m, None, y)
         st = ctx.bem_get_stats()
         ctx.bem_destroy()
-        res[tree] = (_rel(y[rows], yo), st["p2p_pairs"], st["lmax"])
-        print(f"tree {tree}: error {res[tree][0]:.2e}, point pairs {st['p2p_pairs']:.3e}, lmax {st['lmax']:.0f}, m2l pairs {st['m2l_pairs']:.0f}")
+        res[tree] = (_rel(y[rows], yo), st["p2p_pairs"], st["lmax"], st["p2p_pairs_wx"])
+        print(f"tree {tree}: error {res[tree][0]:.2e}, point pairs {st['p2p_pairs']:.3e} (W/X ranges {st['p2p_pairs_wx']:.3e}), "
+              f"lmax {st['lmax']:.0f}, m2l pairs {st['m2l_pairs']:.0f}, m2m pairs {st['m2m_pairs']:.0f} -> {st['m2m_parents']:.0f} parents")
+        assert 0 < st["m2m_parents"] <= st["m2m_pairs"] <= 8 * st["m2m_parents"]
     assert res[0][0] <= 1e-5 and res[1][0] <= 1e-5
     assert res[1][1] < 0.2 * res[0][1] and res[1][2] > res[0][2]
+    # BEM_S_P2P_PAIRS_WX: the uniform tree has no W or X list; a graded cloud must have both, and they are part of the direct pairs
+    assert res[0][3] == 0 and 0 < res[1][3] < res[1][1]
 
 
 def test_adaptive_tree_evaluator_and_refusals():
