@@ -11,6 +11,9 @@ CUDA library, and only tests/ and bench.py's cpu legs import it.
                     (n x v)_j = 1/(3 s_j) sum_{k ni j} (n x v)_k A_k                                            (Eq. 27)
   filter_matrix     Eqs. 37-42: F = G (G* G)^-1 G*, G_ij = Y_j(theta_i, phi_i), j = (n, m), n < p_f
   filter_apply      Eqs. 41, 43: xhat_l = F x_l for every bubble l and every surface function
+  bubble_volumes    V_m of the polytropic gas law (Eq. 6; "volume" among the surface functions of PAPER.md:612):
+                    the volume enclosed by the flat-triangle surface of bubble m, by the divergence theorem with the field r/3:
+                    V_m = 1/3 sum_{k in bubble m} A_k N_k . c_k  (c_k the centroid; r . N is constant on a flat triangle)
 
 Parity pinned by tests/test_oracle_pins.py (closed forms on the sphere, projector identities).
 """
@@ -37,6 +40,23 @@ def vertex_geometry(V, F):
         np.add.at(m, F[:, a], Ntri * A[:, None])
     n = m / np.linalg.norm(m, axis=1)[:, None]
     return s, n, A, Ntri
+
+
+def bubble_volumes(V, F, bubble_id=None):
+    """V_m = 1/3 sum_k A_k N_k . c_k over the triangles of bubble m (divergence theorem, F = r/3; N_k points out of the
+    bubble).  The paper prints no formula for V_m (it only uses it in the gas law); for a
+    closed flat-triangle surface this is its definition written out.  Returns [n_bubbles]."""
+    V = np.asarray(V, dtype=np.float64)
+    F = np.asarray(F, dtype=np.int64)
+    _, _, A, Ntri = vertex_geometry(V, F)
+    cen = (V[F[:, 0]] + V[F[:, 1]] + V[F[:, 2]]) / 3.0
+    contrib = A * np.einsum("kd,kd->k", Ntri, cen) / 3.0
+    if bubble_id is None:
+        return np.array([contrib.sum()])
+    b = np.asarray(bubble_id, dtype=np.int64)[F[:, 0]]
+    vol = np.zeros(int(b.max()) + 1)
+    np.add.at(vol, b, contrib)
+    return vol
 
 
 def surface_velocity(V, F, phi, q):

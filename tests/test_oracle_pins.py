@@ -585,3 +585,44 @@ def test_s5_mean_curvature_paraboloid_fit():
     c, s = np.cos(0.7), np.sin(0.7)
     Rm = np.array([[c, -s, 0], [s, c, 0], [0, 0, 1.0]]) @ np.array([[1, 0, 0], [0, c, -s], [0, s, c]])
     assert np.max(np.abs(so.mean_curvature(V, f) - so.mean_curvature(V @ Rm.T, f))) < 1e-10
+
+
+def test_s6_bubble_volumes_closed_forms():
+    """V_m of the gas law: exact volumes of polyhedra with a closed form (regular tetrahedron
+    a^3 / (6 sqrt 2), unit cube cut into 12 triangles), invariance under translation (the sum is origin-free only because
+    the surface is closed: a dropped triangle or a flipped normal breaks it), scaling by s^3, the sphere 4 pi R^3 / 3 from
+    below at O(h^2), and two bubbles kept apart by bubble_id."""
+    # regular tetrahedron with edge a = 2 sqrt 2: vertices at alternate corners of the cube [-1, 1]^3
+    Vt = np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], float)
+    Ft = np.array([[0, 1, 2], [0, 3, 1], [0, 2, 3], [1, 3, 2]])
+    if so.bubble_volumes(Vt, Ft)[0] < 0:                     # make the triangles counter-clockwise seen from outside
+        Ft = Ft[:, ::-1]
+    a = 2 * np.sqrt(2.0)
+    assert abs(so.bubble_volumes(Vt, Ft)[0] - a ** 3 / (6 * np.sqrt(2.0))) <= 1e-14 * 3
+    assert abs(so.bubble_volumes(Vt[:, ::-1] * 1.0, Ft)[0] + a ** 3 / (6 * np.sqrt(2.0))) <= 1e-14 * 3      # mirror image: orientation flips the sign
+    # unit cube, outward orientation
+    Vc = np.array([[x, y, z] for x in (0, 1) for y in (0, 1) for z in (0, 1)], float)
+    quads = [(0, 1, 3, 2), (4, 6, 7, 5), (0, 4, 5, 1), (2, 3, 7, 6), (0, 2, 6, 4), (1, 5, 7, 3)]
+    Fc = np.array([t for (p, q, r, s) in quads for t in ((p, q, r), (p, r, s))])
+    vol = so.bubble_volumes(Vc, Fc)[0]
+    assert abs(abs(vol) - 1.0) <= 1e-15
+    if vol < 0:
+        Fc = Fc[:, ::-1]
+    shift = np.array([13.0, -7.5, 4.25])
+    assert abs(so.bubble_volumes(Vc + shift, Fc)[0] - 1.0) <= 1e-12
+    assert abs(so.bubble_volumes(2.5 * Vc, Fc)[0] - 2.5 ** 3) <= 1e-13
+    # sphere: inscribed polyhedron, error O(h^2)
+    R, err = 1.3, []
+    for lvl in (2, 3, 4):
+        v, f = bi.icosphere(lvl)
+        err.append(1.0 - so.bubble_volumes(R * v, f)[0] / (4 * np.pi * R ** 3 / 3))
+    assert all(e > 0 for e in err) and 3.5 < err[0] / err[1] < 4.5 and 3.5 < err[1] / err[2] < 4.5 and err[2] < 3e-3
+    # two bubbles of different size in one mesh
+    v, f = bi.icosphere(2)
+    n = v.shape[0]
+    V2 = np.vstack([v + [5, 0, 0], 0.5 * v - [0, 3, 0]])
+    F2 = np.vstack([f, f + n])
+    bid = np.r_[np.zeros(n, int), np.ones(n, int)]
+    v2 = so.bubble_volumes(V2, F2, bid)
+    v1 = so.bubble_volumes(v, f)[0]
+    assert v2.shape == (2,) and abs(v2[0] - v1) <= 1e-12 and abs(v2[1] - v1 / 8) <= 1e-13
