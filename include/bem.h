@@ -318,6 +318,16 @@ bem_status bem_surface_velocity(bem_ctx *ctx, const double *phi, const double *q
  * or the system is singular.  H: [n_vertices], host or device. */
 bem_status bem_surface_curvature(bem_ctx *ctx, double *H);
 
+/* bem_bubble_volume -- V_m, the volume of every bubble: what the polytropic gas law needs each time step
+ * (p_g = p_g0 (V_m0 / V_m)^kappa) and the "volume" among the surface functions of PAPER.md:612.  It is
+ * the volume enclosed by the bubble's flat triangles (exact for the polyhedron; 4 pi R^3 / 3 (1 - O(h^2)) on a sphere).
+ * A triangle belongs to the bubble of its first vertex (bem_create refuses triangles that join two bubbles).
+ *   vol_out    [n_bubbles] fp64, host or device; n_bubbles must equal the mesh's bubble count (largest id + 1, or 1
+ *              when bem_create got no ids), else BEM_ERR_INVALID_ARG.
+ * Needs no bem_setup.  The grouping of triangles by bubble is built at the first call and kept.  Fixed summation
+ * order: repeated calls return the same bits. */
+bem_status bem_bubble_volume(bem_ctx *ctx, double *vol_out, int64_t n_bubbles);
+
 /* Shape filter of bandwidth p_f (Eqs. 34-43): every bubble surface is a map of the unit sphere, the
  * mesh points keep their spherical angles (theta_i, phi_i) for all times, and a surface function sampled at them is
  * replaced by its least-squares fit with the spherical harmonics of degree n < p_f,

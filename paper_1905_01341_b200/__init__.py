@@ -31,7 +31,7 @@ STAT_NAMES = ["n_targets", "n_sources", "lmax", "n_src_leaves", "n_tgt_leaves", 
 # every symbol include/bem.h declares
 EXPORTS = ["bem_create", "bem_create_points", "bem_create_evaluator", "bem_set_option", "bem_set_stream", "bem_setup", "bem_apply", "bem_solve", "bem_get_timings",
            "bem_get_stats", "bem_get_free_term", "bem_fp64_peak", "bem_fp64_tensor_peak", "bem_last_error", "bem_destroy",
-           "bem_surface_velocity", "bem_surface_curvature", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy",
+           "bem_surface_velocity", "bem_surface_curvature", "bem_bubble_volume", "bem_filter_create", "bem_filter_apply", "bem_filter_last_error", "bem_filter_destroy",
            "bem_direct_sum_static", "bem_direct_sum_static_last_error"]
 DIRECT_STATIC_MAX_TARGETS = 65536      # BEM_DIRECT_STATIC_MAX_TARGETS of include/bem.h
 
@@ -74,6 +74,7 @@ def load_library() -> ctypes.CDLL:
     lib.bem_destroy.restype = None
     lib.bem_surface_velocity.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.bem_surface_curvature.argtypes = [vp, vp]
+    lib.bem_bubble_volume.argtypes = [vp, vp, i64]
     lib.bem_filter_create.argtypes = [vp, vp, i64, i32, ctypes.POINTER(vp)]
     lib.bem_filter_apply.argtypes = [vp, vp, i64, vp, vp]
     lib.bem_filter_last_error.argtypes = [vp]
@@ -211,6 +212,12 @@ class Bem:
         """Mean curvature by the fitted paraboloid (Eqs. 28-29); H: [n_vertices] output."""
         self._check(self._lib.bem_surface_curvature(self._ctx, _ptr(H)))
         return H
+
+    def bem_bubble_volume(self, vol_out):
+        """vol_out [n_bubbles] <- V_m of every bubble; host or device float64."""
+        n = vol_out.numel() if hasattr(vol_out, "numel") else vol_out.size
+        self._check(self._lib.bem_bubble_volume(self._ctx, _ptr(vol_out), int(n)))
+        return vol_out
 
     def bem_destroy(self):
         if self._ctx:

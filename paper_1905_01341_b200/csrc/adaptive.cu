@@ -488,6 +488,7 @@ void build_adaptive(bem_ctx *c)
     KERNEL_CHECK();
     int longest = 0;
     d2h_sync(&longest, mx.get(), sizeof(int), s);
+    ad.row_overflow = longest > SEG_MAX;                           // bem_setup tries once more without the direct far pairs (api.cu)
     if (longest > SEG_MAX)
         throw Error(BEM_ERR_INVALID_ARG, "adaptive tree: a target leaf has more than 256 direct source ranges (raise leaf_size or lower direct_pairs)");
     ad.near_rng.alloc(nseg);

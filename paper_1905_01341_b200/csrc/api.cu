@@ -405,8 +405,21 @@ static void setup_impl(bem_ctx *c, int p, int leaf_size, double eta)
             const double w = 800.0 * (double)c->nre * (double)c->nre / 6400.0;
             c->direct_max_eff = c->direct_max >= 0 ? c->direct_max : (int64_t)w;
         }
-        if (c->adaptive) build_adaptive(c);
-        else build_lists(c);
+        if (c->adaptive) {
+            try {
+                build_adaptive(c);
+            } catch (const Error &) {
+                // A target leaf met more direct source ranges than the pair kernel's segment table holds (SEG_MAX).  With a small
+                // leaf_size the cost model above moves up to 189 leaf-level far pairs per leaf from the M2L list to the direct
+                // list, which leaves few slots for the coarser leaves next to the ancestors of a leaf in a strongly graded
+                // cloud.  When that choice was the library's (direct_pairs = -1), build the lists again with every far pair
+                // translated: a row then holds at most the 27 neighbours of the leaf and of each ancestor.  An explicit
+                // direct_pairs is the caller's to lower: the refusal stands.
+                if (!c->ad.row_overflow || c->direct_max >= 0 || c->direct_max_eff == 0) throw;
+                c->direct_max_eff = 0;
+                build_adaptive(c);
+            }
+        } else build_lists(c);
         pack_scratch(c);
         for (int i = 0; i < c->n_lay; ++i) layout_stats(c, c->lay[i]);
         activate_layout(c, 0);

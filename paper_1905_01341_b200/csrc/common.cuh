@@ -194,6 +194,7 @@ struct Adaptive {
     dvec<int32_t> near_ptr;                                     // [n_tleaf + 1] CSR of the direct source ranges of a target leaf
     dvec<int2> near_rng;                                        // (first source, count)
     dvec<int32_t> x_ptr[MAX_LEVEL + 1], x_src[MAX_LEVEL + 1];   // far pairs of two sparse leaves, summed directly (per level)
+    bool row_overflow = false;                                  // the last build met a target leaf with more than SEG_MAX direct ranges
 };
 
 // Everything bem_setup builds that depends on the truncation number.  A context holds one layout for the products without
@@ -237,6 +238,9 @@ struct bem_ctx {
     // vertex -> incident triangle corners, sorted by vertex (bem_surface_velocity; built at first use)
     bem::dvec<int32_t> vc_begin;    // [N+1]
     bem::dvec<uint32_t> vc_corner;  // [3T] corner index 3 k + a, in mesh order within a vertex
+    // triangles grouped by bubble (bem_bubble_volume; built at first use)
+    bem::dvec<int32_t> bv_begin;    // [nbubbles+1]
+    bem::dvec<uint32_t> bv_tri;     // [T] triangle indices, mesh order within a bubble
 
     // options
     // quadrature: 0 = G3, 1 = V1, 2 = point cloud (bem_create_points), 3 = evaluator of a mesh context off its surface

@@ -147,6 +147,60 @@ __global__ void surface_curvature_kernel(const double *__restrict__ V, const int
     H[j] = -B[2] - B[4];                                               // Eq. 29
 }
 
+// ------------------------------------------------------------------ bubble volumes (PAPER.md:108-115 gas law; "volume")
+__global__ void bv_keys(const int32_t *F, const int32_t *bid, int64_t T, uint64_t *keys)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < T) keys[k] = bid ? (uint64_t)bid[F[3 * k]] : 0ull;
+}
+
+// One warp per bubble.  V_m = sum_k (r_k1 - o).((r_k2 - o) x (r_k3 - o)) / 6 over the bubble's triangles -- the signed
+// tetrahedra from a point o to every outward-oriented triangle of a closed surface; o = the first vertex of the bubble's
+// first triangle, so that a bubble far from the origin loses no digits.  Lane l adds triangles l, l + 32, ... in mesh order,
+// then a shuffle tree: the same bits on every call.
+__global__ void bubble_volume_kernel(const double *__restrict__ V, const int32_t *__restrict__ F, const int32_t *__restrict__ begin,
+                                     const uint32_t *__restrict__ tri, int nb, double *__restrict__ vol)
+{
+    const int b = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+    if (b >= nb) return;
+    const int i0 = begin[b], i1 = begin[b + 1];
+    double acc = 0.0;
+    if (i1 > i0) {
+        const int64_t vo = F[3 * (int64_t)tri[i0]];
+        const double ox = V[3 * vo], oy = V[3 * vo + 1], oz = V[3 * vo + 2];
+        for (int i = i0 + lane; i < i1; i += 32) {
+            const int64_t k = tri[i];
+            const int64_t a = F[3 * k], bb = F[3 * k + 1], c = F[3 * k + 2];
+            const double ax = V[3 * a] - ox, ay = V[3 * a + 1] - oy, az = V[3 * a + 2] - oz;
+            const double bx = V[3 * bb] - ox, by = V[3 * bb + 1] - oy, bz = V[3 * bb + 2] - oz;
+            const double cx = V[3 * c] - ox, cy = V[3 * c + 1] - oy, cz = V[3 * c + 2] - oz;
+            acc += ax * (by * cz - bz * cy) + ay * (bz * cx - bx * cz) + az * (bx * cy - by * cx);
+        }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+    if (lane == 0) vol[b] = acc / 6.0;
+}
+
+static void build_bubble_triangles(bem_ctx *c)
+{
+    if (c->bv_begin.p && c->bv_begin.n == (size_t)c->nbubbles + 1) return;
+    cudaStream_t s = c->stream;
+    const int64_t T = c->T;
+    dvec<uint64_t> keys, keys_tmp;
+    dvec<uint32_t> vals_tmp;
+    keys.alloc(T); keys_tmp.alloc(T); vals_tmp.alloc(T);
+    c->bv_tri.alloc(T);
+    c->bv_begin.alloc(c->nbubbles + 1);
+    bv_keys<<<cdiv(T, 256), 256, 0, s>>>(c->F.get(), c->bid.p, T, keys.get());
+    KERNEL_CHECK();
+    iota_u32(c->bv_tri.get(), T, s);
+    if (c->nbubbles > 1) radix_sort_pairs(keys.get(), c->bv_tri.get(), keys_tmp.get(), vals_tmp.get(), T, 0, 32, s);   // stable
+    sv_vertex_ranges<<<cdiv(T + 1, 256), 256, 0, s>>>(keys.get(), T, c->nbubbles, c->bv_begin.get());
+    KERNEL_CHECK();
+    CUDA_TRY(cudaStreamSynchronize(s));
+}
+
 // ------------------------------------------------------------------ shape filter
 }  // namespace bem
 
@@ -446,6 +500,42 @@ bem_status bem_surface_curvature(bem_ctx *c, double *H)
         KERNEL_CHECK();
         if (ph != H) {
             CUDA_TRY(cudaMemcpyAsync(H, ph, N * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            CUDA_TRY(cudaStreamSynchronize(c->stream));
+        }
+        return BEM_OK;
+    } catch (const Error &e) {
+        c->err = e.what();
+        cudaGetLastError();
+        return e.status;
+    } catch (const std::bad_alloc &) {
+        return BEM_ERR_OOM;
+    } catch (const std::exception &) {
+        cudaGetLastError();
+        return BEM_ERR_CUDA;                                  // nothing may cross the extern "C" boundary
+    } catch (...) {
+        return BEM_ERR_CUDA;
+    }
+}
+
+bem_status bem_bubble_volume(bem_ctx *c, double *vol_out, int64_t n_bubbles)
+{
+    if (!c || !vol_out) return BEM_ERR_INVALID_ARG;
+    if (c->quadrature >= 2 || c->T == 0) { c->err = "bem_bubble_volume: the context holds no mesh"; return BEM_ERR_INVALID_ARG; }
+    if (n_bubbles != c->nbubbles) {
+        c->err = "bem_bubble_volume: n_bubbles must be the number of bubbles of the mesh (largest bubble id + 1; 1 without ids): " + std::to_string(c->nbubbles);
+        return BEM_ERR_INVALID_ARG;
+    }
+    try {
+        CUDA_TRY(cudaSetDevice(c->device));
+        build_bubble_triangles(c);
+        const int nb = c->nbubbles;
+        dvec<double> dv;
+        double *pv = vol_out;
+        if (!is_device_ptr(vol_out)) { dv.alloc(nb); pv = dv.get(); }
+        bubble_volume_kernel<<<cdiv((int64_t)nb * 32, 128), 128, 0, c->stream>>>(c->V.get(), c->F.get(), c->bv_begin.get(), c->bv_tri.get(), nb, pv);
+        KERNEL_CHECK();
+        if (pv != vol_out) {
+            CUDA_TRY(cudaMemcpyAsync(vol_out, pv, nb * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
             CUDA_TRY(cudaStreamSynchronize(c->stream));
         }
         return BEM_OK;

@@ -174,3 +174,34 @@ def test_surface_curvature_matches_oracle(case):
     torch.cuda.synchronize()
     assert np.array_equal(hd.cpu().numpy(), H)
     ctx.bem_destroy()
+
+
+def test_bubble_volume_matches_oracle():
+    """bem_bubble_volume against oracle bubble_volumes: a cluster of 40 polydisperse bubbles in a
+    cube of side 40 (far from the origin: the kernel sums tetrahedra from a vertex of the bubble, the oracle uses
+    A_k N_k . c_k / 3 about the origin -- different formulas, both exact for the polyhedron), a single mesh without
+    ids, host and device outputs, the same bits on a second call, and the size check."""
+    import torch
+    bem = _bem()
+    c = make_config(4, n_bubbles=40)
+    V, F, bid = c["V"], c["F"], c["bubble_id"]
+    ctx = bem.bem_create(V, F, bid)
+    nb = int(bid.max()) + 1
+    vo = so.bubble_volumes(V, F, bid)
+    vh = np.full(nb, np.nan)
+    ctx.bem_bubble_volume(vh)
+    assert _maxrel(vh, vo) <= 1e-12 and (vh > 0).all()
+    vd = torch.full((nb,), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.bem_bubble_volume(vd)
+    assert np.array_equal(vd.cpu().numpy(), vh)
+    with pytest.raises(bem.BemError):
+        ctx.bem_bubble_volume(np.zeros(nb + 1))
+    ctx.bem_destroy()
+    # one bubble, no ids, shifted off the origin: translation must not cost digits
+    v, f = bi.icosphere(4)
+    ctx = bem.bem_create(0.7 * v + np.array([100.0, -50.0, 25.0]), f, None)
+    one = np.zeros(1)
+    ctx.bem_bubble_volume(one)
+    assert abs(one[0] - so.bubble_volumes(0.7 * v, f)[0]) <= 1e-12 * one[0]
+    assert 0.99 < one[0] / (4 * np.pi * 0.7 ** 3 / 3) < 1.0
+    ctx.bem_destroy()
