@@ -208,6 +208,12 @@ bem_status bem_create_evaluator(bem_ctx *mesh_ctx, const double *targets, int64_
  *                   join sparsely filled boxes (the balance of A^(dense) and A^(sparse), per pair).
  *                   -1 = 800 (nre / 80)^2 from the measured costs (default), 0 = off (the uniform lists of
  *                   PAPER.md:440).  Direct pairs are exact, so the error can only fall.
+ *                   Adaptive tree: the pair kernel holds at most 256 direct source ranges per target leaf (27 of the own
+ *                   level, the coarser leaves next to its ancestors, up to 189 direct far pairs).  When a leaf exceeds
+ *                   that and direct_pairs is -1, bem_setup rebuilds the lists with every far pair translated; with an
+ *                   explicit direct_pairs > 0 it returns BEM_ERR_INVALID_ARG (lower it, or raise leaf_size).
+ *   "max_direct_ranges"  1..256 (default 256): lowers that limit (a test hook for the rebuild above; no reason to set it
+ *                   otherwise).
  *   "graph"         1 (default): bem_apply with DEVICE pointers q, phi, y on a stream other than the legacy default stream is
  *                   captured into a CUDA graph the second time the same (q, phi, y) is asked for and replayed from then
  *                   on -- one launch instead of 20-40 on the launch-bound small meshes.  Any bem_set_option,

@@ -488,9 +488,11 @@ void build_adaptive(bem_ctx *c)
     KERNEL_CHECK();
     int longest = 0;
     d2h_sync(&longest, mx.get(), sizeof(int), s);
-    ad.row_overflow = longest > SEG_MAX;                           // bem_setup tries once more without the direct far pairs (api.cu)
-    if (longest > SEG_MAX)
-        throw Error(BEM_ERR_INVALID_ARG, "adaptive tree: a target leaf has more than 256 direct source ranges (raise leaf_size or lower direct_pairs)");
+    const int limit = std::min(c->seg_limit, (int)SEG_MAX);
+    ad.row_overflow = longest > limit;                             // bem_setup tries once more without the direct far pairs (api.cu)
+    if (longest > limit)
+        throw Error(BEM_ERR_INVALID_ARG, "adaptive tree: a target leaf has " + std::to_string(longest) + " direct source ranges, more than the " +
+                                         std::to_string(limit) + " the pair kernel's table holds (raise leaf_size or lower direct_pairs)");
     ad.near_rng.alloc(nseg);
     near_lists<<<cdiv(ad.n_tleaf, 128), 128, 0, s>>>(ad.tleaf_gbox.get(), ad.tleaf_begin.get(), ad.n_tleaf, L, nullptr, ad.near_ptr.get(),
                                                      ad.near_rng.get(), pc.get(), pc.get() + 1, pc.get() + 2);

@@ -675,6 +675,7 @@ bem_status bem_set_option(bem_ctx *c, const char *key, double value)
         // inside a stream capture of the caller, where an allocation is not allowed
         if (v == 1 && c->ready && c->mode == 0 && !c->adaptive) return guarded(c, [&]() { ensure_p2p_f32(c); CUDA_TRY(cudaStreamSynchronize(c->stream)); });
     }
+    else if (!strcmp(key, "max_direct_ranges")) { if (v < 1 || v > 256) return BEM_ERR_INVALID_ARG; c->seg_limit = v; c->ready = false; }
     else if (!strcmp(key, "direct_pairs")) { if (value < -1 || value > 1e9) return BEM_ERR_INVALID_ARG; c->direct_max = (int64_t)value; c->ready = false; }
     else if (!strcmp(key, "p2p_ctas")) { if (v < 0 || v > 16) return BEM_ERR_INVALID_ARG; c->p2p_ctas = v; }
     else if (!strcmp(key, "m2l_order_radius")) { if (!(value >= 0 && value < 1.0)) return BEM_ERR_INVALID_ARG; c->m2l_order_radius = value; c->ready = false; }

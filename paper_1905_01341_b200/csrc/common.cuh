@@ -295,6 +295,8 @@ struct bem_ctx {
     int64_t xdir_pairs = 0;
     int64_t direct_max = -1;        // option "direct_pairs": nt x ns threshold, -1 = from the cost model, 0 = off
     int64_t direct_max_eff = 0;
+    int seg_limit = 256;            // option "max_direct_ranges": longest row of direct source ranges a target leaf of the adaptive tree may
+                                    // have (<= SEG_MAX of segments.cuh, the pair kernel's segment table)
     bem::dptr<double> mats;         // views of the active layout (FmmLayout)
     bem::dptr<double2> rot;
     bem::dptr<int32_t> kinfo, mat_ne, mat_cls, mat_w;

@@ -233,3 +233,50 @@ def test_degenerate_inputs_both_trees():
         ctx.bem_apply(np.array([2.0]), np.array([[0.1, -0.2, 0.3]]), y)
         ctx.bem_destroy()
         assert _rel(y, yo) <= 1e-6, (tree, _rel(y, yo))
+
+
+def test_adaptive_tree_row_overflow_rebuilds_without_direct_far_pairs():
+    """include/bem.h, option "direct_pairs": a target leaf of the adaptive tree may hold at most max_direct_ranges (256)
+    direct source ranges.  Lower the limit until the library's own choice of direct far pairs no longer fits: an explicit
+    direct_pairs is then refused, the default (-1) rebuilds the lists with every far pair translated -- the same lists as
+    direct_pairs = 0 -- and still meets the tolerance."""
+    bem = _bem()
+    rng = np.random.default_rng(78)
+    n = 30000
+    dense = 0.5 + 0.005 * rng.normal(size=(int(0.9 * n), 3))
+    pts = np.vstack([dense, rng.uniform(0, 1, size=(n - dense.shape[0], 3))])
+    m = rng.uniform(-1, 1, size=n)
+    rows = np.sort(rng.choice(n, 200, replace=False))
+    yo = oracle.monopole_sum(pts, m, pts[rows])
+
+    def run(direct_pairs, limit):
+        ctx = bem.bem_create_points(pts, pts)
+        ctx.bem_set_option("tree", 1)
+        ctx.bem_set_option("direct_pairs", direct_pairs)
+        ctx.bem_set_option("max_direct_ranges", limit)
+        try:
+            ctx.bem_setup(12, 8, 2.5)
+            y = np.full(n, np.nan)
+            ctx.bem_apply(m, None, y)
+            return _rel(y[rows], yo), ctx.bem_get_stats()
+        finally:
+            ctx.bem_destroy()
+
+    found = False
+    for limit in (200, 160, 120, 90, 70, 50, 40):
+        try:
+            e0, st0 = run(0, limit)
+        except bem.BemError:
+            break                                            # even the plain lists no longer fit: nothing below will
+        try:
+            run(800, limit)
+            continue                                         # the direct far pairs still fit under this limit
+        except bem.BemError as ex:
+            assert ex.status == bem.BEM_ERR_INVALID_ARG and "direct source ranges" in str(ex)
+        e, st = run(-1, limit)
+        print(f"limit {limit}: rebuilt, error {e:.2e}, m2l pairs {st['m2l_pairs']:.0f} (direct_pairs = 0: {st0['m2l_pairs']:.0f})")
+        assert e <= 1e-5 and e0 <= 1e-5
+        assert st["m2l_pairs"] == st0["m2l_pairs"] and st["p2p_pairs"] == st0["p2p_pairs"]
+        found = True
+        break
+    assert found, "no limit separated the lists with and without direct far pairs"
