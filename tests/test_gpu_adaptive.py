@@ -208,6 +208,11 @@ def test_degenerate_inputs_both_trees():
             y = np.full(4, np.nan)
             ctx.bem_apply(q, ph, y)
             ctx.bem_destroy()
+            # FMM tolerance 1e-4, not the north_star's 1e-5: this mesh is set up at p = 6 (S - D then runs at 9, R5'), below every
+            # stated p of BASELINE.json (8 / 10 / 12) -- the bound is Table 1's p = 8 column relaxed by the missing degrees
+            # (DESIGN.md section 3 R5': about one digit per 2.5 degrees), and with 12 sources at leaf_size 1 nearly every
+            # pair is a far pair, so the product IS the truncation error.  What the case checks is that a 4-vertex mesh
+            # builds a tree and lists at all; accuracy at the stated p is tests/test_gpu_parity.py's.
             assert _rel(y, yo) <= (1e-12 if mode else 1e-4), (tree, mode, _rel(y, yo))
     rng = np.random.default_rng(9)
     src = rng.uniform(0, 1, size=(500, 3))
